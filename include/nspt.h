@@ -1,0 +1,152 @@
+/*
+ * nspt.h -- C ABI of libnspt: the FFT-based convolution (FFT-CONV) star-product of truncated
+ * perturbative series with dense N x N complex128 matrix coefficients, and the TEK staple
+ * built from it, for one NVIDIA B200 (sm_100a).
+ *
+ * Source of every definition: Gonzalez-Arroyo et al., "Towards higher order numerical
+ * stochastic perturbation computation applied to the twisted Eguchi-Kawai model"
+ * (arXiv:2001.02835), cited below as PAPER.md:<line> (section / equation).
+ *
+ * ---------------------------------------------------------------------------------------
+ * Series layout (all entry points).  A polynomial matrix truncated at O(g^Ntrunc)
+ *     X = sum_{k=0}^{Ntrunc} g^k X^(k)                     (eq. 2.4)
+ * is an array of n = Ntrunc+1 row-major N x N matrices of nspt_c128, order index slowest:
+ *     X[(k*N + i)*N + j] = X^(k)_{ij},   k = 0..Ntrunc,  i, j = 0..N-1,
+ * contiguous, n*N*N elements, 16-byte aligned.  nspt_c128 is layout-identical to C
+ * `double _Complex`, cuDoubleComplex and torch.complex128.
+ *
+ * Pointers.  Entry points WITHOUT the _host suffix take DEVICE pointers valid on the
+ * current CUDA device; they enqueue kernels on the library stream (nspt_set_stream) and
+ * return without synchronising.  Entry points WITH the _host suffix take HOST pointers
+ * (pinned memory recommended), copy host->device, run the same kernels, copy device->host
+ * and synchronise the stream before returning.  The twist tensor z is always a HOST array.
+ *
+ * Ownership.  The caller owns every array it passes; the library keeps no caller pointer
+ * past the stream-ordered work of the call.  Library-owned state (plan tables, the internal
+ * frequency-domain workspace, staging buffers of the _host calls) is released by nspt_release.
+ *
+ * Aliasing.  The output of nspt_series_mul[_batched] may be exactly one of its inputs (all
+ * inputs are transformed into the workspace before any output is written); partial overlap
+ * is undefined.  In nspt_staple S[mu] may alias U[mu] for the same reason.
+ *
+ * Errors.  Every call returns 0 (NSPT_OK) or a negative code; nothing throws, aborts or
+ * prints.  Kernel faults are asynchronous and surface at the caller's next synchronisation.
+ *
+ * Threads.  The library has one process-wide context guarded by a mutex; calls from several
+ * host threads are serialised.
+ * ---------------------------------------------------------------------------------------
+ */
+#ifndef NSPT_H
+#define NSPT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct { double re, im; } nspt_c128;
+
+enum {
+    NSPT_OK = 0,
+    NSPT_EINVAL = -1,  /* null / misaligned pointer, N < 1, Ntrunc < 0, batch < 1, transform length > 256 */
+    NSPT_ENOMEM = -2,  /* device or host allocation failed, or caller workspace too small */
+    NSPT_ECUDA = -3,   /* CUDA runtime / launch error (text: nspt_strerror) */
+    NSPT_EARCH = -4    /* current device is not compute capability 10.x */
+};
+
+enum { NSPT_OP_SERIES_MUL = 0, NSPT_OP_STAPLE = 1 };
+
+/* Largest supported truncation order: the transform length L = smallest power of two
+ * >= 2*Ntrunc+1 must be <= 256 (Ntrunc <= 127; the paper uses Ntrunc <= 63). */
+#define NSPT_MAX_NTRUNC 127
+
+/*
+ * C = A * B, the convolution product truncated at O(g^Ntrunc):
+ *     C^(k) = sum_{l=0}^{k} A^(l) B^(k-l),  k = 0..Ntrunc     (eq. 2.5)
+ * with the left factor always from A.  Computed by FFT-CONV (Steps 1-5,
+ * eqs. 2.6-2.9): zero-padded forward transforms of length L along the order index for every
+ * matrix element, one N x N complex matrix product per Fourier mode, inverse transform with
+ * 1/L, orders above Ntrunc discarded.  L = smallest power of two >= 2*Ntrunc+1 (= 2*N_p of
+ * the paper when Ntrunc = N_p - 1 = 2^s - 1); any Ntrunc in [0, 127] is accepted.
+ * A, B, C: device pointers, (Ntrunc+1)*N*N elements each.
+ */
+int nspt_series_mul(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc);
+
+/*
+ * batch independent products C_b = A_b * B_b (e.g. the four P_mu * U_mu of the link update,
+ * PAPER.md:50, eq. 2.3; batching of independent transforms / products: PAPER.md:106).
+ * Operand b starts at element offset b*(Ntrunc+1)*N*N.  Device pointers.
+ */
+int nspt_series_mul_batched(const nspt_c128* A, const nspt_c128* B, nspt_c128* C,
+                            int N, int Ntrunc, int batch);
+
+/*
+ * The TEK staple for all four directions (eq. 2.3; eq. 2.2):
+ *     S_mu = U_mu * [ sum_{nu != mu} ( z_{mu nu}   U_nu  * U_mu^+ * U_nu^+
+ *                                    - z_{mu nu}^* U_nu^+ * U_mu^+ * U_nu ) ],  mu = 0..3,
+ * every * truncated at O(g^Ntrunc); X^+ is the coefficient-wise conjugate transpose.
+ * U[4], S[4]: HOST arrays of four DEVICE pointers to series of (Ntrunc+1)*N*N elements.
+ * z: HOST 4x4 row-major array, z[4*mu+nu] = z_{mu nu}; the diagonal is ignored and the
+ * second term uses conj(z[4*mu+nu]) exactly as the equation prints it.  z is not checked
+ * for antisymmetry or unit modulus.
+ */
+int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4],
+                int N, int Ntrunc);
+
+/* Host-buffer forms of the three calls above: same semantics, HOST pointers for the series,
+ * host<->device copies on the library stream inside the call, stream synchronised on return. */
+int nspt_series_mul_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc);
+int nspt_series_mul_batched_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C,
+                                 int N, int Ntrunc, int batch);
+int nspt_staple_host(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4],
+                     int N, int Ntrunc);
+
+/* ------------------------------------------------------------------------- context calls */
+
+/* CUDA stream (a cudaStream_t passed as void*) all later calls enqueue on.  Default: the
+ * legacy default stream (NULL). */
+int nspt_set_stream(void* cuda_stream);
+
+/* Optional magnitude balancing: coefficient k is multiplied by s^k before the forward
+ * transform and the result by s^-k after the inverse one; exact in exact arithmetic because
+ * (s^l)(s^(k-l)) = s^k.  s = 1 (default) switches it off.  s must be finite and > 0. */
+int nspt_set_order_scale(double s);
+
+/* Bytes of device workspace a call needs (op = NSPT_OP_SERIES_MUL with its batch, or
+ * NSPT_OP_STAPLE, batch ignored). */
+int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out);
+
+/* Give the library a caller-owned device workspace (256-byte aligned).  Calls that need more
+ * return NSPT_ENOMEM.  Pass (NULL, 0) to go back to the library-owned, grow-only workspace. */
+int nspt_set_workspace(void* dptr, size_t bytes);
+
+/* Select the mode-wise matrix product kernel: 0 = reference kernel (one thread per output
+ * element, plain double FMAs; for debugging), 1 = tensor-core kernel (DMMA, TMA-fed,
+ * 3-multiplication complex product; default). */
+int nspt_set_gemm_variant(int variant);
+
+/* Per-stage device timing.  After nspt_profile(1) every kernel the library launches is
+ * bracketed by CUDA events on the library stream; nspt_profile_read synchronises the stream,
+ * and for stage = 0 forward transforms, 1 mode-wise matrix products, 2 inverse transforms,
+ * 3 re-truncation transforms, 4 other (dagger / copies) returns the summed milliseconds and
+ * the number of launches since the last read, then resets the counters. */
+int nspt_profile(int enable);
+int nspt_profile_read(int stage, double* ms, long long* launches);
+
+/* Total kernels launched by the library since it was loaded. */
+long long nspt_launch_count(void);
+
+/* Free all library-owned device / host memory and cached plans. */
+int nspt_release(void);
+
+/* Text for an error code; for NSPT_ECUDA the text of the last CUDA error seen. */
+const char* nspt_strerror(int code);
+
+/* Version: major*10000 + minor*100 + patch. */
+int nspt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NSPT_H */

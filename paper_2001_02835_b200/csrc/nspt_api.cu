@@ -1,0 +1,507 @@
+// nspt_api.cu -- the C ABI of libnspt (include/nspt.h): context, plans, workspace, and the
+// composition of the kernels into nspt_series_mul / _batched (FFT-CONV Steps 1-5,
+// PAPER.md:68-102) and nspt_staple (eq. 2.3).
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "nspt_internal.cuh"
+
+namespace nspt {
+namespace {
+
+struct Plan {
+    int L, n;
+    double s;
+    double2* tw_fwd = nullptr;
+    double2* tw_inv = nullptr;
+    double* scale_in = nullptr;   // null when s == 1
+    double* scale_out = nullptr;  // s^-k / L
+};
+
+struct ProfEvent {
+    cudaEvent_t a, b;
+    int stage;
+};
+
+struct Context {
+    std::mutex mu;
+    cudaStream_t stream = nullptr;
+    double order_scale = 1.0;
+    int gemm_variant = 1;
+    bool arch_checked = false;
+    // workspace
+    void* user_ws = nullptr;
+    size_t user_ws_bytes = 0;
+    void* own_ws = nullptr;
+    size_t own_ws_bytes = 0;
+    // staging for the _host calls
+    void* stage_dev = nullptr;
+    size_t stage_dev_bytes = 0;
+    std::vector<Plan> plans;
+    // profiling
+    bool profiling = false;
+    std::vector<ProfEvent> prof_used;
+    std::vector<ProfEvent> prof_free;
+    double prof_ms[ST_COUNT] = {0, 0, 0, 0, 0};
+    long long prof_n[ST_COUNT] = {0, 0, 0, 0, 0};
+    long long launches = 0;
+    char cuda_msg[256] = "no CUDA error recorded";
+};
+
+Context g;
+
+int cuda_fail(cudaError_t e) {
+    snprintf(g.cuda_msg, sizeof(g.cuda_msg), "CUDA error: %s", cudaGetErrorString(e));
+    if (e == cudaErrorMemoryAllocation) return NSPT_ENOMEM;
+    return NSPT_ECUDA;
+}
+
+#define NSPT_CUDA(x)                                 \
+    do {                                             \
+        cudaError_t e__ = (x);                       \
+        if (e__ != cudaSuccess) return cuda_fail(e__); \
+    } while (0)
+
+int check_arch() {
+    if (g.arch_checked) return NSPT_OK;
+    int dev = 0;
+    NSPT_CUDA(cudaGetDevice(&dev));
+    int major = 0;
+    NSPT_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return NSPT_EARCH;
+    g.arch_checked = true;
+    return NSPT_OK;
+}
+
+int check_dims(int N, int Ntrunc, int batch) {
+    if (N < 1 || Ntrunc < 0 || batch < 1) return NSPT_EINVAL;
+    if (Ntrunc > NSPT_MAX_NTRUNC) return NSPT_EINVAL;
+    if ((long long)N * N > (1ll << 40)) return NSPT_EINVAL;
+    return NSPT_OK;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+// ---- plans ---------------------------------------------------------------------------------
+int get_plan(int L, int n, double s, PlanTables* out) {
+    for (const Plan& p : g.plans) {
+        if (p.L == L && p.n == n && p.s == s) {
+            *out = PlanTables{p.tw_fwd, p.tw_inv, p.scale_in, p.scale_out, 1.0 / L};
+            return NSPT_OK;
+        }
+    }
+    Plan p;
+    p.L = L;
+    p.n = n;
+    p.s = s;
+    std::vector<double2> f(L), b(L);
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int m = 0; m < L; ++m) {
+        // exact values on the axes and diagonals, long double elsewhere
+        long double ang = two_pi * (long double)m / (long double)L;
+        double c = (double)cosl(ang), sn = (double)sinl(ang);
+        if ((4 * m) % L == 0) {  // multiples of pi/2
+            const int q = (4 * m) / L;
+            c = (q == 0) ? 1.0 : (q == 2 ? -1.0 : 0.0);
+            sn = (q == 1) ? 1.0 : (q == 3 ? -1.0 : 0.0);
+        }
+        f[m] = make_double2(c, sn);   // w^m,  w = exp(+2 pi i / L)   (eq. 2.7)
+        b[m] = make_double2(c, -sn);  // w^-m                          (eq. 2.9)
+    }
+    std::vector<double> so(n), si(n);
+    for (int k = 0; k < n; ++k) {
+        si[k] = (double)powl((long double)s, (long double)k);
+        so[k] = (double)(powl((long double)s, -(long double)k) / (long double)L);
+    }
+    NSPT_CUDA(cudaMalloc(&p.tw_fwd, sizeof(double2) * L));
+    NSPT_CUDA(cudaMalloc(&p.tw_inv, sizeof(double2) * L));
+    NSPT_CUDA(cudaMalloc(&p.scale_out, sizeof(double) * n));
+    NSPT_CUDA(cudaMemcpy(p.tw_fwd, f.data(), sizeof(double2) * L, cudaMemcpyHostToDevice));
+    NSPT_CUDA(cudaMemcpy(p.tw_inv, b.data(), sizeof(double2) * L, cudaMemcpyHostToDevice));
+    NSPT_CUDA(cudaMemcpy(p.scale_out, so.data(), sizeof(double) * n, cudaMemcpyHostToDevice));
+    if (s != 1.0) {
+        NSPT_CUDA(cudaMalloc(&p.scale_in, sizeof(double) * n));
+        NSPT_CUDA(cudaMemcpy(p.scale_in, si.data(), sizeof(double) * n, cudaMemcpyHostToDevice));
+    }
+    g.plans.push_back(p);
+    *out = PlanTables{p.tw_fwd, p.tw_inv, p.scale_in, p.scale_out, 1.0 / L};
+    return NSPT_OK;
+}
+
+// ---- workspace -----------------------------------------------------------------------------
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+size_t spectrum_bytes(const FreqLayout& f, int batch) { return align_up(f.spectrum_doubles(batch) * 8, 1024); }
+
+size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
+    if (op == NSPT_OP_STAPLE) return 11 * spectrum_bytes(f, 1);
+    return 3 * spectrum_bytes(f, batch);
+}
+
+int get_workspace(size_t bytes, char** out) {
+    if (g.user_ws) {
+        if (g.user_ws_bytes < bytes) return NSPT_ENOMEM;
+        *out = static_cast<char*>(g.user_ws);
+        return NSPT_OK;
+    }
+    if (g.own_ws_bytes < bytes) {
+        if (g.own_ws) {
+            NSPT_CUDA(cudaStreamSynchronize(g.stream));
+            NSPT_CUDA(cudaFree(g.own_ws));
+            g.own_ws = nullptr;
+            g.own_ws_bytes = 0;
+        }
+        NSPT_CUDA(cudaMalloc(&g.own_ws, bytes));
+        g.own_ws_bytes = bytes;
+    }
+    *out = static_cast<char*>(g.own_ws);
+    return NSPT_OK;
+}
+
+int get_staging(size_t bytes, char** out) {
+    if (g.stage_dev_bytes < bytes) {
+        if (g.stage_dev) {
+            NSPT_CUDA(cudaStreamSynchronize(g.stream));
+            NSPT_CUDA(cudaFree(g.stage_dev));
+            g.stage_dev = nullptr;
+            g.stage_dev_bytes = 0;
+        }
+        NSPT_CUDA(cudaMalloc(&g.stage_dev, bytes));
+        g.stage_dev_bytes = bytes;
+    }
+    *out = static_cast<char*>(g.stage_dev);
+    return NSPT_OK;
+}
+
+// ---- profiling -----------------------------------------------------------------------------
+int prof_flush() {
+    if (g.prof_used.empty()) return NSPT_OK;
+    NSPT_CUDA(cudaStreamSynchronize(g.stream));
+    for (ProfEvent& e : g.prof_used) {
+        float ms = 0.f;
+        NSPT_CUDA(cudaEventElapsedTime(&ms, e.a, e.b));
+        g.prof_ms[e.stage] += ms;
+        g.prof_n[e.stage] += 1;
+        g.prof_free.push_back(e);
+    }
+    g.prof_used.clear();
+    return NSPT_OK;
+}
+
+struct StageTimer {
+    bool on = false;
+    ProfEvent ev{};
+    int begin(int stage) {
+        g.launches += 1;
+        if (!g.profiling) return NSPT_OK;
+        if (g.prof_used.size() >= 4096) {
+            int rc = prof_flush();
+            if (rc) return rc;
+        }
+        if (!g.prof_free.empty()) {
+            ev = g.prof_free.back();
+            g.prof_free.pop_back();
+        } else {
+            NSPT_CUDA(cudaEventCreate(&ev.a));
+            NSPT_CUDA(cudaEventCreate(&ev.b));
+        }
+        ev.stage = stage;
+        on = true;
+        NSPT_CUDA(cudaEventRecord(ev.a, g.stream));
+        return NSPT_OK;
+    }
+    int end() {
+        if (!on) return NSPT_OK;
+        NSPT_CUDA(cudaEventRecord(ev.b, g.stream));
+        g.prof_used.push_back(ev);
+        on = false;
+        return NSPT_OK;
+    }
+};
+
+#define NSPT_TRY(x)            \
+    do {                       \
+        int rc__ = (x);        \
+        if (rc__) return rc__; \
+    } while (0)
+
+// Each helper = one kernel launch, bracketed for the profiler.
+int k_forward(const FreqLayout& f, const PlanTables& t, int batch, const nspt_c128* s0, double* d0,
+              const nspt_c128* s1, double* d1) {
+    StageTimer tm;
+    NSPT_TRY(tm.begin(ST_FWD));
+    NSPT_CUDA(launch_fft_forward(f, t, batch, s0, d0, s1, d1, g.stream));
+    return tm.end();
+}
+int k_inverse(const FreqLayout& f, const PlanTables& t, int batch, const double* src, nspt_c128* dst) {
+    StageTimer tm;
+    NSPT_TRY(tm.begin(ST_INV));
+    NSPT_CUDA(launch_fft_inverse(f, t, batch, src, dst, g.stream));
+    return tm.end();
+}
+int k_retrunc(const FreqLayout& f, const PlanTables& t, int batch, const double* src, double* dst) {
+    StageTimer tm;
+    NSPT_TRY(tm.begin(ST_RETRUNC));
+    NSPT_CUDA(launch_fft_retruncate(f, t, batch, src, dst, g.stream));
+    return tm.end();
+}
+int k_dagger(const FreqLayout& f, int batch, const double* src, double* dst) {
+    StageTimer tm;
+    NSPT_TRY(tm.begin(ST_OTHER));
+    NSPT_CUDA(launch_freq_dagger(f, batch, src, dst, g.stream));
+    return tm.end();
+}
+int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, double* C, Cplx alpha, bool acc) {
+    StageTimer tm;
+    NSPT_TRY(tm.begin(ST_GEMM));
+    NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, C, alpha, acc, g.gemm_variant, g.stream));
+    return tm.end();
+}
+
+// ---- the products --------------------------------------------------------------------------
+int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc, int batch) {
+    NSPT_TRY(check_dims(N, Ntrunc, batch));
+    if (!A || !B || !C || !aligned16(A) || !aligned16(B) || !aligned16(C)) return NSPT_EINVAL;
+    NSPT_TRY(check_arch());
+    const FreqLayout f = make_layout(N, Ntrunc);
+    if (!fft_length_supported(f.L)) return NSPT_EINVAL;
+    PlanTables t;
+    NSPT_TRY(get_plan(f.L, f.n, g.order_scale, &t));
+    char* ws = nullptr;
+    NSPT_TRY(get_workspace(ws_bytes_for(f, batch, NSPT_OP_SERIES_MUL), &ws));
+    const size_t sb = spectrum_bytes(f, batch);
+    double* At = reinterpret_cast<double*>(ws);
+    double* Bt = reinterpret_cast<double*>(ws + sb);
+    double* Ct = reinterpret_cast<double*>(ws + 2 * sb);
+    // Steps 1-2 (eqs. 2.6-2.7): zero-padded forward transforms of A and B, one launch
+    NSPT_TRY(k_forward(f, t, batch, A, At, B, Bt));
+    // Step 3 (eq. 2.8): mode-wise matrix products
+    NSPT_TRY(k_gemm(f, batch, At, Bt, Ct, Cplx{1.0, 0.0}, false));
+    // Steps 4-5 (eq. 2.9): inverse transform, 1/L, truncation
+    NSPT_TRY(k_inverse(f, t, batch, Ct, C));
+    return NSPT_OK;
+}
+
+int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4], int N, int Ntrunc) {
+    NSPT_TRY(check_dims(N, Ntrunc, 1));
+    if (!U || !z || !S) return NSPT_EINVAL;
+    for (int mu = 0; mu < 4; ++mu)
+        if (!U[mu] || !S[mu] || !aligned16(U[mu]) || !aligned16(S[mu])) return NSPT_EINVAL;
+    NSPT_TRY(check_arch());
+    const FreqLayout f = make_layout(N, Ntrunc);
+    if (!fft_length_supported(f.L)) return NSPT_EINVAL;
+    PlanTables t;
+    NSPT_TRY(get_plan(f.L, f.n, g.order_scale, &t));
+    char* ws = nullptr;
+    NSPT_TRY(get_workspace(ws_bytes_for(f, 1, NSPT_OP_STAPLE), &ws));
+    const size_t sb = spectrum_bytes(f, 1);
+    auto spec = [&](int i) { return reinterpret_cast<double*>(ws + (size_t)i * sb); };
+    double* Ut[4] = {spec(0), spec(1), spec(2), spec(3)};   // U~_mu
+    double* Ud[4] = {spec(4), spec(5), spec(6), spec(7)};   // spectrum of U_mu^+
+    double* W = spec(8);                                    // first-level product, re-truncated in place
+    double* X = spec(9);                                    // accumulated bracket of eq. 2.3
+    double* St = spec(10);                                  // U_mu * X
+    // all four links are transformed before any output is written (S may alias U)
+    NSPT_TRY(k_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1]));
+    NSPT_TRY(k_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3]));
+    for (int mu = 0; mu < 4; ++mu) NSPT_TRY(k_dagger(f, 1, Ut[mu], Ud[mu]));
+    for (int mu = 0; mu < 4; ++mu) {
+        bool first = true;
+        for (int nu = 0; nu < 4; ++nu) {
+            if (nu == mu) continue;
+            const Cplx zmn{z[4 * mu + nu].re, z[4 * mu + nu].im};
+            // + z_{mu nu} (U_nu * U_mu^+) * U_nu^+
+            NSPT_TRY(k_gemm(f, 1, Ut[nu], Ud[mu], W, Cplx{1.0, 0.0}, false));
+            NSPT_TRY(k_retrunc(f, t, 1, W, W));
+            NSPT_TRY(k_gemm(f, 1, W, Ud[nu], X, zmn, !first));
+            first = false;
+            // - z_{mu nu}^* (U_nu^+ * U_mu^+) * U_nu
+            NSPT_TRY(k_gemm(f, 1, Ud[nu], Ud[mu], W, Cplx{1.0, 0.0}, false));
+            NSPT_TRY(k_retrunc(f, t, 1, W, W));
+            NSPT_TRY(k_gemm(f, 1, W, Ut[nu], X, Cplx{-zmn.re, zmn.im}, true));
+        }
+        NSPT_TRY(k_retrunc(f, t, 1, X, X));
+        NSPT_TRY(k_gemm(f, 1, Ut[mu], X, St, Cplx{1.0, 0.0}, false));
+        NSPT_TRY(k_inverse(f, t, 1, St, S[mu]));
+    }
+    return NSPT_OK;
+}
+
+}  // namespace
+}  // namespace nspt
+
+using namespace nspt;
+
+extern "C" {
+
+int nspt_series_mul(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    return series_mul_device(A, B, C, N, Ntrunc, 1);
+}
+
+int nspt_series_mul_batched(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc, int batch) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    return series_mul_device(A, B, C, N, Ntrunc, batch);
+}
+
+int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4], int N, int Ntrunc) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    return staple_device(U, z, S, N, Ntrunc);
+}
+
+int nspt_series_mul_batched_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc, int batch) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_TRY(check_dims(N, Ntrunc, batch));
+    if (!A || !B || !C) return NSPT_EINVAL;
+    const size_t bytes = (size_t)batch * (Ntrunc + 1) * N * N * sizeof(nspt_c128);
+    const size_t slot = align_up(bytes, 256);
+    char* dev = nullptr;
+    NSPT_TRY(get_staging(3 * slot, &dev));
+    nspt_c128* dA = reinterpret_cast<nspt_c128*>(dev);
+    nspt_c128* dB = reinterpret_cast<nspt_c128*>(dev + slot);
+    nspt_c128* dC = reinterpret_cast<nspt_c128*>(dev + 2 * slot);
+    NSPT_CUDA(cudaMemcpyAsync(dA, A, bytes, cudaMemcpyHostToDevice, g.stream));
+    NSPT_CUDA(cudaMemcpyAsync(dB, B, bytes, cudaMemcpyHostToDevice, g.stream));
+    NSPT_TRY(series_mul_device(dA, dB, dC, N, Ntrunc, batch));
+    NSPT_CUDA(cudaMemcpyAsync(C, dC, bytes, cudaMemcpyDeviceToHost, g.stream));
+    NSPT_CUDA(cudaStreamSynchronize(g.stream));
+    return NSPT_OK;
+}
+
+int nspt_series_mul_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc) {
+    return nspt_series_mul_batched_host(A, B, C, N, Ntrunc, 1);
+}
+
+int nspt_staple_host(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4], int N, int Ntrunc) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_TRY(check_dims(N, Ntrunc, 1));
+    if (!U || !z || !S) return NSPT_EINVAL;
+    for (int mu = 0; mu < 4; ++mu)
+        if (!U[mu] || !S[mu]) return NSPT_EINVAL;
+    const size_t bytes = (size_t)(Ntrunc + 1) * N * N * sizeof(nspt_c128);
+    const size_t slot = align_up(bytes, 256);
+    char* dev = nullptr;
+    NSPT_TRY(get_staging(8 * slot, &dev));
+    const nspt_c128* dU[4];
+    nspt_c128* dS[4];
+    for (int mu = 0; mu < 4; ++mu) {
+        dU[mu] = reinterpret_cast<nspt_c128*>(dev + (size_t)mu * slot);
+        dS[mu] = reinterpret_cast<nspt_c128*>(dev + (size_t)(4 + mu) * slot);
+        NSPT_CUDA(cudaMemcpyAsync(const_cast<nspt_c128*>(dU[mu]), U[mu], bytes, cudaMemcpyHostToDevice, g.stream));
+    }
+    NSPT_TRY(staple_device(dU, z, dS, N, Ntrunc));
+    for (int mu = 0; mu < 4; ++mu) NSPT_CUDA(cudaMemcpyAsync(S[mu], dS[mu], bytes, cudaMemcpyDeviceToHost, g.stream));
+    NSPT_CUDA(cudaStreamSynchronize(g.stream));
+    return NSPT_OK;
+}
+
+int nspt_set_stream(void* cuda_stream) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    if (g.profiling) NSPT_TRY(prof_flush());
+    g.stream = static_cast<cudaStream_t>(cuda_stream);
+    return NSPT_OK;
+}
+
+int nspt_set_order_scale(double s) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    if (!(s > 0.0) || !std::isfinite(s)) return NSPT_EINVAL;
+    g.order_scale = s;
+    return NSPT_OK;
+}
+
+int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out) {
+    if (!out) return NSPT_EINVAL;
+    if (op != NSPT_OP_SERIES_MUL && op != NSPT_OP_STAPLE) return NSPT_EINVAL;
+    if (op == NSPT_OP_STAPLE) batch = 1;
+    NSPT_TRY(check_dims(N, Ntrunc, batch));
+    const FreqLayout f = make_layout(N, Ntrunc);
+    if (!fft_length_supported(f.L)) return NSPT_EINVAL;
+    *out = ws_bytes_for(f, batch, op);
+    return NSPT_OK;
+}
+
+int nspt_set_workspace(void* dptr, size_t bytes) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    if (dptr && (reinterpret_cast<uintptr_t>(dptr) & 255)) return NSPT_EINVAL;
+    if (!dptr && bytes) return NSPT_EINVAL;
+    g.user_ws = dptr;
+    g.user_ws_bytes = dptr ? bytes : 0;
+    return NSPT_OK;
+}
+
+int nspt_set_gemm_variant(int variant) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    if (variant != 0 && variant != 1) return NSPT_EINVAL;
+    g.gemm_variant = variant;
+    return NSPT_OK;
+}
+
+int nspt_profile(int enable) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    if (!enable && g.profiling) NSPT_TRY(prof_flush());
+    g.profiling = enable != 0;
+    return NSPT_OK;
+}
+
+int nspt_profile_read(int stage, double* ms, long long* launches) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    if (stage < 0 || stage >= ST_COUNT || !ms || !launches) return NSPT_EINVAL;
+    NSPT_TRY(prof_flush());
+    *ms = g.prof_ms[stage];
+    *launches = g.prof_n[stage];
+    g.prof_ms[stage] = 0.0;
+    g.prof_n[stage] = 0;
+    return NSPT_OK;
+}
+
+long long nspt_launch_count(void) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    return g.launches;
+}
+
+int nspt_release(void) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    cudaStreamSynchronize(g.stream);
+    for (Plan& p : g.plans) {
+        cudaFree(p.tw_fwd);
+        cudaFree(p.tw_inv);
+        cudaFree(p.scale_in);
+        cudaFree(p.scale_out);
+    }
+    g.plans.clear();
+    if (g.own_ws) cudaFree(g.own_ws);
+    g.own_ws = nullptr;
+    g.own_ws_bytes = 0;
+    if (g.stage_dev) cudaFree(g.stage_dev);
+    g.stage_dev = nullptr;
+    g.stage_dev_bytes = 0;
+    for (ProfEvent& e : g.prof_used) {
+        cudaEventDestroy(e.a);
+        cudaEventDestroy(e.b);
+    }
+    for (ProfEvent& e : g.prof_free) {
+        cudaEventDestroy(e.a);
+        cudaEventDestroy(e.b);
+    }
+    g.prof_used.clear();
+    g.prof_free.clear();
+    return NSPT_OK;
+}
+
+const char* nspt_strerror(int code) {
+    switch (code) {
+        case NSPT_OK: return "ok";
+        case NSPT_EINVAL: return "invalid argument (null or misaligned pointer, N < 1, Ntrunc outside [0,127], batch < 1)";
+        case NSPT_ENOMEM: return "out of memory, or the caller's workspace is too small";
+        case NSPT_ECUDA: return g.cuda_msg;
+        case NSPT_EARCH: return "the current CUDA device is not compute capability 10.x (B200, sm_100a)";
+        default: return "unknown error code";
+    }
+}
+
+int nspt_version(void) { return 100; }
+
+}  // extern "C"

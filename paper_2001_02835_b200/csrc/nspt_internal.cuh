@@ -1,0 +1,82 @@
+// nspt_internal.cuh -- shared declarations of libnspt (CUDA path only; the oracle shares nothing with this).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <cstdint>
+#include "../../include/nspt.h"
+
+namespace nspt {
+
+// ---------------------------------------------------------------------------------------------
+// Frequency-domain workspace layout (internal; eq. 2.7 defines the content).
+// One "spectrum" holds the Fourier coefficients X~(p), p = 0..L-1, of `batch` series as PLANAR
+// real / imaginary planes so that the mode-wise matrix product (eq. 2.8) can feed FP64 tensor
+// cores directly:
+//     plane(b, p, c)[i*ld + j],  c = 0 (real) / 1 (imag),  at double offset ((b*L + p)*2 + c)*ps
+// ld = N rounded up to a multiple of 4 (rows start 32-byte aligned), ps = N*ld rounded up to 16.
+// ---------------------------------------------------------------------------------------------
+struct FreqLayout {
+    int N;        // matrix dimension
+    int n;        // Ntrunc + 1 coefficients
+    int L;        // transform length: power of two >= 2*Ntrunc + 1
+    int ld;       // leading dimension of a plane, doubles
+    size_t ps;    // plane stride, doubles
+    size_t NN;    // N*N
+    size_t spectrum_doubles(int batch) const { return (size_t)batch * L * 2 * ps; }
+};
+
+inline int transform_length(int Ntrunc) {
+    int need = 2 * Ntrunc + 1, L = 1;
+    while (L < need) L <<= 1;
+    return L;
+}
+
+inline FreqLayout make_layout(int N, int Ntrunc) {
+    FreqLayout f;
+    f.N = N;
+    f.n = Ntrunc + 1;
+    f.L = transform_length(Ntrunc);
+    f.ld = (N + 3) & ~3;
+    f.ps = (((size_t)N * f.ld) + 15) & ~(size_t)15;
+    f.NN = (size_t)N * N;
+    return f;
+}
+
+// Per-L tables living in device memory (built on the host in long double).
+struct PlanTables {
+    const double2* tw_fwd;   // w^m  = exp(+2 pi i m / L), m < L      (eq. 2.7)
+    const double2* tw_inv;   // w^-m                                   (eq. 2.9)
+    const double* scale_in;  // s^k, k < n          (order scale, 1 when off)
+    const double* scale_out; // s^-k / L, k < n     (unscale and the 1/L of eq. 2.9)
+    double inv_L;
+};
+
+enum Stage { ST_FWD = 0, ST_GEMM = 1, ST_INV = 2, ST_RETRUNC = 3, ST_OTHER = 4, ST_COUNT = 5 };
+
+// Complex scalar for epilogues.
+struct Cplx { double re, im; };
+
+// ---- transforms (nspt_fft.cu) ---------------------------------------------------------------
+// Forward: up to two operands per launch (src1 may be null). series -> spectrum.
+cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int batch,
+                               const nspt_c128* src0, double* dst0,
+                               const nspt_c128* src1, double* dst1, cudaStream_t st);
+// Inverse + 1/L + truncation (+ unscale): spectrum -> series.
+cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int batch,
+                               const double* src, nspt_c128* dst, cudaStream_t st);
+// Re-truncation in place in frequency space: inverse, zero orders > Ntrunc, forward.
+cudaError_t launch_fft_retruncate(const FreqLayout& f, const PlanTables& t, int batch,
+                                  const double* src, double* dst, cudaStream_t st);
+// Spectrum of the daggered series: Xd~(p) = (X~((L - p) mod L))^H.
+cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src, double* dst,
+                               cudaStream_t st);
+bool fft_length_supported(int L);
+
+// ---- mode-wise matrix product (nspt_zgemm.cu) -----------------------------------------------
+// C~(p) = alpha * A~(p) B~(p) [+ C~(p) if accumulate], for all batch*L modes.
+cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B,
+                               double* C, Cplx alpha, bool accumulate, int variant,
+                               cudaStream_t st);
+cudaError_t zgemm_init();   // resolves the driver entry point for tensor maps
+
+}  // namespace nspt

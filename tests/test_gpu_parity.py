@@ -1,0 +1,309 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle
+on the same seeded inputs.  Tolerance (BASELINE.json north_star): per order k,
+    ||C_gpu^(k) - C_oracle^(k)||_F <= 1e-11 * sum_{j<=k} ||A^(j)||_F ||B^(k-j)||_F,
+and bit-exact after rounding on small-integer inputs.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def nspt():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2001_02835_b200 import binding
+    binding.use_current_stream()
+    binding.nspt_set_order_scale(1.0)
+    binding.nspt_set_gemm_variant(1)
+    yield binding
+    binding.nspt_set_order_scale(1.0)
+    binding.nspt_set_gemm_variant(1)
+
+
+def to_dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def gpu_mul(nspt, A, B):
+    import torch
+    C = nspt.nspt_series_mul(to_dev(A), to_dev(B))
+    torch.cuda.synchronize()
+    return C.cpu().numpy()
+
+
+def check_product(nspt, A, B, tol=TOL):
+    import oracle
+    ref = oracle.series_mul(A, B)
+    got = gpu_mul(nspt, A, B)
+    err = oracle.per_order_error(got, ref, oracle.product_bound(A, B))
+    assert np.isfinite(got).all()
+    assert err.max() <= tol, f"max per-order error {err.max():.3e} at k={err.argmax()}"
+    return err.max()
+
+
+# ----------------------------------------------------------------------------- config 1
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config1_gaussian(nspt, variant):
+    from paper_2001_02835_b200 import workloads as wl
+    nspt.nspt_set_gemm_variant(variant)
+    A, B = wl.config1_gaussian()
+    check_product(nspt, A, B)
+    nspt.nspt_set_gemm_variant(1)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config1_integer_bit_exact(nspt, variant):
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    nspt.nspt_set_gemm_variant(variant)
+    A, B = wl.config1_integer()
+    ref = oracle.series_mul(A, B)
+    got = gpu_mul(nspt, A, B)
+    assert np.array_equal(np.round(got.real), ref.real)
+    assert np.array_equal(np.round(got.imag), ref.imag)
+    assert np.abs(got - ref).max() < 1e-10      # and the unrounded deviation is tiny
+    nspt.nspt_set_gemm_variant(1)
+
+
+# ----------------------------------------------------------------------------- shapes: tiles, ragged tails, degenerate
+
+SHAPES = [
+    (1, 0), (1, 5), (2, 1), (3, 2), (7, 3), (8, 7), (9, 7), (17, 4), (24, 8), (47, 15), (48, 15),
+    (49, 15), (50, 12), (97, 5), (100, 31), (33, 63), (20, 127), (121, 7), (145, 3),
+]
+
+
+@pytest.mark.parametrize("N,Ntrunc", SHAPES)
+def test_gaussian_shapes(nspt, N, Ntrunc):
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([1, N, Ntrunc])
+    A = wl.gaussian_series(N, Ntrunc, rng)
+    B = wl.gaussian_series(N, Ntrunc, rng)
+    check_product(nspt, A, B)
+
+
+@pytest.mark.parametrize("N,Ntrunc", [(5, 3), (48, 7), (57, 9), (64, 31)])
+def test_integer_shapes_bit_exact(nspt, N, Ntrunc):
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([2, N, Ntrunc])
+    A = wl.integer_series(N, Ntrunc, rng)
+    B = wl.integer_series(N, Ntrunc, rng)
+    ref = oracle.series_mul(A, B)
+    got = gpu_mul(nspt, A, B)
+    assert np.array_equal(np.round(got.real), ref.real) and np.array_equal(np.round(got.imag), ref.imag)
+
+
+def test_reference_variant_agrees_with_tensor_core_variant(nspt):
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(77)
+    A = wl.gaussian_series(75, 15, rng)
+    B = wl.gaussian_series(75, 15, rng)
+    nspt.nspt_set_gemm_variant(0)
+    e0 = check_product(nspt, A, B)
+    nspt.nspt_set_gemm_variant(1)
+    e1 = check_product(nspt, A, B)
+    assert e0 < 1e-13 and e1 < 1e-13
+
+
+def test_unit_and_zero(nspt):
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(3)
+    N, Ntrunc = 30, 7
+    A = wl.gaussian_series(N, Ntrunc, rng)
+    one = np.zeros_like(A)
+    one[0] = np.eye(N)
+    got = gpu_mul(nspt, one, A)
+    assert np.abs(got - A).max() < 1e-13
+    got = gpu_mul(nspt, A, np.zeros_like(A))
+    assert np.abs(got).max() == 0
+
+
+def test_output_may_alias_input(nspt):
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(4)
+    A = wl.gaussian_series(40, 7, rng)
+    B = wl.gaussian_series(40, 7, rng)
+    ref = oracle.series_mul(A, B)
+    dA, dB = to_dev(A), to_dev(B)
+    nspt.nspt_series_mul(dA, dB, dA)
+    torch.cuda.synchronize()
+    assert oracle.per_order_error(dA.cpu().numpy(), ref, oracle.product_bound(A, B)).max() <= TOL
+    dA = to_dev(A)
+    nspt.nspt_series_mul(dA, dA, dA)       # C = A * A in place
+    torch.cuda.synchronize()
+    assert oracle.per_order_error(dA.cpu().numpy(), oracle.series_mul(A, A), oracle.product_bound(A, A)).max() <= TOL
+
+
+# ----------------------------------------------------------------------------- batched, host, scale
+
+def test_batched_matches_oracle(nspt):
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(5)
+    batch, N, Ntrunc = 4, 27, 15
+    A = np.stack([wl.gaussian_series(N, Ntrunc, rng) for _ in range(batch)])
+    B = np.stack([wl.gaussian_series(N, Ntrunc, rng) for _ in range(batch)])
+    C = nspt.nspt_series_mul_batched(to_dev(A), to_dev(B))
+    torch.cuda.synchronize()
+    C = C.cpu().numpy()
+    for b in range(batch):
+        err = oracle.per_order_error(C[b], oracle.series_mul(A[b], B[b]), oracle.product_bound(A[b], B[b]))
+        assert err.max() <= TOL
+
+
+def test_host_entry_points(nspt):
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(6)
+    A = wl.gaussian_series(31, 7, rng)
+    B = wl.gaussian_series(31, 7, rng)
+    C = np.empty_like(A)
+    nspt.nspt_series_mul_host(A, B, C)
+    assert oracle.per_order_error(C, oracle.series_mul(A, B), oracle.product_bound(A, B)).max() <= TOL
+    Ab, Bb = np.stack([A, B]), np.stack([B, A])
+    Cb = np.empty_like(Ab)
+    nspt.nspt_series_mul_batched_host(Ab, Bb, Cb)
+    assert oracle.per_order_error(Cb[1], oracle.series_mul(B, A), oracle.product_bound(B, A)).max() <= TOL
+
+
+def test_order_scale_is_transparent(nspt):
+    from paper_2001_02835_b200 import workloads as wl
+    A, B = wl.config_product(25, 31, seed=[8, 25, 31])
+    try:
+        for s in (0.97, 1.05):
+            nspt.nspt_set_order_scale(s)
+            check_product(nspt, A, B)
+    finally:
+        nspt.nspt_set_order_scale(1.0)
+
+
+def test_caller_workspace(nspt):
+    import torch
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(9)
+    A = wl.gaussian_series(20, 7, rng)
+    B = wl.gaussian_series(20, 7, rng)
+    need = nspt.nspt_workspace_bytes(20, 7, 1, nspt.NSPT_OP_SERIES_MUL)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    try:
+        nspt.nspt_set_workspace(ws.data_ptr(), need)
+        check_product(nspt, A, B)
+        nspt.nspt_set_workspace(ws.data_ptr(), need // 2)
+        with pytest.raises(nspt.NsptError) as ei:
+            nspt.nspt_series_mul(to_dev(A), to_dev(B))
+        assert ei.value.code == nspt.NSPT_ENOMEM
+    finally:
+        nspt.nspt_set_workspace(None, 0)
+
+
+def test_error_codes(nspt):
+    import torch
+    lib = nspt.raw()
+    x = torch.zeros(2, 2, 2, dtype=torch.complex128, device="cuda")
+    p = x.data_ptr()
+    assert lib.nspt_series_mul(None, p, p, 2, 1) == nspt.NSPT_EINVAL
+    assert lib.nspt_series_mul(p, p, p, 0, 1) == nspt.NSPT_EINVAL
+    assert lib.nspt_series_mul(p, p, p, 2, -1) == nspt.NSPT_EINVAL
+    assert lib.nspt_series_mul(p, p, p, 2, 128) == nspt.NSPT_EINVAL
+    assert lib.nspt_series_mul(p + 8, p, p, 2, 1) == nspt.NSPT_EINVAL
+    assert lib.nspt_series_mul_batched(p, p, p, 2, 1, 0) == nspt.NSPT_EINVAL
+    assert lib.nspt_set_order_scale(0.0) == nspt.NSPT_EINVAL
+    assert "invalid" in nspt.nspt_strerror(nspt.NSPT_EINVAL)
+    assert nspt.nspt_version() >= 100
+
+
+# ----------------------------------------------------------------------------- the staple
+
+def check_staple(nspt, U, z):
+    import torch
+    import oracle
+    ref = oracle.staple(U, z)
+    S = nspt.nspt_staple([to_dev(u) for u in U], z)
+    torch.cuda.synchronize()
+    bounds = oracle.staple_bound(U)
+    worst = 0.0
+    for mu in range(4):
+        err = oracle.per_order_error(S[mu].cpu().numpy(), ref[mu], bounds[mu])
+        worst = max(worst, err.max())
+    assert worst <= TOL, f"staple error {worst:.3e}"
+    return worst
+
+
+@pytest.mark.parametrize("N,Ntrunc,seed", [(9, 7, 40), (4, 3, 41), (25, 15, 42), (50, 5, 43)])
+def test_staple_small(nspt, N, Ntrunc, seed):
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(seed)
+    U = [wl.unitary_series(N, Ntrunc, rng) for _ in range(4)]
+    z = wl.twist_tensor(int(round(np.sqrt(N))) if int(round(np.sqrt(N))) ** 2 == N else 7, 1)
+    check_staple(nspt, U, z)
+
+
+def test_staple_generic_links_and_z(nspt):
+    # not unitary, z not unimodular / antisymmetric: the library must use z as given
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(44)
+    U = [wl.gaussian_series(12, 6, rng) for _ in range(4)]
+    z = rng.standard_normal((4, 4)) + 1j * rng.standard_normal((4, 4))
+    check_staple(nspt, U, z)
+
+
+def test_staple_output_may_alias_links(nspt):
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(45)
+    U = [wl.unitary_series(16, 7, rng) for _ in range(4)]
+    z = wl.twist_tensor(4, 1)
+    ref = oracle.staple(U, z)
+    dU = [to_dev(u) for u in U]
+    nspt.nspt_staple(dU, z, dU)
+    torch.cuda.synchronize()
+    bounds = oracle.staple_bound(U)
+    for mu in range(4):
+        assert oracle.per_order_error(dU[mu].cpu().numpy(), ref[mu], bounds[mu]).max() <= TOL
+
+
+# ----------------------------------------------------------------------------- full-size configs
+
+def test_config2_full(nspt):
+    from paper_2001_02835_b200 import workloads as wl
+    A, B = wl.config_product(225, 31, seed=2)
+    check_product(nspt, A, B)
+
+
+def test_config3_full(nspt):
+    from paper_2001_02835_b200 import workloads as wl
+    A, B = wl.config_product(225, 63, seed=3)
+    check_product(nspt, A, B)
+
+
+def test_config4_staple_full(nspt):
+    from paper_2001_02835_b200 import workloads as wl
+    U, z = wl.config_staple(225, 31, seed=4)
+    check_staple(nspt, U, z)
+
+
+@pytest.mark.parametrize("N,Ntrunc", [(225, 7), (225, 15), (225, 127), (16, 31), (49, 31), (100, 31), (400, 31)])
+def test_config5_sweep_points_sampled_rows(nspt, N, Ntrunc):
+    # full-size sweep points: compare sampled rows of every order, each computed by the oracle
+    # from the definition (eq. 2.5) one row at a time.
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    A, B = wl.config_product(N, Ntrunc, seed=[5, N, Ntrunc])
+    got = gpu_mul(nspt, A, B)
+    rows = sorted(set([0, N // 3, N - 1]))
+    ref = oracle.series_mul_rows(A, B, rows)
+    bound = oracle.product_bound(A, B) * np.sqrt(len(rows) / N)     # share of the Frobenius bound
+    d = got[:, rows, :] - ref
+    err = np.sqrt((np.abs(d) ** 2).sum(axis=(1, 2))) / bound
+    assert err.max() <= TOL, f"{err.max():.3e}"
