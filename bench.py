@@ -1,0 +1,492 @@
+#!/usr/bin/env python
+"""bench.py -- series star-products per second on B200 (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg2|staple|batched4]
+    python bench.py --impl reference ...        # the CPU oracle as the reference arm
+
+A step is one pass of the whole hot path over one synthetic input: for the default workload
+(cfg3: N=225, N_trunc=63, the configuration the north-star target is quoted on) that is one
+nspt_series_mul = forward transforms of A and B, 128 mode-wise 225^3 complex matrix products,
+inverse transform with truncation.  Inputs are seeded synthetic unitary series
+(paper_2001_02835_b200.workloads), resident in HBM before the timed region; the timed steps
+rotate over R buffer sets whose total size exceeds twice the L2 so every step reads HBM.
+
+Reported beside `value`:
+  e2e          the same metric through the host-buffer C-ABI call (pinned host memory, H2D of A, B
+               and D2H of C inside every step);
+  roofline     the dominant kernel (mode-wise matrix product): conventional 8 N^3 L flops per launch
+               / its mean launch duration (CUDA events on the library stream, second pass of K steps
+               with the library's stage profiler on) against the FP64 tensor-pipe peak measured
+               in-run by nspt_probe_fp64_peak (MEASURED_PEAKS.json has no FP64 entry);
+  cpu_baseline the oracle (naive O(N_trunc^2) convolution, C + OpenMP) on this box's host cores,
+               one full product of the same workload, rank 0 at N=1 only.
+
+Multi-GPU: the path does not shard ("replicas only"): --gpus N runs N independent
+replicas, one process per GPU (torchrun), no data-path collective; value = products of all ranks
+/ max-over-ranks time, scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "series_star_products_per_sec"
+L2_BYTES = 126e6
+
+WORKLOADS = {
+    # name: (kind, N, Ntrunc, batch, seed)
+    "cfg3": ("product", 225, 63, 1, 3),
+    "cfg2": ("product", 225, 31, 1, 2),
+    "batched4": ("batched", 225, 31, 4, 2),
+    "staple": ("staple", 225, 31, 1, 4),
+    "small": ("product", 9, 7, 1, 0),
+}
+
+
+def transform_length(Ntrunc: int) -> int:
+    L = 1
+    while L < 2 * Ntrunc + 1:
+        L *= 2
+    return L
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    return rank, local, world
+
+
+def max_over_ranks(value: float, world: int, device=None) -> float:
+    """Max of a scalar over all ranks (torch.distributed if initialised; identity otherwise)."""
+    if world <= 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(value: float, world: int, device=None) -> float:
+    if world <= 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def aggregate_throughput(units_this_rank: float, ms_this_rank: float, world: int, device=None):
+    """Whole-job throughput: units of all ranks / max-over-ranks time.  Returns (units/s, ms)."""
+    ms = max_over_ranks(ms_this_rank, world, device)
+    units = sum_over_ranks(units_this_rank, world, device)
+    return units / (ms * 1e-3), ms
+
+
+# ------------------------------------------------------------------------------------ clocks
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.index = index
+        self.samples = []
+        self.reasons = set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        self._nvml = None
+
+    def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nvml = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nvml = None
+            return self
+        self._thread = threading.Thread(target=self._run, daemon=True)
+        self._thread.start()
+        return self
+
+    def _run(self):
+        nv = self._nvml
+        names = {
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def stop(self):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join(timeout=2.0)
+        med = int(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------ inputs
+
+def make_inputs(kind, N, Ntrunc, batch, seed):
+    from paper_2001_02835_b200 import workloads as wl
+    if kind == "staple":
+        U, z = wl.config_staple(N, Ntrunc, seed=seed)
+        return {"U": U, "z": z}
+    if kind == "batched":
+        rng = np.random.default_rng(seed)
+        A = np.stack([wl.unitary_series(N, Ntrunc, rng) for _ in range(batch)])
+        B = np.stack([wl.unitary_series(N, Ntrunc, rng) for _ in range(batch)])
+        return {"A": A, "B": B}
+    if N <= 16:
+        A, B = wl.config1_gaussian()
+    else:
+        A, B = wl.config_product(N, Ntrunc, seed=seed)
+    return {"A": A, "B": B}
+
+
+# ------------------------------------------------------------------------------------ reference arm
+
+def run_reference(args):
+    """The oracle as the reference arm: same metric, each step a bounded sample of the workload."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    import oracle
+    kind, N, Ntrunc, batch, seed = WORKLOADS[args.workload]
+    if kind != "product":
+        kind, N, Ntrunc, batch, seed = WORKLOADS["cfg3"]
+    inp = make_inputs("product", N, Ntrunc, 1, seed)
+    A, B = inp["A"], inp["B"]
+    # sample: a few rows of every order; one product = N rows
+    nrows = max(1, min(N, int(round(N * 0.04))))
+    rows = np.linspace(0, N - 1, nrows).astype(np.int32)
+    for _ in range(args.warmup):
+        oracle.series_mul_rows(A, B, rows)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.series_mul_rows(A, B, rows)
+    dt = time.perf_counter() - t0
+    value = (args.steps * nrows / N) / dt
+    cores = oracle.num_threads()
+    sample = f"{nrows} of {N} rows of every order of one product per step (oracle.series_mul_rows), scaled to whole products"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "products/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"single star-product A*B, N={N}, N_trunc={Ntrunc}, complex128 (BASELINE.json configs[2])"},
+        "cpu_baseline": {"value": value, "unit": "products/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "products/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------ CUDA arm
+
+def run_cuda(args):
+    import torch
+    rank, local, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2001_02835_b200 import build as nspt_build
+    nspt_build.build()
+    from paper_2001_02835_b200 import binding as nspt
+
+    kind, N, Ntrunc, batch, seed = WORKLOADS[args.workload]
+    L = transform_length(Ntrunc)
+    n = Ntrunc + 1
+    inp = make_inputs(kind, N, Ntrunc, batch, seed)
+
+    stream = torch.cuda.Stream(device=dev)
+    nspt.nspt_set_stream(stream.cuda_stream)
+    nspt.nspt_set_order_scale(1.0)
+    nspt.nspt_set_gemm_variant(1)
+
+    series_bytes = n * N * N * 16 * batch
+    with torch.cuda.stream(stream):
+        if kind == "staple":
+            per_set = 8 * series_bytes
+            R = max(2, int(np.ceil(2 * L2_BYTES / per_set)))
+            U0 = [torch.from_numpy(u).to(dev) for u in inp["U"]]
+            sets = []
+            for r in range(R):
+                U = [u.roll(r, dims=-1).contiguous() for u in U0] if r else U0
+                S = [torch.empty_like(u) for u in U]
+                sets.append((U, S))
+            z = inp["z"]
+
+            def step(i):
+                U, S = sets[i % R]
+                nspt.nspt_staple(U, z, S)
+            products_per_step = 52
+            units_name = "staples"
+        else:
+            per_set = 3 * series_bytes
+            R = max(2, int(np.ceil(2 * L2_BYTES / per_set)))
+            A0 = torch.from_numpy(inp["A"]).to(dev)
+            B0 = torch.from_numpy(inp["B"]).to(dev)
+            sets = []
+            for r in range(R):
+                A = A0.roll(r, dims=-1).contiguous() if r else A0
+                B = B0.roll(r, dims=-2).contiguous() if r else B0
+                sets.append((A, B, torch.empty_like(A)))
+            if kind == "batched":
+                def step(i):
+                    A, B, C = sets[i % R]
+                    nspt.nspt_series_mul_batched(A, B, C)
+            else:
+                def step(i):
+                    A, B, C = sets[i % R]
+                    nspt.nspt_series_mul(A, B, C)
+            products_per_step = batch
+            units_name = "products"
+    stream.synchronize()
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    W, K = max(3, args.warmup), args.steps
+    for i in range(W):
+        step(i)
+    stream.synchronize()
+
+    # ---- timed region 1: K steps, inputs resident in HBM, CUDA events on the library stream
+    ev0 = torch.cuda.Event(enable_timing=True)
+    ev1 = torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local).start()
+    launches0 = nspt.nspt_launch_count()
+    barrier()
+    ev0.record(stream)
+    for i in range(K):
+        step(i)
+    ev1.record(stream)
+    barrier()
+    ms_local = ev0.elapsed_time(ev1)
+    launches = nspt.nspt_launch_count() - launches0
+    clocks = sampler.stop()
+    value, ms_total = aggregate_throughput(K * (products_per_step if kind != "staple" else 1), ms_local, world, dev)
+
+    # ---- timed region 2: the same K steps with the stage profiler on -> per-kernel durations
+    nspt.nspt_profile(True)
+    for name in nspt.STAGES:
+        nspt.nspt_profile_read(name)
+    for i in range(K):
+        step(i)
+    stage_ms = {}
+    for name in nspt.STAGES:
+        ms, cnt = nspt.nspt_profile_read(name)
+        if cnt:
+            stage_ms[name] = {"ms_total": ms, "launches": cnt, "ms_per_launch": ms / cnt}
+    nspt.nspt_profile(False)
+
+    # ---- roofline of the dominant kernel (mode-wise matrix product)
+    line_extra = {}
+    if rank == 0:
+        fp64_peak = nspt.nspt_probe_fp64_peak()
+        gemm = stage_ms.get("zgemm_modes")
+        flops_per_launch = 8.0 * N ** 3 * L * batch
+        achieved = flops_per_launch / (gemm["ms_per_launch"] * 1e-3) * 1e-12 if gemm else None
+        traffic = None
+        tfile = ROOT / "profiles" / "traffic.json"
+        if tfile.exists():
+            try:
+                traffic = json.loads(tfile.read_text()).get(args.workload, {}).get("zgemm_modes_dram_bytes_per_launch")
+            except Exception:
+                traffic = None
+        peaks = {}
+        pfile = ROOT / "MEASURED_PEAKS.json"
+        if pfile.exists():
+            try:
+                peaks = json.loads(pfile.read_text())
+            except Exception:
+                peaks = {}
+        hbm = peaks.get("hbm_gbs", 6650.0)
+        hbm_src = "MEASURED_PEAKS.json" if "hbm_gbs" in peaks else "fallback 6.65 TB/s"
+        fft_bytes = {  # algorithmic bytes per launch
+            "fft_forward": 2 * (n + L) * N * N * 16 * batch,      # two operands: read n*e, write L*e each
+            "fft_inverse": (L + n) * N * N * 16 * batch,
+            "fft_retruncate": 2 * L * N * N * 16,
+        }
+        stages_out = {}
+        for name, st in stage_ms.items():
+            o = {"launches_per_step": st["launches"] / K, "us_per_launch": st["ms_per_launch"] * 1e3}
+            if name in fft_bytes:
+                gbs = fft_bytes[name] / (st["ms_per_launch"] * 1e-3) * 1e-9
+                o.update({"algorithmic_GB_s": gbs, "frac_of_hbm_peak": gbs / hbm})
+            stages_out[name] = o
+        t_gemm_roof = flops_per_launch / (fp64_peak * 1e12)
+        t_fft_roof = 9.0 * n * N * N * 16 * batch / (hbm * 1e9)
+        roof_time = max(t_gemm_roof, t_fft_roof)
+        line_extra["roofline"] = {
+            "bound": "tensor", "kernel": "zgemm_modes_dmma_kernel (FP64 tensor pipe, DMMA.8x8x4)",
+            "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
+            "frac": (achieved / fp64_peak) if achieved else None, "traffic": traffic,
+            "flops_basis": "conventional 8*N^3*L per launch; the kernel executes 6*N^3*L (3-multiplication complex product)",
+            "achieved_executed": (achieved * 0.75) if achieved else None,
+            "peak_source": "nspt_probe_fp64_peak: DMMA m8n8k4 chain, measured in this run (MEASURED_PEAKS.json has no FP64 entry)",
+            "hbm_peak_GB_s": hbm, "hbm_peak_source": hbm_src,
+        }
+        if kind != "staple":
+            step_s = ms_local / K * 1e-3
+            line_extra["fftconv_roofline"] = {
+                "definition": "slower of 8*N^3*L flops at FP64 peak and 9*n*16*N^2 bytes at HBM peak (SURVEY.md 8d)",
+                "roofline_products_per_s": batch / roof_time, "t_gemm_us": t_gemm_roof * 1e6, "t_fft_us": t_fft_roof * 1e6,
+                "frac": roof_time / step_s if step_s else None,
+            }
+        line_extra["stages"] = stages_out
+
+    # ---- e2e: host buffers through the C ABI, H2D and D2H inside the timed region
+    e2e = None
+    if kind in ("product", "batched"):
+        hA = torch.from_numpy(inp["A"]).pin_memory()
+        hB = torch.from_numpy(inp["B"]).pin_memory()
+        hC = torch.empty_like(hA).pin_memory()
+        call = nspt.nspt_series_mul_batched_host if kind == "batched" else nspt.nspt_series_mul_host
+        Ke = max(3, min(K, 20))
+        for _ in range(2):
+            call(hA, hB, hC)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(Ke):
+            call(hA, hB, hC)          # synchronous: returns after the D2H copy
+        torch.cuda.synchronize(dev)
+        dt_ms = (time.perf_counter() - t0) * 1e3
+        e2e_value, _ = aggregate_throughput(Ke * products_per_step, dt_ms, world, dev)
+        e2e = {"value": e2e_value, "unit": f"{units_name}/s", "h2d_bytes_per_step": 2 * series_bytes,
+               "d2h_bytes_per_step": series_bytes, "steps": Ke,
+               "how": "nspt_series_mul_host with pinned host buffers; wall clock around synchronous calls"}
+    elif kind == "staple":
+        hU = [torch.from_numpy(u).pin_memory() for u in inp["U"]]
+        hS = [torch.empty_like(u).pin_memory() for u in hU]
+        Ke = max(2, min(K, 5))
+        nspt.nspt_staple_host(hU, z, hS)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(Ke):
+            nspt.nspt_staple_host(hU, z, hS)
+        torch.cuda.synchronize(dev)
+        dt_ms = (time.perf_counter() - t0) * 1e3
+        e2e_value, _ = aggregate_throughput(Ke, dt_ms, world, dev)
+        e2e = {"value": e2e_value, "unit": "staples/s", "h2d_bytes_per_step": 4 * series_bytes,
+               "d2h_bytes_per_step": 4 * series_bytes, "steps": Ke,
+               "how": "nspt_staple_host with pinned host buffers; wall clock around synchronous calls"}
+
+    # ---- CPU baseline: the oracle on this box's cores (rank 0, single-GPU runs only)
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        if kind == "staple":
+            # one of the 52 products of the literal staple, scaled
+            t0 = time.perf_counter()
+            oracle.series_mul(inp["U"][0], inp["U"][1])
+            dt = time.perf_counter() - t0
+            cpu_baseline = {"value": 1.0 / (52 * dt), "unit": "staples/s", "cores": oracle.num_threads(), "kind": "oracle",
+                            "sample": "1 of the 52 star-products of the literal staple (oracle.series_mul), scaled by 52"}
+        else:
+            A = inp["A"] if kind == "product" else inp["A"][0]
+            B = inp["B"] if kind == "product" else inp["B"][0]
+            t0 = time.perf_counter()
+            ref = oracle.series_mul(A, B)
+            dt = time.perf_counter() - t0
+            cpu_baseline = {"value": 1.0 / dt, "unit": "products/s", "cores": oracle.num_threads(), "kind": "oracle",
+                            "sample": f"1 full star-product N={N} N_trunc={Ntrunc} (oracle.series_mul, naive O(N_trunc^2))"}
+            # parity spot check of the timed configuration against the same oracle result
+            with torch.cuda.stream(stream):
+                Cchk = nspt.nspt_series_mul(sets[0][0] if kind == "product" else sets[0][0][0].contiguous(),
+                                            sets[0][1] if kind == "product" else sets[0][1][0].contiguous())
+            stream.synchronize()
+            err = oracle.per_order_error(Cchk.cpu().numpy(), ref, oracle.product_bound(A, B)).max()
+            line_extra["parity_max_err_over_bound"] = float(err)
+
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+
+    desc = {
+        "cfg3": "single star-product A*B, N=225, N_trunc=63 (L=128), complex128, A,B = exp(i sum g^k H_k) series (BASELINE.json configs[2])",
+        "cfg2": "single star-product A*B, N=225, N_trunc=31 (L=64), complex128 (BASELINE.json configs[1])",
+        "batched4": "batch of 4 star-products, N=225, N_trunc=31 (the four P_mu*U_mu of a link update)",
+        "staple": "full TEK staple S_mu, mu=1..4, N=225, N_trunc=31, k=4 twist (BASELINE.json configs[3]); 52 star-products per step",
+        "small": "single star-product A*B, N=9, N_trunc=7 (BASELINE.json configs[0])",
+    }[args.workload]
+    line = {
+        "metric": METRIC if kind != "staple" else "tek_staples_per_sec",
+        "value": value, "unit": f"{units_name}/s", "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": desc, "N": N, "N_trunc": Ntrunc, "L": L, "batch": batch,
+                   "parallelism": "replicas only (no data-path collective)" if world > 1 else "single GPU",
+                   "l2": f"inputs rotate over {R} buffer sets, {R * per_set / 1e6:.0f} MB total > 2 x L2 (126 MB)"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+    }
+    line.update(line_extra)
+    if cpu_baseline is not None:
+        line["cpu_baseline"] = cpu_baseline
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = args.steps if args.steps is not None else 5
+        args.warmup = args.warmup if args.warmup is not None else 1
+        return run_reference(args)
+    args.steps = args.steps if args.steps is not None else (200 if args.workload != "staple" else 10)
+    args.warmup = args.warmup if args.warmup is not None else 5
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

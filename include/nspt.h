@@ -134,6 +134,11 @@ int nspt_set_gemm_variant(int variant);
 int nspt_profile(int enable);
 int nspt_profile_read(int stage, double* ms, long long* launches);
 
+/* Measure the FP64 tensor-pipe peak of the current device (TFLOP/s) with a DMMA.8x8x4 chain
+ * microbenchmark on the legacy default stream (about 50 ms, synchronous).  This is the roofline
+ * denominator for the mode-wise matrix product; it is not part of the hot path. */
+int nspt_probe_fp64_peak(double* tflops);
+
 /* Total kernels launched by the library since it was loaded. */
 long long nspt_launch_count(void);
 

@@ -26,7 +26,7 @@ EXPORTS = [
     "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple",
     "nspt_series_mul_host", "nspt_series_mul_batched_host", "nspt_staple_host",
     "nspt_set_stream", "nspt_set_order_scale", "nspt_workspace_bytes", "nspt_set_workspace",
-    "nspt_set_gemm_variant", "nspt_profile", "nspt_profile_read", "nspt_launch_count",
+    "nspt_set_gemm_variant", "nspt_probe_fp64_peak", "nspt_profile", "nspt_profile_read", "nspt_launch_count",
     "nspt_release", "nspt_strerror", "nspt_version",
 ]
 
@@ -55,6 +55,7 @@ _lib.nspt_set_order_scale.argtypes = [_dbl]
 _lib.nspt_workspace_bytes.argtypes = [_int, _int, _int, _int, ctypes.POINTER(ctypes.c_size_t)]
 _lib.nspt_set_workspace.argtypes = [_vp, ctypes.c_size_t]
 _lib.nspt_set_gemm_variant.argtypes = [_int]
+_lib.nspt_probe_fp64_peak.argtypes = [ctypes.POINTER(_dbl)]
 _lib.nspt_profile.argtypes = [_int]
 _lib.nspt_profile_read.argtypes = [_int, ctypes.POINTER(_dbl), ctypes.POINTER(ctypes.c_longlong)]
 _lib.nspt_launch_count.restype = ctypes.c_longlong
@@ -239,6 +240,13 @@ def nspt_profile_read(stage):
     ms, n = _dbl(0.0), ctypes.c_longlong(0)
     _check(_lib.nspt_profile_read(int(stage), ctypes.byref(ms), ctypes.byref(n)), "nspt_profile_read")
     return float(ms.value), int(n.value)
+
+
+def nspt_probe_fp64_peak() -> float:
+    """Measured FP64 tensor-pipe (DMMA) peak of the current device in TFLOP/s."""
+    out = _dbl(0.0)
+    _check(_lib.nspt_probe_fp64_peak(ctypes.byref(out)), "nspt_probe_fp64_peak")
+    return float(out.value)
 
 
 def nspt_launch_count() -> int:
