@@ -20,7 +20,17 @@
 // Re-truncation (needed between chained products in the staple) fuses inverse, truncation and
 // forward: the orders a thread holds after the pruned inverse are exactly its phase-1 inputs of
 // the forward transform, so no extra exchange is needed.
+//
+// Data movement.  The kernels are HBM-bound (about 1.5 flop per byte), so what matters is keeping
+// loads in flight while a tile is being transformed.  For L >= 16 the kernels are persistent: each
+// CTA walks over tiles of T elements, and the [order][T] input tile of the tile after next is
+// fetched by one TMA box load (cp.async.bulk.tensor, mbarrier complete_tx) into a two-deep ring of
+// shared-memory stages while the current tile is in registers.  Rows beyond Ntrunc and elements
+// beyond N^2 are zero-filled by TMA, which is exactly the zero padding of Step 1.  Results leave
+// with coalesced 16-byte stores (fire and forget).  L <= 8 needs one thread per element and no
+// shared memory; those kernels use plain loads.
 #include "nspt_internal.cuh"
+#include "nspt_tma.cuh"
 
 namespace nspt {
 namespace {
@@ -119,12 +129,14 @@ struct Dft<1, SIGN, ZERO_UPPER, HALF_OUT> {
 
 struct XformParams {
     const double2* src_series[2];  // forward input (interleaved)
-    const double* src_freq;        // inverse / retruncate input (planar)
-    double* dst_freq[2];           // forward / retruncate output (planar)
+    const double2* src_freq;       // inverse / retruncate input (spectrum)
+    double2* dst_freq[2];          // forward / retruncate output (spectrum)
     double2* dst_series;           // inverse output
     size_t NN;
-    size_t ps;
-    int N, ld, n;
+    int N, n;
+    int batch;
+    unsigned tiles_x;              // tiles per (operand, batch) = ceil(NN / T)
+    unsigned total_tiles;
     const double2* tw_fwd;
     const double2* tw_inv;
     const double* scale_in;
@@ -133,20 +145,19 @@ struct XformParams {
     int use_scale;
 };
 
-// ---- forward phases: registers x[r] = coefficient of order S*r + s (r < R/2 non-zero) -> planes
+// ---- forward phases: registers x[r] = coefficient of order S*r + s (r < R/2 non-zero) -> spectrum.
+// For S > 1 the exchange buffer `sm` must be free on entry; on return every thread has passed the
+// __syncthreads that follows the phase-1 writes, but phase-2 reads of `sm` may still be in flight.
 template <int R, int S, int T>
-__device__ __forceinline__ void forward_from_regs(double2 (&x)[R], int s, int c, bool valid, double* out_re,
-                                                  size_t ps, const double2* __restrict__ tw, double2* sm) {
+__device__ __forceinline__ void forward_from_regs(double2 (&x)[R], int s, int c, bool valid, double2* out,
+                                                  size_t NN, const double2* __restrict__ tw, double2* sm) {
     constexpr bool ZU = (R >= 2);
     double2 Y[R];
     Dft<R, +1, ZU, false>::run(x, Y);
     if constexpr (S == 1) {
         if (valid) {
 #pragma unroll
-            for (int p1 = 0; p1 < R; ++p1) {
-                out_re[(size_t)(2 * p1) * ps] = Y[p1].x;
-                out_re[(size_t)(2 * p1 + 1) * ps] = Y[p1].y;
-            }
+            for (int p1 = 0; p1 < R; ++p1) out[(size_t)p1 * NN] = Y[p1];
         }
     } else {
 #pragma unroll
@@ -164,18 +175,15 @@ __device__ __forceinline__ void forward_from_regs(double2 (&x)[R], int s, int c,
             Dft<S, +1, false, false>::run(y, X);
             if (valid) {
 #pragma unroll
-                for (int p2 = 0; p2 < S; ++p2) {
-                    const int p = p1 + R * p2;
-                    out_re[(size_t)(2 * p) * ps] = X[p2].x;
-                    out_re[(size_t)(2 * p + 1) * ps] = X[p2].y;
-                }
+                for (int p2 = 0; p2 < S; ++p2) out[(size_t)(p1 + R * p2) * NN] = X[p2];
             }
         }
     }
 }
 
-// ---- inverse phases: planes -> registers.  On return, for S > 1, xk[a][k2] holds the UNSCALED
-// sum for order k = (s + S a) + R k2 (k2 < S/2); for S == 1, xk[0][k1] holds order k1 (k1 < R).
+// ---- inverse phases: registers x[r] = mode S*r + s -> registers.  On return, for S > 1, v[a][k2]
+// holds the UNSCALED sum for order k = (s + S a) + R k2 (k2 < S/2); for S == 1, v[0][k1] holds
+// order k1 (k1 < R).  Same shared-memory contract as forward_from_regs.
 template <int R, int S, int T>
 struct InvRegs {
     static constexpr int A = (S == 1) ? 1 : R / S;
@@ -184,16 +192,9 @@ struct InvRegs {
 };
 
 template <int R, int S, int T>
-__device__ __forceinline__ void inverse_to_regs(const double* in_re, size_t ps, int s, int c, bool valid,
-                                                const double2* __restrict__ tw, double2* sm,
-                                                InvRegs<R, S, T>& out) {
-    double2 x[R], Y[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int p = S * r + s;
-        x[r] = valid ? make_double2(__ldg(&in_re[(size_t)(2 * p) * ps]), __ldg(&in_re[(size_t)(2 * p + 1) * ps]))
-                     : make_double2(0.0, 0.0);
-    }
+__device__ __forceinline__ void inverse_from_regs(double2 (&x)[R], int s, int c, const double2* __restrict__ tw,
+                                                  double2* sm, InvRegs<R, S, T>& out) {
+    double2 Y[R];
     Dft<R, -1, false, false>::run(x, Y);
     if constexpr (S == 1) {
 #pragma unroll
@@ -218,85 +219,17 @@ __device__ __forceinline__ void inverse_to_regs(const double* in_re, size_t ps, 
     }
 }
 
+// orders held after the pruned inverse -> phase-1 inputs of the forward transform (times 1/L,
+// orders > Ntrunc dropped)
 template <int R, int S, int T>
-__global__ void __launch_bounds__(T* S) fft_forward_kernel(const XformParams P) {
-    extern __shared__ double2 sm[];
-    const int c = threadIdx.x % T, s = threadIdx.x / T;
-    const size_t e = (size_t)blockIdx.x * T + c;
-    const bool valid = e < P.NN;
-    const int b = blockIdx.y, z = blockIdx.z;
-    constexpr int L = R * S;
-    const double2* in = (z ? P.src_series[1] : P.src_series[0]) + (size_t)b * P.n * P.NN + e;
-    double2 x[R];
-    constexpr int RH = (R >= 2) ? R / 2 : 1;
-#pragma unroll
-    for (int r = 0; r < RH; ++r) {
-        const int k = S * r + s;
-        double2 v = make_double2(0.0, 0.0);
-        if (valid && k < P.n) {
-            v = __ldg(&in[(size_t)k * P.NN]);
-            if (P.use_scale) {
-                const double sc = __ldg(&P.scale_in[k]);
-                v.x *= sc;
-                v.y *= sc;
-            }
-        }
-        x[r] = v;
-    }
-#pragma unroll
-    for (int r = RH; r < R; ++r) x[r] = make_double2(0.0, 0.0);
-    const size_t off = valid ? (e / P.N) * P.ld + (e % P.N) : 0;
-    double* out_re = (z ? P.dst_freq[1] : P.dst_freq[0]) + (size_t)b * L * 2 * P.ps + off;
-    forward_from_regs<R, S, T>(x, s, c, valid, out_re, P.ps, P.tw_fwd, sm);
-}
-
-template <int R, int S, int T>
-__global__ void __launch_bounds__(T* S) fft_inverse_kernel(const XformParams P) {
-    extern __shared__ double2 sm[];
-    const int c = threadIdx.x % T, s = threadIdx.x / T;
-    const size_t e = (size_t)blockIdx.x * T + c;
-    const bool valid = e < P.NN;
-    const int b = blockIdx.y;
-    constexpr int L = R * S;
-    const size_t off = valid ? (e / P.N) * P.ld + (e % P.N) : 0;
-    const double* in_re = P.src_freq + (size_t)b * L * 2 * P.ps + off;
-    InvRegs<R, S, T> q;
-    inverse_to_regs<R, S, T>(in_re, P.ps, s, c, valid, P.tw_inv, sm, q);
-    if (!valid) return;
-    double2* out = P.dst_series + (size_t)b * P.n * P.NN + e;
-#pragma unroll
-    for (int a = 0; a < InvRegs<R, S, T>::A; ++a)
-#pragma unroll
-        for (int k2 = 0; k2 < InvRegs<R, S, T>::K2; ++k2) {
-            const int k = (S == 1) ? k2 : (s + S * a) + R * k2;
-            if (k < P.n) {
-                const double sc = __ldg(&P.scale_out[k]);  // s^-k / L
-                out[(size_t)k * P.NN] = make_double2(q.v[a][k2].x * sc, q.v[a][k2].y * sc);
-            }
-        }
-}
-
-template <int R, int S, int T>
-__global__ void __launch_bounds__(T* S) fft_retruncate_kernel(const XformParams P) {
-    extern __shared__ double2 sm[];
-    const int c = threadIdx.x % T, s = threadIdx.x / T;
-    const size_t e = (size_t)blockIdx.x * T + c;
-    const bool valid = e < P.NN;
-    const int b = blockIdx.y;
-    constexpr int L = R * S;
-    const size_t off = valid ? (e / P.N) * P.ld + (e % P.N) : 0;
-    const double* in_re = P.src_freq + (size_t)b * L * 2 * P.ps + off;
-    InvRegs<R, S, T> q;
-    inverse_to_regs<R, S, T>(in_re, P.ps, s, c, valid, P.tw_inv, sm, q);
-    // orders this thread holds are k = s + S r with r = a + (R/S) k2 (S > 1) or r = k1 (S == 1)
-    double2 x[R];
+__device__ __forceinline__ void retruncate_regs(const InvRegs<R, S, T>& q, int s, int n, double inv_L, double2 (&x)[R]) {
     constexpr int RH = (R >= 2) ? R / 2 : 1;
 #pragma unroll
     for (int r = 0; r < R; ++r) x[r] = make_double2(0.0, 0.0);
     if constexpr (S == 1) {
 #pragma unroll
         for (int r = 0; r < RH; ++r)
-            if (r < P.n) x[r] = make_double2(q.v[0][r].x * P.inv_L, q.v[0][r].y * P.inv_L);
+            if (r < n) x[r] = make_double2(q.v[0][r].x * inv_L, q.v[0][r].y * inv_L);
     } else {
 #pragma unroll
         for (int a = 0; a < R / S; ++a)
@@ -304,109 +237,366 @@ __global__ void __launch_bounds__(T* S) fft_retruncate_kernel(const XformParams 
             for (int k2 = 0; k2 < S / 2; ++k2) {
                 const int r = a + (R / S) * k2;
                 const int k = s + S * r;
-                if (k < P.n) x[r] = make_double2(q.v[a][k2].x * P.inv_L, q.v[a][k2].y * P.inv_L);
+                if (k < n) x[r] = make_double2(q.v[a][k2].x * inv_L, q.v[a][k2].y * inv_L);
             }
-        __syncthreads();  // shared memory is reused by the forward phases
     }
-    double* out_re = P.dst_freq[0] + (size_t)b * L * 2 * P.ps + off;
-    forward_from_regs<R, S, T>(x, s, c, valid, out_re, P.ps, P.tw_fwd, sm);
+}
+
+template <int R, int S, int T>
+__device__ __forceinline__ void store_series(const InvRegs<R, S, T>& q, int s, int n, const double* __restrict__ scale_out,
+                                             double2* out, size_t NN) {
+#pragma unroll
+    for (int a = 0; a < InvRegs<R, S, T>::A; ++a)
+#pragma unroll
+        for (int k2 = 0; k2 < InvRegs<R, S, T>::K2; ++k2) {
+            const int k = (S == 1) ? k2 : (s + S * a) + R * k2;
+            if (k < n) {
+                const double sc = __ldg(&scale_out[k]);  // s^-k / L
+                out[(size_t)k * NN] = make_double2(q.v[a][k2].x * sc, q.v[a][k2].y * sc);
+            }
+        }
+}
+
+// =================================================================================================
+// L <= 8: one thread per element, plain loads (S == 1)
+// =================================================================================================
+template <int R, int T>
+__global__ void __launch_bounds__(T) fft_forward_small_kernel(const XformParams P) {
+    const int c = threadIdx.x;
+    const size_t e = (size_t)blockIdx.x * T + c;
+    const bool valid = e < P.NN;
+    const int b = blockIdx.y, z = blockIdx.z;
+    const double2* in = (z ? P.src_series[1] : P.src_series[0]) + (size_t)b * P.n * P.NN + e;
+    double2 x[R];
+    constexpr int RH = (R >= 2) ? R / 2 : 1;
+#pragma unroll
+    for (int r = 0; r < R; ++r) x[r] = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int r = 0; r < RH; ++r) {
+        if (valid && r < P.n) {
+            double2 v = __ldg(&in[(size_t)r * P.NN]);
+            if (P.use_scale) {
+                const double sc = __ldg(&P.scale_in[r]);
+                v.x *= sc;
+                v.y *= sc;
+            }
+            x[r] = v;
+        }
+    }
+    double2* out = (z ? P.dst_freq[1] : P.dst_freq[0]) + (size_t)b * R * P.NN + e;
+    forward_from_regs<R, 1, T>(x, 0, c, valid, out, P.NN, P.tw_fwd, nullptr);
+}
+
+template <int R, int T, bool RETRUNC>
+__global__ void __launch_bounds__(T) fft_inverse_small_kernel(const XformParams P) {
+    const int c = threadIdx.x;
+    const size_t e = (size_t)blockIdx.x * T + c;
+    if (e >= P.NN) return;
+    const int b = blockIdx.y;
+    const double2* in = P.src_freq + (size_t)b * R * P.NN + e;
+    double2 x[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) x[r] = __ldg(&in[(size_t)r * P.NN]);
+    InvRegs<R, 1, T> q;
+    inverse_from_regs<R, 1, T>(x, 0, c, P.tw_inv, nullptr, q);
+    if constexpr (RETRUNC) {
+        double2 xf[R];
+        retruncate_regs<R, 1, T>(q, 0, P.n, P.inv_L, xf);
+        forward_from_regs<R, 1, T>(xf, 0, c, true, P.dst_freq[0] + (size_t)b * R * P.NN + e, P.NN, P.tw_fwd, nullptr);
+    } else {
+        store_series<R, 1, T>(q, 0, P.n, P.scale_out, P.dst_series + (size_t)b * P.n * P.NN + e, P.NN);
+    }
+}
+
+// =================================================================================================
+// L >= 16: persistent CTAs, TMA-staged input tiles
+// =================================================================================================
+template <int R, int S, int T>
+struct Cfg {
+    static constexpr int L = R * S;
+    static constexpr int THREADS = T * S;
+    static constexpr int EXCH_BYTES = L * T * 16;            // exchange buffer [p1][s][c]
+    static constexpr int FWD_STAGE_BYTES = (L / 2) * T * 16;  // input tile [order < L/2][T]
+    static constexpr int INV_STAGE_BYTES = L * T * 16;        // input tile [mode][T]; doubles as the exchange buffer
+    static constexpr int FWD_SMEM = EXCH_BYTES + 2 * FWD_STAGE_BYTES + 16 + 128;
+    static constexpr int INV_SMEM = 2 * INV_STAGE_BYTES + 16 + 128;
+};
+
+__device__ __forceinline__ void tile_coords(unsigned tile, const XformParams& P, unsigned& tx, unsigned& b, unsigned& z) {
+    tx = tile % P.tiles_x;
+    const unsigned zb = tile / P.tiles_x;
+    b = zb % (unsigned)P.batch;
+    z = zb / (unsigned)P.batch;
+}
+
+template <int R, int S, int T>
+__global__ void __launch_bounds__(T* S) fft_forward_tma_kernel(const __grid_constant__ CUtensorMap map0,
+                                                              const __grid_constant__ CUtensorMap map1,
+                                                              const XformParams P) {
+    using C = Cfg<R, S, T>;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
+    uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));
+    double2* exch = reinterpret_cast<double2*>(sgen);
+    const uint32_t stage_addr = base + C::EXCH_BYTES;
+    const double2* stage_gen = reinterpret_cast<const double2*>(sgen + C::EXCH_BYTES);
+    const uint32_t bar = stage_addr + 2 * C::FWD_STAGE_BYTES;  // two 8-byte mbarriers
+
+    const int c = threadIdx.x % T, s = threadIdx.x / T;
+
+    auto issue = [&](unsigned tile, int stage) {
+        unsigned tx, b, z;
+        tile_coords(tile, P, tx, b, z);
+        mbar_expect_tx(bar + 8 * stage, C::FWD_STAGE_BYTES);
+        tma_load_3d(stage_addr + stage * C::FWD_STAGE_BYTES, z ? &map1 : &map0, bar + 8 * stage, (int)(2 * tx * T), 0, (int)b);
+    };
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_init(bar + 8, 1);
+        mbar_fence_init();
+        if (blockIdx.x < P.total_tiles) issue(blockIdx.x, 0);
+        if (blockIdx.x + gridDim.x < P.total_tiles) issue(blockIdx.x + gridDim.x, 1);
+    }
+    __syncthreads();
+
+    unsigned it = 0;
+    for (unsigned tile = blockIdx.x; tile < P.total_tiles; tile += gridDim.x, ++it) {
+        const int stage = it & 1;
+        unsigned tx, b, z;
+        tile_coords(tile, P, tx, b, z);
+        const size_t e = (size_t)tx * T + c;
+        const bool valid = e < P.NN;
+        mbar_wait(bar + 8 * stage, (it >> 1) & 1);
+        const double2* in = stage_gen + (size_t)stage * (C::FWD_STAGE_BYTES / 16);
+        double2 x[R];
+#pragma unroll
+        for (int r = 0; r < R / 2; ++r) {
+            const int k = S * r + s;
+            double2 v = in[k * T + c];  // rows >= n and elements >= N^2 were zero-filled by TMA
+            if (P.use_scale && k < P.n) {
+                const double sc = __ldg(&P.scale_in[k]);
+                v.x *= sc;
+                v.y *= sc;
+            }
+            x[r] = v;
+        }
+#pragma unroll
+        for (int r = R / 2; r < R; ++r) x[r] = make_double2(0.0, 0.0);
+        double2* out = (z ? P.dst_freq[1] : P.dst_freq[0]) + (size_t)b * C::L * P.NN + e;
+        // phase 1 + __syncthreads (all threads have consumed the input stage) + phase 2
+        {
+            double2 Y[R];
+            Dft<R, +1, true, false>::run(x, Y);
+#pragma unroll
+            for (int p1 = 0; p1 < R; ++p1) {
+                const double2 w = __ldg(&P.tw_fwd[s * p1]);
+                exch[(p1 * S + s) * T + c] = (p1 == 0) ? Y[p1] : cmul(Y[p1], w);
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned next = tile + 2 * gridDim.x;
+            if (next < P.total_tiles) issue(next, stage);
+        }
+#pragma unroll
+        for (int a = 0; a < R / S; ++a) {
+            const int p1 = s + S * a;
+            double2 y[S], X[S];
+#pragma unroll
+            for (int sp = 0; sp < S; ++sp) y[sp] = exch[(p1 * S + sp) * T + c];
+            Dft<S, +1, false, false>::run(y, X);
+            if (valid) {
+#pragma unroll
+                for (int p2 = 0; p2 < S; ++p2) out[(size_t)(p1 + R * p2) * P.NN] = X[p2];
+            }
+        }
+        __syncthreads();  // exchange buffer free for the next tile
+    }
+}
+
+template <int R, int S, int T, bool RETRUNC>
+__global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_constant__ CUtensorMap map, const XformParams P) {
+    using C = Cfg<R, S, T>;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
+    uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));
+    const uint32_t bar = base + 2 * C::INV_STAGE_BYTES;
+
+    const int c = threadIdx.x % T, s = threadIdx.x / T;
+
+    auto issue = [&](unsigned tile, int stage) {
+        unsigned tx, b, z;
+        tile_coords(tile, P, tx, b, z);
+        mbar_expect_tx(bar + 8 * stage, C::INV_STAGE_BYTES);
+        tma_load_3d(base + stage * C::INV_STAGE_BYTES, &map, bar + 8 * stage, (int)(2 * tx * T), 0, (int)b);
+    };
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_init(bar + 8, 1);
+        mbar_fence_init();
+        if (blockIdx.x < P.total_tiles) issue(blockIdx.x, 0);
+        if (blockIdx.x + gridDim.x < P.total_tiles) issue(blockIdx.x + gridDim.x, 1);
+    }
+    __syncthreads();
+
+    unsigned it = 0;
+    for (unsigned tile = blockIdx.x; tile < P.total_tiles; tile += gridDim.x, ++it) {
+        const int stage = it & 1;
+        unsigned tx, b, z;
+        tile_coords(tile, P, tx, b, z);
+        const size_t e = (size_t)tx * T + c;
+        const bool valid = e < P.NN;
+        mbar_wait(bar + 8 * stage, (it >> 1) & 1);
+        double2* buf = reinterpret_cast<double2*>(sgen + (size_t)stage * C::INV_STAGE_BYTES);
+        double2 x[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) x[r] = buf[(S * r + s) * T + c];
+        __syncthreads();  // the stage now serves as the exchange buffer
+        InvRegs<R, S, T> q;
+        inverse_from_regs<R, S, T>(x, s, c, P.tw_inv, buf, q);
+        if constexpr (RETRUNC) {
+            double2 xf[R];
+            retruncate_regs<R, S, T>(q, s, P.n, P.inv_L, xf);
+            __syncthreads();  // phase-2 reads of the inverse are done
+            forward_from_regs<R, S, T>(xf, s, c, valid, P.dst_freq[0] + (size_t)b * C::L * P.NN + e, P.NN, P.tw_fwd, buf);
+        } else {
+            if (valid) store_series<R, S, T>(q, s, P.n, P.scale_out, P.dst_series + (size_t)b * P.n * P.NN + e, P.NN);
+        }
+        __syncthreads();  // all reads of this stage are done: refill it
+        if (threadIdx.x == 0) {
+            const unsigned next = tile + 2 * gridDim.x;
+            if (next < P.total_tiles) issue(next, stage);
+        }
+    }
 }
 
 // Spectrum of the daggered series (g is real): FFT[X^+](p) = (X~((L-p) mod L))^H.
-// dst(b,p,c)[i*ld+j] = (c ? -1 : +1) * src(b,(L-p)%L,c)[j*ld+i]; 32x32 tiles through shared memory.
-__global__ void __launch_bounds__(256) freq_dagger_kernel(const double* __restrict__ src, double* __restrict__ dst,
-                                                         int N, int ld, size_t ps, int L) {
-    __shared__ double tile[32][33];
-    const int plane = blockIdx.z;  // (b*L + p)*2 + c
-    const int c = plane & 1;
-    const int bp = plane >> 1;
+// dst(b,p)[i][j] = conj(src(b,(L-p)%L)[j][i]); 32x32 tiles through shared memory.
+__global__ void __launch_bounds__(256) freq_dagger_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
+                                                         int N, size_t NN, int L) {
+    __shared__ double2 tile[32][33];
+    const int bp = blockIdx.z;  // b*L + p
     const int b = bp / L, p = bp % L;
-    const int ps_src = (L - p) % L;
-    const double* s = src + ((size_t)(b * L + ps_src) * 2 + c) * ps;
-    double* d = dst + (size_t)plane * ps;
+    const double2* s = src + (size_t)(b * L + (L - p) % L) * NN;
+    double2* d = dst + (size_t)bp * NN;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;  // 32 x 8
     const int i0 = blockIdx.y * 32, j0 = blockIdx.x * 32;
-    // read src rows j0.., cols i0..  (src[j][i])
 #pragma unroll
     for (int r = ty; r < 32; r += 8) {
         const int j = j0 + r, i = i0 + tx;
-        tile[r][tx] = (j < N && i < N) ? s[(size_t)j * ld + i] : 0.0;
+        tile[r][tx] = (j < N && i < N) ? s[(size_t)j * N + i] : make_double2(0.0, 0.0);
     }
     __syncthreads();
-    const double sgn = c ? -1.0 : 1.0;
 #pragma unroll
     for (int r = ty; r < 32; r += 8) {
         const int i = i0 + r, j = j0 + tx;
-        if (i < N && j < N) d[(size_t)i * ld + j] = sgn * tile[tx][r];
+        if (i < N && j < N) {
+            const double2 v = tile[tx][r];
+            d[(size_t)i * N + j] = make_double2(v.x, -v.y);
+        }
     }
 }
 
-template <int R, int S, int T>
-struct Launcher {
-    static constexpr int L = R * S;
-    static constexpr size_t smem = (S == 1) ? 0 : (size_t)L * T * sizeof(double2);
-    template <typename K>
-    static cudaError_t prep(K kernel) {
-        if (smem > 48 * 1024)
-            return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        return cudaSuccess;
-    }
-    static cudaError_t forward(const XformParams& P, int batch, int nops, cudaStream_t st) {
-        cudaError_t e = prep(fft_forward_kernel<R, S, T>);
-        if (e != cudaSuccess) return e;
-        dim3 grid((unsigned)((P.NN + T - 1) / T), batch, nops);
-        fft_forward_kernel<R, S, T><<<grid, T * S, smem, st>>>(P);
-        return cudaGetLastError();
-    }
-    static cudaError_t inverse(const XformParams& P, int batch, cudaStream_t st) {
-        cudaError_t e = prep(fft_inverse_kernel<R, S, T>);
-        if (e != cudaSuccess) return e;
-        dim3 grid((unsigned)((P.NN + T - 1) / T), batch, 1);
-        fft_inverse_kernel<R, S, T><<<grid, T * S, smem, st>>>(P);
-        return cudaGetLastError();
-    }
-    static cudaError_t retruncate(const XformParams& P, int batch, cudaStream_t st) {
-        cudaError_t e = prep(fft_retruncate_kernel<R, S, T>);
-        if (e != cudaSuccess) return e;
-        dim3 grid((unsigned)((P.NN + T - 1) / T), batch, 1);
-        fft_retruncate_kernel<R, S, T><<<grid, T * S, smem, st>>>(P);
-        return cudaGetLastError();
-    }
-};
-
+// ------------------------------------------------------------------------------------ host side
 enum Which { W_FWD, W_INV, W_RET };
 
-template <int R, int S, int T>
-cudaError_t run_cfg(Which w, const XformParams& P, int batch, int nops, cudaStream_t st) {
-    switch (w) {
-        case W_FWD: return Launcher<R, S, T>::forward(P, batch, nops, st);
-        case W_INV: return Launcher<R, S, T>::inverse(P, batch, st);
-        default: return Launcher<R, S, T>::retruncate(P, batch, st);
+int num_sms() {
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (sms <= 0) sms = 148;
     }
+    return sms;
 }
 
-cudaError_t dispatch(int L, Which w, const XformParams& P, int batch, int nops, cudaStream_t st) {
+template <typename K>
+cudaError_t persistent_grid(K kernel, int threads, int smem, unsigned total_tiles, unsigned* grid) {
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
+    const unsigned cap = (unsigned)(occ * num_sms());
+    *grid = total_tiles < cap ? total_tiles : cap;
+    return cudaSuccess;
+}
+
+template <int R, int T>
+cudaError_t run_small(Which w, XformParams P, int nops, cudaStream_t st) {
+    dim3 grid((unsigned)((P.NN + T - 1) / T), P.batch, nops);
+    switch (w) {
+        case W_FWD: fft_forward_small_kernel<R, T><<<grid, T, 0, st>>>(P); break;
+        case W_INV: fft_inverse_small_kernel<R, T, false><<<grid, T, 0, st>>>(P); break;
+        default: fft_inverse_small_kernel<R, T, true><<<grid, T, 0, st>>>(P); break;
+    }
+    return cudaGetLastError();
+}
+
+template <int R, int S, int T>
+cudaError_t run_tma(Which w, XformParams P, int nops, cudaStream_t st) {
+    using C = Cfg<R, S, T>;
+    P.tiles_x = (unsigned)((P.NN + T - 1) / T);
+    P.total_tiles = P.tiles_x * (unsigned)P.batch * (unsigned)nops;
+    cudaError_t e;
+    unsigned grid = 0;
+    if (w == W_FWD) {
+        // series viewed as doubles: (2 N^2 per order, n orders, batch); box = (2T, L/2, 1)
+        CUtensorMap maps[2];
+        const uint64_t dims[3] = {(uint64_t)(2 * P.NN), (uint64_t)P.n, (uint64_t)P.batch};
+        const uint64_t strides[2] = {(uint64_t)P.NN * 16, (uint64_t)P.n * P.NN * 16};
+        const uint32_t box[3] = {2 * T, (uint32_t)(C::L / 2), 1};
+        for (int z = 0; z < 2; ++z) {
+            const void* src = P.src_series[z] ? P.src_series[z] : P.src_series[0];
+            if ((e = tma_encode_f64(&maps[z], src, 3, dims, strides, box, false)) != cudaSuccess) return e;
+        }
+        auto kern = fft_forward_tma_kernel<R, S, T>;
+        if ((e = persistent_grid(kern, C::THREADS, C::FWD_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
+        kern<<<grid, C::THREADS, C::FWD_SMEM, st>>>(maps[0], maps[1], P);
+    } else {
+        CUtensorMap map;
+        const uint64_t dims[3] = {(uint64_t)(2 * P.NN), (uint64_t)C::L, (uint64_t)P.batch};
+        const uint64_t strides[2] = {(uint64_t)P.NN * 16, (uint64_t)C::L * P.NN * 16};
+        const uint32_t box[3] = {2 * T, (uint32_t)C::L, 1};
+        if ((e = tma_encode_f64(&map, P.src_freq, 3, dims, strides, box, false)) != cudaSuccess) return e;
+        if (w == W_INV) {
+            auto kern = fft_inverse_tma_kernel<R, S, T, false>;
+            if ((e = persistent_grid(kern, C::THREADS, C::INV_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
+            kern<<<grid, C::THREADS, C::INV_SMEM, st>>>(map, P);
+        } else {
+            auto kern = fft_inverse_tma_kernel<R, S, T, true>;
+            if ((e = persistent_grid(kern, C::THREADS, C::INV_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
+            kern<<<grid, C::THREADS, C::INV_SMEM, st>>>(map, P);
+        }
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t dispatch(int L, Which w, const XformParams& P, int nops, cudaStream_t st) {
     switch (L) {
-        case 1: return run_cfg<1, 1, 128>(w, P, batch, nops, st);
-        case 2: return run_cfg<2, 1, 128>(w, P, batch, nops, st);
-        case 4: return run_cfg<4, 1, 128>(w, P, batch, nops, st);
-        case 8: return run_cfg<8, 1, 128>(w, P, batch, nops, st);
-        case 16: return run_cfg<4, 4, 32>(w, P, batch, nops, st);
-        case 32: return run_cfg<8, 4, 32>(w, P, batch, nops, st);
-        case 64: return run_cfg<8, 8, 32>(w, P, batch, nops, st);
-        case 128: return run_cfg<16, 8, 32>(w, P, batch, nops, st);
-        case 256: return run_cfg<16, 16, 16>(w, P, batch, nops, st);
+        case 1: return run_small<1, 128>(w, P, nops, st);
+        case 2: return run_small<2, 128>(w, P, nops, st);
+        case 4: return run_small<4, 128>(w, P, nops, st);
+        case 8: return run_small<8, 128>(w, P, nops, st);
+        case 16: return run_tma<4, 4, 32>(w, P, nops, st);
+        case 32: return run_tma<8, 4, 32>(w, P, nops, st);
+        case 64: return run_tma<8, 8, 16>(w, P, nops, st);
+        case 128: return run_tma<16, 8, 16>(w, P, nops, st);
+        case 256: return run_tma<16, 16, 8>(w, P, nops, st);
         default: return cudaErrorInvalidValue;
     }
 }
 
-XformParams base_params(const FreqLayout& f, const PlanTables& t) {
+XformParams base_params(const FreqLayout& f, const PlanTables& t, int batch) {
     XformParams P{};
     P.NN = f.NN;
-    P.ps = f.ps;
     P.N = f.N;
-    P.ld = f.ld;
     P.n = f.n;
+    P.batch = batch;
     P.tw_fwd = t.tw_fwd;
     P.tw_inv = t.tw_inv;
     P.scale_in = t.scale_in;
@@ -422,34 +612,35 @@ bool fft_length_supported(int L) { return L >= 1 && L <= 256 && (L & (L - 1)) ==
 
 cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int batch, const nspt_c128* src0,
                                double* dst0, const nspt_c128* src1, double* dst1, cudaStream_t st) {
-    XformParams P = base_params(f, t);
+    XformParams P = base_params(f, t, batch);
     P.src_series[0] = reinterpret_cast<const double2*>(src0);
     P.src_series[1] = reinterpret_cast<const double2*>(src1);
-    P.dst_freq[0] = dst0;
-    P.dst_freq[1] = dst1;
+    P.dst_freq[0] = reinterpret_cast<double2*>(dst0);
+    P.dst_freq[1] = reinterpret_cast<double2*>(dst1);
     P.use_scale = (t.scale_in != nullptr) ? 1 : 0;
-    return dispatch(f.L, W_FWD, P, batch, src1 ? 2 : 1, st);
+    return dispatch(f.L, W_FWD, P, src1 ? 2 : 1, st);
 }
 
 cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int batch, const double* src,
                                nspt_c128* dst, cudaStream_t st) {
-    XformParams P = base_params(f, t);
-    P.src_freq = src;
+    XformParams P = base_params(f, t, batch);
+    P.src_freq = reinterpret_cast<const double2*>(src);
     P.dst_series = reinterpret_cast<double2*>(dst);
-    return dispatch(f.L, W_INV, P, batch, 1, st);
+    return dispatch(f.L, W_INV, P, 1, st);
 }
 
 cudaError_t launch_fft_retruncate(const FreqLayout& f, const PlanTables& t, int batch, const double* src,
                                   double* dst, cudaStream_t st) {
-    XformParams P = base_params(f, t);
-    P.src_freq = src;
-    P.dst_freq[0] = dst;
-    return dispatch(f.L, W_RET, P, batch, 1, st);
+    XformParams P = base_params(f, t, batch);
+    P.src_freq = reinterpret_cast<const double2*>(src);
+    P.dst_freq[0] = reinterpret_cast<double2*>(dst);
+    return dispatch(f.L, W_RET, P, 1, st);
 }
 
 cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src, double* dst, cudaStream_t st) {
-    dim3 grid((f.N + 31) / 32, (f.N + 31) / 32, (unsigned)(batch * f.L * 2));
-    freq_dagger_kernel<<<grid, 256, 0, st>>>(src, dst, f.N, f.ld, f.ps, f.L);
+    dim3 grid((f.N + 31) / 32, (f.N + 31) / 32, (unsigned)(batch * f.L));
+    freq_dagger_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst), f.N,
+                                             f.NN, f.L);
     return cudaGetLastError();
 }
 

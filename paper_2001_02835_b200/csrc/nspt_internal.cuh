@@ -9,20 +9,19 @@ namespace nspt {
 
 // ---------------------------------------------------------------------------------------------
 // Frequency-domain workspace layout (internal; eq. 2.7 defines the content).
-// One "spectrum" holds the Fourier coefficients X~(p), p = 0..L-1, of `batch` series as PLANAR
-// real / imaginary planes so that the mode-wise matrix product (eq. 2.8) can feed FP64 tensor
-// cores directly:
-//     plane(b, p, c)[i*ld + j],  c = 0 (real) / 1 (imag),  at double offset ((b*L + p)*2 + c)*ps
-// ld = N rounded up to a multiple of 4 (rows start 32-byte aligned), ps = N*ld rounded up to 16.
+// One "spectrum" holds the Fourier coefficients X~(p), p = 0..L-1, of `batch` series in the same
+// shape as a series, with the mode index in place of the order index:
+//     X~[((b*L + p)*N + i)*N + j]   interleaved complex128, row-major N x N per mode.
+// The transforms write / read 16-byte complex elements with the threads running along (i,j); the
+// mode-wise matrix product loads 128-byte rows of 8 complex through TMA (row pitch N*16 bytes is
+// always a multiple of 16, so no padding is needed for any N).
 // ---------------------------------------------------------------------------------------------
 struct FreqLayout {
     int N;        // matrix dimension
     int n;        // Ntrunc + 1 coefficients
     int L;        // transform length: power of two >= 2*Ntrunc + 1
-    int ld;       // leading dimension of a plane, doubles
-    size_t ps;    // plane stride, doubles
     size_t NN;    // N*N
-    size_t spectrum_doubles(int batch) const { return (size_t)batch * L * 2 * ps; }
+    size_t spectrum_doubles(int batch) const { return (size_t)batch * L * NN * 2; }
 };
 
 inline int transform_length(int Ntrunc) {
@@ -36,8 +35,6 @@ inline FreqLayout make_layout(int N, int Ntrunc) {
     f.N = N;
     f.n = Ntrunc + 1;
     f.L = transform_length(Ntrunc);
-    f.ld = (N + 3) & ~3;
-    f.ps = (((size_t)N * f.ld) + 15) & ~(size_t)15;
     f.NN = (size_t)N * N;
     return f;
 }

@@ -12,32 +12,34 @@
 // (6 N^3 real flops instead of 8 N^3; normwise stable).  The sums Ar+Ai, Br+Bi are formed on the
 // register fragments (2 DADD per 9 DMMA).
 //
-// Tiling.  CTA tile 48 x 48, four consumer warps in 2 x 2, warp tile 24 x 24 = 3 x 3 DMMA blocks and
-// three accumulator sets; one extra producer warp feeds a ring of K-slices of 8 through TMA
-// (cp.async.bulk.tensor, mbarrier complete_tx).  Out-of-range rows / columns / k are zero-filled by
-// TMA, so N need not be a multiple of anything; fully out-of-range 8-row / 8-column blocks of edge
-// tiles are skipped (warp-uniform), and so is the odd half of the last K-slice.
+// Tiling.  CTA tile 48 x 48, four warps in 2 x 2, warp tile 24 x 24 = 3 x 3 DMMA blocks and three
+// accumulator sets (108 registers); 128 threads and 168 registers per thread let three CTAs share an
+// SM (12 warps, 3 per scheduler).  Operands arrive through TMA (cp.async.bulk.tensor, mbarrier
+// complete_tx) in a ring of K-slices of 8; the refill of a slice is issued by the warps in turn, two
+// iterations after the slice was consumed, so nobody waits on it.  Out-of-range rows / columns / k
+// are zero-filled by TMA, so N need not be a multiple of anything; fully out-of-range 8-row /
+// 8-column blocks of edge tiles are skipped (warp-uniform), and so is the odd half of the last slice.
 //
-// Shared-memory layouts are chosen so every fragment load is bank-conflict free:
-//   A slice  [plane][m 0..47][k 0..7]            (64-byte rows, no swizzle).  Lane (g = lane/4, t = lane%4)
-//            reads the pair A[m][2t], A[m][2t+1] with one 16-byte load; the slice is consumed as two
-//            k4 sub-steps whose k-slots are {0,2,4,6} and {1,3,5,7} (any k permutation is legal as long
-//            as A and B agree).
-//   B slice  [chunk 0..2][plane][k 0..7][n 0..15] (128-byte rows, TMA SWIZZLE_128B).  Lane (g, t) reads
-//            B[2t+s][n] with 8-byte loads; rows {0,2,4,6} (or {1,3,5,7}) XOR-swizzle onto disjoint banks.
+// Shared-memory layout: every operand row is 8 complex128 = 128 bytes, written by TMA with
+// SWIZZLE_128B (16-byte chunk index XOR row index mod 8).  A slice: [m 0..47][k 0..7]; B slice: six
+// boxes [k 0..7][n 0..7].  Lane (g = lane/4, t = lane%4) loads one complex element (re, im) per
+// fragment with a 16-byte ld.shared; a slice is consumed as two k4 sub-steps whose k-slots are
+// {0,2,4,6} and {1,3,5,7} (any k permutation is legal as long as A and B agree), which makes the
+// eight lanes of every quarter-warp hit eight different 16-byte chunks: no bank conflicts.
 #include <cuda.h>
 #include "nspt_internal.cuh"
+#include "nspt_tma.cuh"
 
 namespace nspt {
 namespace {
 
 constexpr int BM = 48, BN = 48, BK = 8;
-constexpr int STAGES = 6;
-constexpr int A_STAGE_BYTES = 2 * BM * BK * 8;                 // 6144
-constexpr int B_CHUNK_BYTES = 2 * BK * 16 * 8;                 // 2048: [plane][k][16]
-constexpr int B_STAGE_BYTES = (BN / 16) * B_CHUNK_BYTES;       // 6144
+constexpr int STAGES = 5;
+constexpr int A_STAGE_BYTES = BM * BK * 16;                    // 6144: [m][8 complex]
+constexpr int B_BOX_BYTES = BK * 8 * 16;                       // 1024: [k][8 complex]
+constexpr int B_STAGE_BYTES = (BN / 8) * B_BOX_BYTES;          // 6144
 constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;     // 12288
-constexpr int GEMM_THREADS = 160;                              // 4 consumer warps + 1 producer warp
+constexpr int GEMM_THREADS = 128;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8 + 1024;  // + barriers + alignment slack
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -45,37 +47,6 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn g_encode = nullptr;
 
-// ---------------------------------------------------------------- PTX wrappers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(dst),
-        "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
-        : "memory");
-}
 __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};"
         : "+d"(c0), "+d"(c1)
@@ -83,15 +54,24 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 }
 
 struct GemmParams {
-    double* C;
-    size_t ps;
-    int N, ld;
+    double2* C;
+    size_t NN;
+    int N;
     int tiles_m, tiles_n;
     double alpha_re, alpha_im;
     int accumulate;
 };
 
-__global__ void __launch_bounds__(GEMM_THREADS, 2)
+__device__ __forceinline__ void issue_slice(const CUtensorMap* mapA, const CUtensorMap* mapB, uint32_t stage_addr,
+                                            uint32_t full_bar, int k0, int m0, int n0, int mode) {
+    mbar_expect_tx(full_bar, STAGE_BYTES);
+    tma_load_3d(stage_addr, mapA, full_bar, 2 * k0, m0, mode);
+#pragma unroll
+    for (int c = 0; c < BN / 8; ++c)
+        tma_load_3d(stage_addr + A_STAGE_BYTES + c * B_BOX_BYTES, mapB, full_bar, 2 * (n0 + 8 * c), k0, mode);
+}
+
+__global__ void __launch_bounds__(GEMM_THREADS, 3)
 zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
                         const GemmParams P) {
     extern __shared__ uint8_t smem_raw[];
@@ -114,31 +94,13 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
             mbar_init(bar_full + 8 * s, 1);
             mbar_init(bar_empty + 8 * s, 4);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
+        const int pre = nk < STAGES ? nk : STAGES;
+        for (int it = 0; it < pre; ++it)
+            issue_slice(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, it * BK, m0, n0, mode);
     }
     __syncthreads();
 
-    if (warp == 4) {
-        // ------------------------------------------------------------ producer
-        if (lane == 0) {
-            for (int it = 0; it < nk; ++it) {
-                const int slot = it % STAGES;
-                if (it >= STAGES) mbar_wait(bar_empty + 8 * slot, ((it / STAGES) - 1) & 1);
-                const uint32_t full = bar_full + 8 * slot;
-                mbar_expect_tx(full, STAGE_BYTES);
-                const uint32_t sa = base + slot * STAGE_BYTES;
-                const uint32_t sb = sa + A_STAGE_BYTES;
-                const int k0 = it * BK;
-                tma_load_3d(sa, &mapA, full, k0, m0, 2 * mode);
-#pragma unroll
-                for (int c = 0; c < BN / 16; ++c)
-                    tma_load_3d(sb + c * B_CHUNK_BYTES, &mapB, full, n0 + 16 * c, k0, 2 * mode);
-            }
-        }
-        return;
-    }
-
-    // ---------------------------------------------------------------- consumers
     const int g = lane >> 2, t = lane & 3;
     const int wm = warp >> 1, wn = warp & 1;
     const int mw = 24 * wm, nw = 24 * wn;  // warp offsets inside the CTA tile
@@ -159,56 +121,52 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
             p3[i][j][0] = p3[i][j][1] = 0.0;
         }
 
-    // per-lane constant byte offsets of the fragment loads inside a stage
-    uint32_t offA[3];
-#pragma unroll
-    for (int bm = 0; bm < 3; ++bm) offA[bm] = (uint32_t)(((mw + 8 * bm + g) * BK + 2 * t) * 8);
-    uint32_t offB[2][3];
-#pragma unroll
-    for (int s = 0; s < 2; ++s)
-#pragma unroll
-        for (int bn = 0; bn < 3; ++bn) {
-            const int k = 2 * t + s;
-            const int n = nw + 8 * bn + g;
-            const int chunk = n >> 4, n16 = n & 15;
-            offB[s][bn] = (uint32_t)(A_STAGE_BYTES + chunk * B_CHUNK_BYTES + k * 128 + ((((n16 >> 1) ^ k) & 7) << 4) +
-                                     (n16 & 1) * 8);
-        }
+    // per-lane byte offsets of the fragment loads inside a stage (sub-step 0; sub-step 1 is derived)
+    const uint32_t offA0 = (uint32_t)((mw + g) * 128 + (((2 * t) ^ g) << 4));           // + bm*1024
+    const uint32_t offA1 = offA0 ^ 16u;                                                   // k-slot 2t+1
+    const uint32_t offB0 = (uint32_t)(A_STAGE_BYTES + (3 * wn) * B_BOX_BYTES + (2 * t) * 128 + ((g ^ (2 * t)) << 4));
+    const uint32_t offB1 = (offB0 + 128u) ^ 16u;                                          // row 2t+1
 
     for (int it = 0; it < nk; ++it) {
+        // refill, two iterations late, by the warps in turn
+        if (it >= 2 && warp == (it & 3)) {
+            const int j = it - 2;
+            if (j + STAGES < nk && lane == 0) {
+                const int slot = j % STAGES;
+                mbar_wait(bar_empty + 8 * slot, (j / STAGES) & 1);
+                issue_slice(&mapA, &mapB, base + slot * STAGE_BYTES, bar_full + 8 * slot, (j + STAGES) * BK, m0, n0, mode);
+            }
+            __syncwarp();
+        }
         const int slot = it % STAGES;
         mbar_wait(bar_full + 8 * slot, (it / STAGES) & 1);
         if (active) {
             const uint8_t* st = sgen + slot * STAGE_BYTES;
-            double2 ar[3], ai[3];
-#pragma unroll
-            for (int bm = 0; bm < 3; ++bm) {
-                ar[bm] = *reinterpret_cast<const double2*>(st + offA[bm]);
-                ai[bm] = *reinterpret_cast<const double2*>(st + offA[bm] + BM * BK * 8);
-            }
             const int nsub = (it * BK + 1 < N) ? 2 : 1;  // odd k-slots of the last slice may all be padding
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
                 if (s < nsub) {
-                    double br[3], bi[3], bs[3];
+                    double2 a[3], b[3];
+                    double as[3], bs[3];
+#pragma unroll
+                    for (int bm = 0; bm < 3; ++bm) {
+                        a[bm] = *reinterpret_cast<const double2*>(st + (s ? offA1 : offA0) + bm * 1024);
+                        as[bm] = a[bm].x + a[bm].y;
+                    }
 #pragma unroll
                     for (int bn = 0; bn < 3; ++bn) {
-                        br[bn] = *reinterpret_cast<const double*>(st + offB[s][bn]);
-                        bi[bn] = *reinterpret_cast<const double*>(st + offB[s][bn] + BK * 16 * 8);
-                        bs[bn] = br[bn] + bi[bn];
+                        b[bn] = *reinterpret_cast<const double2*>(st + (s ? offB1 : offB0) + bn * B_BOX_BYTES);
+                        bs[bn] = b[bn].x + b[bn].y;
                     }
 #pragma unroll
                     for (int bm = 0; bm < 3; ++bm) {
                         if (bm < nbm) {
-                            const double a_r = s ? ar[bm].y : ar[bm].x;
-                            const double a_i = s ? ai[bm].y : ai[bm].x;
-                            const double a_s = a_r + a_i;
 #pragma unroll
                             for (int bn = 0; bn < 3; ++bn) {
                                 if (bn < nbn) {
-                                    dmma(p1[bm][bn][0], p1[bm][bn][1], a_r, br[bn]);
-                                    dmma(p2[bm][bn][0], p2[bm][bn][1], a_i, bi[bn]);
-                                    dmma(p3[bm][bn][0], p3[bm][bn][1], a_s, bs[bn]);
+                                    dmma(p1[bm][bn][0], p1[bm][bn][1], a[bm].x, b[bn].x);
+                                    dmma(p2[bm][bn][0], p2[bm][bn][1], a[bm].y, b[bn].y);
+                                    dmma(p3[bm][bn][0], p3[bm][bn][1], as[bm], bs[bn]);
                                 }
                             }
                         }
@@ -222,8 +180,7 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
 
     if (!active) return;
     // ---------------------------------------------------------------- epilogue
-    double* Cr = P.C + (size_t)(2 * mode) * P.ps;
-    double* Ci = Cr + P.ps;
+    double2* Cm = P.C + (size_t)mode * P.NN;
 #pragma unroll
     for (int bm = 0; bm < 3; ++bm) {
         const int m = m0 + mw + 8 * bm + g;
@@ -232,25 +189,26 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
             for (int bn = 0; bn < 3; ++bn) {
                 const int n = n0 + nw + 8 * bn + 2 * t;
                 if (bn < nbn && n < N) {
-                    double cr0 = p1[bm][bn][0] - p2[bm][bn][0];
-                    double cr1 = p1[bm][bn][1] - p2[bm][bn][1];
-                    double ci0 = p3[bm][bn][0] - p1[bm][bn][0] - p2[bm][bn][0];
-                    double ci1 = p3[bm][bn][1] - p1[bm][bn][1] - p2[bm][bn][1];
-                    double or0 = P.alpha_re * cr0 - P.alpha_im * ci0;
-                    double oi0 = P.alpha_re * ci0 + P.alpha_im * cr0;
-                    double or1 = P.alpha_re * cr1 - P.alpha_im * ci1;
-                    double oi1 = P.alpha_re * ci1 + P.alpha_im * cr1;
-                    double2* dr = reinterpret_cast<double2*>(Cr + (size_t)m * P.ld + n);
-                    double2* di = reinterpret_cast<double2*>(Ci + (size_t)m * P.ld + n);
+                    const double cr0 = p1[bm][bn][0] - p2[bm][bn][0];
+                    const double cr1 = p1[bm][bn][1] - p2[bm][bn][1];
+                    const double ci0 = p3[bm][bn][0] - p1[bm][bn][0] - p2[bm][bn][0];
+                    const double ci1 = p3[bm][bn][1] - p1[bm][bn][1] - p2[bm][bn][1];
+                    double2 o0 = make_double2(P.alpha_re * cr0 - P.alpha_im * ci0, P.alpha_re * ci0 + P.alpha_im * cr0);
+                    double2 o1 = make_double2(P.alpha_re * cr1 - P.alpha_im * ci1, P.alpha_re * ci1 + P.alpha_im * cr1);
+                    double2* d = Cm + (size_t)m * N + n;
+                    const bool second = (n + 1 < N);
                     if (P.accumulate) {
-                        const double2 oldr = *dr, oldi = *di;
-                        or0 += oldr.x;
-                        or1 += oldr.y;
-                        oi0 += oldi.x;
-                        oi1 += oldi.y;
+                        const double2 old0 = d[0];
+                        o0.x += old0.x;
+                        o0.y += old0.y;
+                        if (second) {
+                            const double2 old1 = d[1];
+                            o1.x += old1.x;
+                            o1.y += old1.y;
+                        }
                     }
-                    *dr = make_double2(or0, or1);  // n+1 may be the first padding column (n+1 < ld): harmless
-                    *di = make_double2(oi0, oi1);
+                    d[0] = o0;
+                    if (second) d[1] = o1;
                 }
             }
         }
@@ -260,57 +218,70 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
 // Reference kernel (variant 0): one thread per output element, conventional 4-multiplication
 // complex product with plain FMAs.  For debugging the tensor-core kernel; never the default.
 __global__ void __launch_bounds__(256)
-zgemm_modes_ref_kernel(const double* __restrict__ A, const double* __restrict__ B, double* __restrict__ C, int N, int ld,
-                       size_t ps, double alpha_re, double alpha_im, int accumulate) {
+zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict__ B, double2* __restrict__ C, int N,
+                       size_t NN, double alpha_re, double alpha_im, int accumulate) {
     const int mode = blockIdx.z;
     const int j = blockIdx.x * 16 + (threadIdx.x & 15);
     const int i = blockIdx.y * 16 + (threadIdx.x >> 4);
     if (i >= N || j >= N) return;
-    const double* Ar = A + (size_t)(2 * mode) * ps;
-    const double* Ai = Ar + ps;
-    const double* Br = B + (size_t)(2 * mode) * ps;
-    const double* Bi = Br + ps;
+    const double2* Am = A + (size_t)mode * NN;
+    const double2* Bm = B + (size_t)mode * NN;
     double cr = 0.0, ci = 0.0;
     for (int k = 0; k < N; ++k) {
-        const double ar = Ar[(size_t)i * ld + k], ai = Ai[(size_t)i * ld + k];
-        const double br = Br[(size_t)k * ld + j], bi = Bi[(size_t)k * ld + j];
-        cr += ar * br - ai * bi;
-        ci += ar * bi + ai * br;
+        const double2 a = Am[(size_t)i * N + k];
+        const double2 b = Bm[(size_t)k * N + j];
+        cr += a.x * b.x - a.y * b.y;
+        ci += a.x * b.y + a.y * b.x;
     }
-    double outr = alpha_re * cr - alpha_im * ci;
-    double outi = alpha_re * ci + alpha_im * cr;
-    double* Cr = C + (size_t)(2 * mode) * ps;
-    double* Ci = Cr + ps;
+    double2 out = make_double2(alpha_re * cr - alpha_im * ci, alpha_re * ci + alpha_im * cr);
+    double2* c = C + (size_t)mode * NN + (size_t)i * N + j;
     if (accumulate) {
-        outr += Cr[(size_t)i * ld + j];
-        outi += Ci[(size_t)i * ld + j];
+        out.x += c->x;
+        out.y += c->y;
     }
-    Cr[(size_t)i * ld + j] = outr;
-    Ci[(size_t)i * ld + j] = outi;
+    *c = out;
 }
 
-CUresult encode_3d(CUtensorMap* map, const double* basep, const FreqLayout& f, int planes, int box0, int box1,
-                   CUtensorMapSwizzle swz) {
-    cuuint64_t dims[3] = {(cuuint64_t)f.N, (cuuint64_t)f.N, (cuuint64_t)planes};
-    cuuint64_t strides[2] = {(cuuint64_t)f.ld * 8, (cuuint64_t)f.ps * 8};
-    cuuint32_t box[3] = {(cuuint32_t)box0, (cuuint32_t)box1, 2};
-    cuuint32_t estr[3] = {1, 1, 1};
-    return g_encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(basep), dims, strides, box, estr,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+// 3-D view of a spectrum as doubles: (2N doubles per row, N rows, modes); boxes are 16 doubles wide
+// (8 complex = 128 bytes, the swizzle span).
+cudaError_t encode_operand(CUtensorMap* map, const double* basep, const FreqLayout& f, int modes, int box_rows) {
+    const uint64_t dims[3] = {(uint64_t)(2 * f.N), (uint64_t)f.N, (uint64_t)modes};
+    const uint64_t strides[2] = {(uint64_t)f.N * 16, (uint64_t)f.NN * 16};
+    const uint32_t box[3] = {16, (uint32_t)box_rows, 1};
+    return tma_encode_f64(map, basep, 3, dims, strides, box, true);
 }
 
 }  // namespace
 
+cudaError_t tma_encode_f64(CUtensorMap* map, const void* base, int rank, const uint64_t* dims,
+                           const uint64_t* strides_bytes, const uint32_t* box, bool swizzle128) {
+    if (!g_encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess) return e;
+        if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+        g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+    }
+    cuuint64_t d[3] = {1, 1, 1}, st[2] = {16, 16};
+    cuuint32_t bx[3] = {1, 1, 1}, es[3] = {1, 1, 1};
+    for (int i = 0; i < rank; ++i) {
+        d[i] = dims[i];
+        bx[i] = box[i];
+    }
+    for (int i = 0; i + 1 < rank; ++i) st[i] = strides_bytes[i];
+    const CUresult r = g_encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, const_cast<void*>(base), d, st, bx, es,
+                                CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 cudaError_t zgemm_init() {
-    if (g_encode) return cudaSuccess;
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
-    if (e != cudaSuccess) return e;
-    if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
-    g_encode = reinterpret_cast<EncodeTiledFn>(fn);
-    e = cudaFuncSetAttribute(zgemm_modes_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    static bool done = false;
+    if (done) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(zgemm_modes_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e == cudaSuccess) done = true;
     return e;
 }
 
@@ -319,19 +290,20 @@ cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, 
     const int modes = batch * f.L;
     if (variant == 0) {
         dim3 grid((f.N + 15) / 16, (f.N + 15) / 16, modes);
-        zgemm_modes_ref_kernel<<<grid, 256, 0, st>>>(A, B, C, f.N, f.ld, f.ps, alpha.re, alpha.im, accumulate ? 1 : 0);
+        zgemm_modes_ref_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(A), reinterpret_cast<const double2*>(B),
+                                                     reinterpret_cast<double2*>(C), f.N, f.NN, alpha.re, alpha.im,
+                                                     accumulate ? 1 : 0);
         return cudaGetLastError();
     }
     cudaError_t e = zgemm_init();
     if (e != cudaSuccess) return e;
     CUtensorMap mapA, mapB;
-    if (encode_3d(&mapA, A, f, 2 * modes, BK, BM, CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS) return cudaErrorInvalidValue;
-    if (encode_3d(&mapB, B, f, 2 * modes, 16, BK, CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    if ((e = encode_operand(&mapA, A, f, modes, BM)) != cudaSuccess) return e;
+    if ((e = encode_operand(&mapB, B, f, modes, BK)) != cudaSuccess) return e;
     GemmParams P;
-    P.C = C;
-    P.ps = f.ps;
+    P.C = reinterpret_cast<double2*>(C);
+    P.NN = f.NN;
     P.N = f.N;
-    P.ld = f.ld;
     P.tiles_m = (f.N + BM - 1) / BM;
     P.tiles_n = (f.N + BN - 1) / BN;
     P.alpha_re = alpha.re;
