@@ -96,6 +96,22 @@ def aggregate_throughput(units_this_rank: float, ms_this_rank: float, world: int
     return units / (ms * 1e-3), ms
 
 
+def read_traffic(workload: str, kernel: str):
+    """DRAM bytes per launch of a kernel from the committed ncu summary table (profiles/traffic.csv:
+    dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture), or None."""
+    tfile = ROOT / "profiles" / "traffic.csv"
+    if not tfile.exists():
+        return None
+    try:
+        for line in tfile.read_text().splitlines()[1:]:
+            cols = line.split(",")
+            if len(cols) >= 3 and cols[0] == workload and cols[1] == kernel:
+                return float(cols[2])
+    except Exception:
+        return None
+    return None
+
+
 # ------------------------------------------------------------------------------------ clocks
 
 class ClockSampler:
@@ -327,13 +343,7 @@ def run_cuda(args):
         gemm = stage_ms.get("zgemm_modes")
         flops_per_launch = 8.0 * N ** 3 * L * batch
         achieved = flops_per_launch / (gemm["ms_per_launch"] * 1e-3) * 1e-12 if gemm else None
-        traffic = None
-        tfile = ROOT / "profiles" / "traffic.json"
-        if tfile.exists():
-            try:
-                traffic = json.loads(tfile.read_text()).get(args.workload, {}).get("zgemm_modes_dram_bytes_per_launch")
-            except Exception:
-                traffic = None
+        traffic = read_traffic(args.workload, "zgemm_modes")
         peaks = {}
         pfile = ROOT / "MEASURED_PEAKS.json"
         if pfile.exists():

@@ -46,9 +46,8 @@ def test_argument_validation_without_a_gpu(lib):
     lib.nspt_workspace_bytes.argtypes = [ctypes.c_int] * 4 + [ctypes.POINTER(ctypes.c_size_t)]
     out = ctypes.c_size_t(0)
     assert lib.nspt_workspace_bytes(225, 63, 1, 0, ctypes.byref(out)) == 0
-    # three spectra of L=128 modes x 2 planes x 225 rows x ld=228 doubles (rounded up)
-    per_plane = (225 * 228 + 15) // 16 * 16
-    assert out.value >= 3 * 128 * 2 * per_plane * 8
+    # three spectra of L=128 modes x 225 x 225 interleaved complex128
+    assert out.value >= 3 * 128 * 225 * 225 * 16
     assert lib.nspt_workspace_bytes(225, 31, 1, 1, ctypes.byref(out)) == 0 and out.value > 0
     assert lib.nspt_workspace_bytes(0, 3, 1, 0, ctypes.byref(out)) == -1
     assert lib.nspt_workspace_bytes(4, 128, 1, 0, ctypes.byref(out)) == -1
