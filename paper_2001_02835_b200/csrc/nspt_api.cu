@@ -137,7 +137,7 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 size_t spectrum_bytes(const FreqLayout& f, int batch) { return align_up(f.spectrum_doubles(batch) * 8, 1024); }
 
 size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
-    if (op == NSPT_OP_STAPLE) return 11 * spectrum_bytes(f, 1);
+    if (op == NSPT_OP_STAPLE) return 15 * spectrum_bytes(f, 1);
     return 3 * spectrum_bytes(f, batch);
 }
 
@@ -254,11 +254,16 @@ int k_dagger(const FreqLayout& f, int batch, const double* src, double* dst) {
     NSPT_CUDA(launch_freq_dagger(f, batch, src, dst, g.stream));
     return tm.end();
 }
-int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, double* C, Cplx alpha, bool acc) {
+int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_GEMM));
-    NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, C, alpha, acc, g.gemm_variant, g.stream));
+    NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, out, g.gemm_variant, g.stream));
     return tm.end();
+}
+int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, double* C) {
+    GemmOut out;
+    out.C = C;
+    return k_gemm(f, batch, A, B, out);
 }
 
 // ---- the products --------------------------------------------------------------------------
@@ -279,7 +284,7 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
     // Steps 1-2 (eqs. 2.6-2.7): zero-padded forward transforms of A and B, one launch
     NSPT_TRY(k_forward(f, t, batch, A, At, B, Bt));
     // Step 3 (eq. 2.8): mode-wise matrix products
-    NSPT_TRY(k_gemm(f, batch, At, Bt, Ct, Cplx{1.0, 0.0}, false));
+    NSPT_TRY(k_gemm(f, batch, At, Bt, Ct));
     // Steps 4-5 (eq. 2.9): inverse transform, 1/L, truncation
     NSPT_TRY(k_inverse(f, t, batch, Ct, C));
     return NSPT_OK;
@@ -299,34 +304,64 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     NSPT_TRY(get_workspace(ws_bytes_for(f, 1, NSPT_OP_STAPLE), &ws));
     const size_t sb = spectrum_bytes(f, 1);
     auto spec = [&](int i) { return reinterpret_cast<double*>(ws + (size_t)i * sb); };
-    double* Ut[4] = {spec(0), spec(1), spec(2), spec(3)};   // U~_mu
-    double* Ud[4] = {spec(4), spec(5), spec(6), spec(7)};   // spectrum of U_mu^+
-    double* W = spec(8);                                    // first-level product, re-truncated in place
-    double* X = spec(9);                                    // accumulated bracket of eq. 2.3
-    double* St = spec(10);                                  // U_mu * X
-    // all four links are transformed before any output is written (S may alias U)
+    double* Ut[4] = {spec(0), spec(1), spec(2), spec(3)};      // U~_mu
+    double* Ud[4] = {spec(4), spec(5), spec(6), spec(7)};      // spectrum of U_mu^+
+    double* St[4] = {spec(8), spec(9), spec(10), spec(11)};    // S~_mu, accumulated in frequency space
+    double* W = spec(12);                                      // U_mu * U_nu^+
+    double* Y = spec(13);                                      // U_mu^+ * U_nu
+    double* T = spec(14);                                      // U_nu * W
+    // Eq. 2.3 with U_mu distributed over the sum (the truncated series form a ring, so this is exact):
+    //     S_mu = sum_{nu != mu} ( z_{mu nu} P_{mu nu} - z_{mu nu}^* R_{mu nu} ),
+    //     P_{mu nu} = U_mu U_nu U_mu^+ U_nu^+,     R_{mu nu} = U_mu U_nu^+ U_mu^+ U_nu       (all products are *).
+    // For each unordered pair mu < nu, with W = U_mu U_nu^+ and Y = U_mu^+ U_nu:
+    //     R_{mu nu} = W Y,   R_{nu mu} = (Y W)^+,   P_{nu mu} = (U_nu W) U_mu^+,   P_{mu nu} = P_{nu mu}^+ .
+    // Six mode-wise products per pair, 36 in all (the literal form needs 52).  The daggers of PRODUCTS are
+    // taken by the GEMM epilogue (conjugate-transposed accumulate into the mirrored mode), the sums over
+    // nu are accumulated in frequency space, and each S_mu is inverse-transformed once.
+    // All four links are transformed before any output is written (S may alias U).
     NSPT_TRY(k_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1]));
     NSPT_TRY(k_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3]));
     for (int mu = 0; mu < 4; ++mu) NSPT_TRY(k_dagger(f, 1, Ut[mu], Ud[mu]));
+    bool touched[4] = {false, false, false, false};
     for (int mu = 0; mu < 4; ++mu) {
-        bool first = true;
-        for (int nu = 0; nu < 4; ++nu) {
-            if (nu == mu) continue;
+        for (int nu = mu + 1; nu < 4; ++nu) {
             const Cplx zmn{z[4 * mu + nu].re, z[4 * mu + nu].im};
-            // + z_{mu nu} (U_nu * U_mu^+) * U_nu^+
-            NSPT_TRY(k_gemm(f, 1, Ut[nu], Ud[mu], W, Cplx{1.0, 0.0}, false));
+            const Cplx znm{z[4 * nu + mu].re, z[4 * nu + mu].im};
+            NSPT_TRY(k_gemm(f, 1, Ut[mu], Ud[nu], W));
             NSPT_TRY(k_retrunc(f, t, 1, W, W));
-            NSPT_TRY(k_gemm(f, 1, W, Ud[nu], X, zmn, !first));
-            first = false;
-            // - z_{mu nu}^* (U_nu^+ * U_mu^+) * U_nu
-            NSPT_TRY(k_gemm(f, 1, Ud[nu], Ud[mu], W, Cplx{1.0, 0.0}, false));
-            NSPT_TRY(k_retrunc(f, t, 1, W, W));
-            NSPT_TRY(k_gemm(f, 1, W, Ut[nu], X, Cplx{-zmn.re, zmn.im}, true));
+            NSPT_TRY(k_gemm(f, 1, Ud[mu], Ut[nu], Y));
+            NSPT_TRY(k_retrunc(f, t, 1, Y, Y));
+            {   // S_mu -= z_{mu nu}^* R_{mu nu},  R_{mu nu} = W Y
+                GemmOut o;
+                o.C = St[mu];
+                o.alpha = Cplx{-zmn.re, zmn.im};
+                o.accumulate = touched[mu];
+                NSPT_TRY(k_gemm(f, 1, W, Y, o));
+                touched[mu] = true;
+            }
+            {   // S_nu -= z_{nu mu}^* R_{nu mu},  R_{nu mu} = (Y W)^+
+                GemmOut o;
+                o.D = St[nu];
+                o.beta = Cplx{-znm.re, znm.im};
+                o.accumulate_d = touched[nu];
+                NSPT_TRY(k_gemm(f, 1, Y, W, o));
+                touched[nu] = true;
+            }
+            NSPT_TRY(k_gemm(f, 1, Ut[nu], W, T));
+            NSPT_TRY(k_retrunc(f, t, 1, T, T));
+            {   // S_nu += z_{nu mu} P_{nu mu},  S_mu += z_{mu nu} P_{nu mu}^+,  P_{nu mu} = T U_mu^+
+                GemmOut o;
+                o.C = St[nu];
+                o.alpha = znm;
+                o.accumulate = true;
+                o.D = St[mu];
+                o.beta = zmn;
+                o.accumulate_d = true;
+                NSPT_TRY(k_gemm(f, 1, T, Ud[mu], o));
+            }
         }
-        NSPT_TRY(k_retrunc(f, t, 1, X, X));
-        NSPT_TRY(k_gemm(f, 1, Ut[mu], X, St, Cplx{1.0, 0.0}, false));
-        NSPT_TRY(k_inverse(f, t, 1, St, S[mu]));
     }
+    for (int mu = 0; mu < 4; ++mu) NSPT_TRY(k_inverse(f, t, 1, St[mu], S[mu]));
     return NSPT_OK;
 }
 

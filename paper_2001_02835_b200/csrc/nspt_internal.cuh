@@ -70,10 +70,20 @@ cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src
 bool fft_length_supported(int L);
 
 // ---- mode-wise matrix product (nspt_zgemm.cu) -----------------------------------------------
-// C~(p) = alpha * A~(p) B~(p) [+ C~(p) if accumulate], for all batch*L modes.
+// For all batch*L modes p, with M(p) = A~(p) B~(p):
+//     C(p)             (+)= alpha * M(p)        if C is not null  (accumulate selects +=)
+//     D((L-p) mod L)   (+)= beta  * M(p)^H      if D is not null  (accumulate_d selects +=)
+// The second form adds the spectrum of the DAGGERED product series, FFT[X^+](p') = (X~((L-p') mod L))^H.
+struct GemmOut {
+    double* C = nullptr;
+    Cplx alpha{1.0, 0.0};
+    bool accumulate = false;
+    double* D = nullptr;
+    Cplx beta{1.0, 0.0};
+    bool accumulate_d = false;
+};
 cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B,
-                               double* C, Cplx alpha, bool accumulate, int variant,
-                               cudaStream_t st);
+                               const GemmOut& out, int variant, cudaStream_t st);
 cudaError_t zgemm_init();   // resolves the driver entry point for tensor maps
 
 }  // namespace nspt

@@ -54,12 +54,14 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 }
 
 struct GemmParams {
-    double2* C;
+    double2* C;   // direct target:   C(p)            (+)= alpha * A(p) B(p)          (may be null)
+    double2* D;   // daggered target: D((L-p) mod L)  (+)= beta * (A(p) B(p))^H       (may be null)
     size_t NN;
-    int N;
+    int N, L;
     int tiles_m, tiles_n;
     double alpha_re, alpha_im;
-    int accumulate;
+    double beta_re, beta_im;
+    int accumulate, accumulate_d;
 };
 
 __device__ __forceinline__ void issue_slice(const CUtensorMap* mapA, const CUtensorMap* mapB, uint32_t stage_addr,
@@ -180,7 +182,10 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
 
     if (!active) return;
     // ---------------------------------------------------------------- epilogue
-    double2* Cm = P.C + (size_t)mode * P.NN;
+    double2* Cm = P.C ? P.C + (size_t)mode * P.NN : nullptr;
+    // spectrum of the daggered series: FFT[X^+](p') = (X~(p))^H with p' = (L - p) mod L, same batch element
+    const int pm = mode % P.L;
+    double2* Dm = P.D ? P.D + (size_t)(mode - pm + ((P.L - pm) % P.L)) * P.NN : nullptr;
 #pragma unroll
     for (int bm = 0; bm < 3; ++bm) {
         const int m = m0 + mw + 8 * bm + g;
@@ -193,22 +198,43 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
                     const double cr1 = p1[bm][bn][1] - p2[bm][bn][1];
                     const double ci0 = p3[bm][bn][0] - p1[bm][bn][0] - p2[bm][bn][0];
                     const double ci1 = p3[bm][bn][1] - p1[bm][bn][1] - p2[bm][bn][1];
-                    double2 o0 = make_double2(P.alpha_re * cr0 - P.alpha_im * ci0, P.alpha_re * ci0 + P.alpha_im * cr0);
-                    double2 o1 = make_double2(P.alpha_re * cr1 - P.alpha_im * ci1, P.alpha_re * ci1 + P.alpha_im * cr1);
-                    double2* d = Cm + (size_t)m * N + n;
                     const bool second = (n + 1 < N);
-                    if (P.accumulate) {
-                        const double2 old0 = d[0];
-                        o0.x += old0.x;
-                        o0.y += old0.y;
-                        if (second) {
-                            const double2 old1 = d[1];
-                            o1.x += old1.x;
-                            o1.y += old1.y;
+                    if (Cm) {
+                        double2 o0 = make_double2(P.alpha_re * cr0 - P.alpha_im * ci0, P.alpha_re * ci0 + P.alpha_im * cr0);
+                        double2 o1 = make_double2(P.alpha_re * cr1 - P.alpha_im * ci1, P.alpha_re * ci1 + P.alpha_im * cr1);
+                        double2* d = Cm + (size_t)m * N + n;
+                        if (P.accumulate) {
+                            const double2 old0 = d[0];
+                            o0.x += old0.x;
+                            o0.y += old0.y;
+                            if (second) {
+                                const double2 old1 = d[1];
+                                o1.x += old1.x;
+                                o1.y += old1.y;
+                            }
                         }
+                        d[0] = o0;
+                        if (second) d[1] = o1;
                     }
-                    d[0] = o0;
-                    if (second) d[1] = o1;
+                    if (Dm) {
+                        // beta * conj(c): the eight lanes g = 0..7 of a quarter-warp write 128 contiguous bytes
+                        double2 o0 = make_double2(P.beta_re * cr0 + P.beta_im * ci0, P.beta_im * cr0 - P.beta_re * ci0);
+                        double2 o1 = make_double2(P.beta_re * cr1 + P.beta_im * ci1, P.beta_im * cr1 - P.beta_re * ci1);
+                        double2* d0 = Dm + (size_t)n * N + m;
+                        double2* d1 = d0 + N;
+                        if (P.accumulate_d) {
+                            const double2 old0 = *d0;
+                            o0.x += old0.x;
+                            o0.y += old0.y;
+                            if (second) {
+                                const double2 old1 = *d1;
+                                o1.x += old1.x;
+                                o1.y += old1.y;
+                            }
+                        }
+                        *d0 = o0;
+                        if (second) *d1 = o1;
+                    }
                 }
             }
         }
@@ -218,14 +244,14 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
 // Reference kernel (variant 0): one thread per output element, conventional 4-multiplication
 // complex product with plain FMAs.  For debugging the tensor-core kernel; never the default.
 __global__ void __launch_bounds__(256)
-zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict__ B, double2* __restrict__ C, int N,
-                       size_t NN, double alpha_re, double alpha_im, int accumulate) {
+zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict__ B, const GemmParams P) {
     const int mode = blockIdx.z;
     const int j = blockIdx.x * 16 + (threadIdx.x & 15);
     const int i = blockIdx.y * 16 + (threadIdx.x >> 4);
+    const int N = P.N;
     if (i >= N || j >= N) return;
-    const double2* Am = A + (size_t)mode * NN;
-    const double2* Bm = B + (size_t)mode * NN;
+    const double2* Am = A + (size_t)mode * P.NN;
+    const double2* Bm = B + (size_t)mode * P.NN;
     double cr = 0.0, ci = 0.0;
     for (int k = 0; k < N; ++k) {
         const double2 a = Am[(size_t)i * N + k];
@@ -233,13 +259,25 @@ zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict_
         cr += a.x * b.x - a.y * b.y;
         ci += a.x * b.y + a.y * b.x;
     }
-    double2 out = make_double2(alpha_re * cr - alpha_im * ci, alpha_re * ci + alpha_im * cr);
-    double2* c = C + (size_t)mode * NN + (size_t)i * N + j;
-    if (accumulate) {
-        out.x += c->x;
-        out.y += c->y;
+    if (P.C) {
+        double2 out = make_double2(P.alpha_re * cr - P.alpha_im * ci, P.alpha_re * ci + P.alpha_im * cr);
+        double2* c = P.C + (size_t)mode * P.NN + (size_t)i * N + j;
+        if (P.accumulate) {
+            out.x += c->x;
+            out.y += c->y;
+        }
+        *c = out;
     }
-    *c = out;
+    if (P.D) {
+        const int pm = mode % P.L;
+        double2 out = make_double2(P.beta_re * cr + P.beta_im * ci, P.beta_im * cr - P.beta_re * ci);
+        double2* d = P.D + (size_t)(mode - pm + ((P.L - pm) % P.L)) * P.NN + (size_t)j * N + i;
+        if (P.accumulate_d) {
+            out.x += d->x;
+            out.y += d->y;
+        }
+        *d = out;
+    }
 }
 
 // 3-D view of a spectrum as doubles: (2N doubles per row, N rows, modes); boxes are 16 doubles wide
@@ -285,14 +323,27 @@ cudaError_t zgemm_init() {
     return e;
 }
 
-cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B, double* C, Cplx alpha,
-                               bool accumulate, int variant, cudaStream_t st) {
+cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out,
+                               int variant, cudaStream_t st) {
     const int modes = batch * f.L;
+    if (!out.C && !out.D) return cudaErrorInvalidValue;
+    GemmParams P;
+    P.C = reinterpret_cast<double2*>(out.C);
+    P.D = reinterpret_cast<double2*>(out.D);
+    P.NN = f.NN;
+    P.N = f.N;
+    P.L = f.L;
+    P.tiles_m = (f.N + BM - 1) / BM;
+    P.tiles_n = (f.N + BN - 1) / BN;
+    P.alpha_re = out.alpha.re;
+    P.alpha_im = out.alpha.im;
+    P.beta_re = out.beta.re;
+    P.beta_im = out.beta.im;
+    P.accumulate = out.accumulate ? 1 : 0;
+    P.accumulate_d = out.accumulate_d ? 1 : 0;
     if (variant == 0) {
         dim3 grid((f.N + 15) / 16, (f.N + 15) / 16, modes);
-        zgemm_modes_ref_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(A), reinterpret_cast<const double2*>(B),
-                                                     reinterpret_cast<double2*>(C), f.N, f.NN, alpha.re, alpha.im,
-                                                     accumulate ? 1 : 0);
+        zgemm_modes_ref_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(A), reinterpret_cast<const double2*>(B), P);
         return cudaGetLastError();
     }
     cudaError_t e = zgemm_init();
@@ -300,15 +351,6 @@ cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, 
     CUtensorMap mapA, mapB;
     if ((e = encode_operand(&mapA, A, f, modes, BM)) != cudaSuccess) return e;
     if ((e = encode_operand(&mapB, B, f, modes, BK)) != cudaSuccess) return e;
-    GemmParams P;
-    P.C = reinterpret_cast<double2*>(C);
-    P.NN = f.NN;
-    P.N = f.N;
-    P.tiles_m = (f.N + BM - 1) / BM;
-    P.tiles_n = (f.N + BN - 1) / BN;
-    P.alpha_re = alpha.re;
-    P.alpha_im = alpha.im;
-    P.accumulate = accumulate ? 1 : 0;
     const unsigned grid = (unsigned)(modes * P.tiles_m * P.tiles_n);
     zgemm_modes_dmma_kernel<<<grid, GEMM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, P);
     return cudaGetLastError();

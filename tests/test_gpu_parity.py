@@ -257,6 +257,39 @@ def test_staple_generic_links_and_z(nspt):
     check_staple(nspt, U, z)
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (1, 5), (3, 0), (57, 9), (8, 1)])
+def test_staple_edge_shapes_both_gemm_variants(nspt, N, Ntrunc, variant):
+    # degenerate sizes (N = 1, a single coefficient so L = 1, ragged tiles) and both mode-wise product
+    # kernels: the conjugate-transposed accumulate epilogue exists in each
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([46, N, Ntrunc])
+    U = [wl.gaussian_series(N, Ntrunc, rng) for _ in range(4)]
+    z = rng.standard_normal((4, 4)) + 1j * rng.standard_normal((4, 4))
+    nspt.nspt_set_gemm_variant(variant)
+    try:
+        check_staple(nspt, U, z)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+
+
+def test_staple_integer_links_bit_exact(nspt):
+    # small-integer links and a Gaussian-integer twist: every S_mu coefficient is an exact integer
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(47)
+    U = [wl.integer_series(10, 3, rng, -2, 2) for _ in range(4)]
+    z = (rng.integers(-1, 2, (4, 4)) + 1j * rng.integers(-1, 2, (4, 4))).astype(np.complex128)
+    ref = oracle.staple(U, z)
+    S = nspt.nspt_staple([to_dev(u) for u in U], z)
+    torch.cuda.synchronize()
+    for mu in range(4):
+        got = S[mu].cpu().numpy()
+        assert np.array_equal(np.rint(got.real), ref[mu].real) and np.array_equal(np.rint(got.imag), ref[mu].imag)
+        assert np.abs(got - ref[mu]).max() < 1e-6
+
+
 def test_staple_output_may_alias_links(nspt):
     import torch
     import oracle
