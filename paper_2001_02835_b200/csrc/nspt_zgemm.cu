@@ -73,62 +73,14 @@ __device__ __forceinline__ void issue_slice(const CUtensorMap* mapA, const CUten
         tma_load_3d(stage_addr + A_STAGE_BYTES + c * B_BOX_BYTES, mapB, full_bar, 2 * (n0 + 8 * c), k0, mode);
 }
 
-__global__ void __launch_bounds__(GEMM_THREADS, 3)
-zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
-                        const GemmParams P) {
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));  // same address, generic-shared pointer for loads
-    const uint32_t bar_full = base + STAGES * STAGE_BYTES;
-    const uint32_t bar_empty = bar_full + STAGES * 8;
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int tiles = P.tiles_m * P.tiles_n;
-    const int mode = blockIdx.x / tiles;
-    const int tile = blockIdx.x % tiles;
-    const int m0 = (tile / P.tiles_n) * BM, n0 = (tile % P.tiles_n) * BN;
+template <bool FULL>
+__device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUtensorMap& mapB, const GemmParams& P,
+                                              uint32_t base, const uint8_t* sgen, uint32_t bar_full, uint32_t bar_empty,
+                                              int warp, int lane, int nk, int m0, int n0, int mode, int nbm, int nbn,
+                                              uint32_t offA0, uint32_t offA1, uint32_t offB0, uint32_t offB1,
+                                              double (&p1)[3][3][2], double (&p2)[3][3][2], double (&p3)[3][3][2]) {
     const int N = P.N;
-    const int nk = (N + BK - 1) / BK;
-
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(bar_full + 8 * s, 1);
-            mbar_init(bar_empty + 8 * s, 4);
-        }
-        mbar_fence_init();
-        const int pre = nk < STAGES ? nk : STAGES;
-        for (int it = 0; it < pre; ++it)
-            issue_slice(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, it * BK, m0, n0, mode);
-    }
-    __syncthreads();
-
-    const int g = lane >> 2, t = lane & 3;
-    const int wm = warp >> 1, wn = warp & 1;
-    const int mw = 24 * wm, nw = 24 * wn;  // warp offsets inside the CTA tile
-    // number of 8-row / 8-column blocks of this warp that intersect the matrix
-    int nbm = (N - (m0 + mw) + 7) >> 3;
-    nbm = nbm < 0 ? 0 : (nbm > 3 ? 3 : nbm);
-    int nbn = (N - (n0 + nw) + 7) >> 3;
-    nbn = nbn < 0 ? 0 : (nbn > 3 ? 3 : nbn);
-    const bool active = (nbm > 0) && (nbn > 0);
-
-    double p1[3][3][2], p2[3][3][2], p3[3][3][2];
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-            p1[i][j][0] = p1[i][j][1] = 0.0;
-            p2[i][j][0] = p2[i][j][1] = 0.0;
-            p3[i][j][0] = p3[i][j][1] = 0.0;
-        }
-
-    // per-lane byte offsets of the fragment loads inside a stage (sub-step 0; sub-step 1 is derived)
-    const uint32_t offA0 = (uint32_t)((mw + g) * 128 + (((2 * t) ^ g) << 4));           // + bm*1024
-    const uint32_t offA1 = offA0 ^ 16u;                                                   // k-slot 2t+1
-    const uint32_t offB0 = (uint32_t)(A_STAGE_BYTES + (3 * wn) * B_BOX_BYTES + (2 * t) * 128 + ((g ^ (2 * t)) << 4));
-    const uint32_t offB1 = (offB0 + 128u) ^ 16u;                                          // row 2t+1
-
+    const bool active = FULL || ((nbm > 0) && (nbn > 0));
     for (int it = 0; it < nk; ++it) {
         // refill, two iterations late, by the warps in turn
         if (it >= 2 && warp == (it & 3)) {
@@ -162,10 +114,10 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
                     }
 #pragma unroll
                     for (int bm = 0; bm < 3; ++bm) {
-                        if (bm < nbm) {
+                        if (FULL || bm < nbm) {
 #pragma unroll
                             for (int bn = 0; bn < 3; ++bn) {
-                                if (bn < nbn) {
+                                if (FULL || bn < nbn) {
                                     dmma(p1[bm][bn][0], p1[bm][bn][1], a[bm].x, b[bn].x);
                                     dmma(p2[bm][bn][0], p2[bm][bn][1], a[bm].y, b[bn].y);
                                     dmma(p3[bm][bn][0], p3[bm][bn][1], as[bm], bs[bn]);
@@ -179,6 +131,77 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
     }
+
+}
+
+__global__ void __launch_bounds__(GEMM_THREADS, 3)
+zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
+                        const GemmParams P) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));  // same address, generic-shared pointer for loads
+    const uint32_t bar_full = base + STAGES * STAGE_BYTES;
+    const uint32_t bar_empty = bar_full + STAGES * 8;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tiles = P.tiles_m * P.tiles_n;
+    const int mode = blockIdx.x / tiles;
+    const int tile = blockIdx.x % tiles;
+    const int m0 = (tile / P.tiles_n) * BM, n0 = (tile % P.tiles_n) * BN;
+    const int N = P.N;
+    const int nk = (N + BK - 1) / BK;
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_empty + 8 * s, 4);
+        }
+        mbar_fence_init();
+        const int pre = nk < STAGES ? nk : STAGES;
+        for (int it = 0; it < pre; ++it)
+            issue_slice(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, it * BK, m0, n0, mode);
+    }
+    __syncthreads();
+
+    const int g = lane >> 2, t = lane & 3;
+    // Quadrant of the CTA tile this warp owns.  Edge tiles give the quadrants unequal work (out-of-range
+    // 8-blocks are skipped) and warp w always runs on scheduler w of its SM, each with its own DMMA pipe:
+    // rotating the assignment with the CTA index spreads the light quadrants over the four schedulers.
+    const int quad = (warp + blockIdx.x) & 3;
+    const int wm = quad >> 1, wn = quad & 1;
+    const int mw = 24 * wm, nw = 24 * wn;  // warp offsets inside the CTA tile
+    // number of 8-row / 8-column blocks of this warp that intersect the matrix
+    int nbm = (N - (m0 + mw) + 7) >> 3;
+    nbm = nbm < 0 ? 0 : (nbm > 3 ? 3 : nbm);
+    int nbn = (N - (n0 + nw) + 7) >> 3;
+    nbn = nbn < 0 ? 0 : (nbn > 3 ? 3 : nbn);
+    const bool active = (nbm > 0) && (nbn > 0);
+
+    double p1[3][3][2], p2[3][3][2], p3[3][3][2];
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            p1[i][j][0] = p1[i][j][1] = 0.0;
+            p2[i][j][0] = p2[i][j][1] = 0.0;
+            p3[i][j][0] = p3[i][j][1] = 0.0;
+        }
+
+    // per-lane byte offsets of the fragment loads inside a stage (sub-step 0; sub-step 1 is derived)
+    const uint32_t offA0 = (uint32_t)((mw + g) * 128 + (((2 * t) ^ g) << 4));           // + bm*1024
+    const uint32_t offA1 = offA0 ^ 16u;                                                   // k-slot 2t+1
+    const uint32_t offB0 = (uint32_t)(A_STAGE_BYTES + (3 * wn) * B_BOX_BYTES + (2 * t) * 128 + ((g ^ (2 * t)) << 4));
+    const uint32_t offB1 = (offB0 + 128u) ^ 16u;                                          // row 2t+1
+
+    // Warps whose 3 x 3 blocks all intersect the matrix (all but those on the last tile row / column) run
+    // an unpredicated copy of the loop: predicated mma.sync costs a WARPSYNC and issue bubbles per group.
+    if (nbm == 3 && nbn == 3)
+        gemm_mainloop<true>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, mode, 3, 3, offA0, offA1,
+                            offB0, offB1, p1, p2, p3);
+    else
+        gemm_mainloop<false>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, mode, nbm, nbn, offA0,
+                             offA1, offB0, offB1, p1, p2, p3);
 
     if (!active) return;
     // ---------------------------------------------------------------- epilogue
