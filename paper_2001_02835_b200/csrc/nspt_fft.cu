@@ -315,11 +315,17 @@ template <int R, int S, int T>
 struct Cfg {
     static constexpr int L = R * S;
     static constexpr int THREADS = T * S;
-    static constexpr int EXCH_BYTES = L * T * 16;            // exchange buffer [p1][s][c]
-    static constexpr int FWD_STAGE_BYTES = (L / 2) * T * 16;  // input tile [order < L/2][T]
-    static constexpr int INV_STAGE_BYTES = L * T * 16;        // input tile [mode][T]; doubles as the exchange buffer
-    static constexpr int FWD_SMEM = EXCH_BYTES + 2 * FWD_STAGE_BYTES + 16 + 128;
-    static constexpr int INV_SMEM = 2 * INV_STAGE_BYTES + 16 + 128;
+    static constexpr int FULL_TILE_BYTES = L * T * 16;        // [mode][T] tile, also the exchange buffer
+    static constexpr int HALF_TILE_BYTES = (L / 2) * T * 16;  // [order < L/2][T] tile
+    // forward: ring of input tiles (orders) + two exchange buffers that double as TMA-store sources
+    static constexpr int FWD_STAGES = 3, FWD_OUTS = 2;
+    static constexpr int FWD_SMEM = FWD_STAGES * HALF_TILE_BYTES + FWD_OUTS * FULL_TILE_BYTES + 64 + 128;
+    // inverse: ring of input tiles (modes) + exchange buffer + one output tile (orders)
+    static constexpr int INV_STAGES = 2;
+    static constexpr int INV_SMEM = INV_STAGES * FULL_TILE_BYTES + FULL_TILE_BYTES + HALF_TILE_BYTES + 64 + 128;
+    // re-truncation: ring of input tiles (modes) + one exchange buffer that is also the store source
+    static constexpr int RET_STAGES = 2;
+    static constexpr int RET_SMEM = RET_STAGES * FULL_TILE_BYTES + FULL_TILE_BYTES + 64 + 128;
 };
 
 __device__ __forceinline__ void tile_coords(unsigned tile, const XformParams& P, unsigned& tx, unsigned& b, unsigned& z) {
@@ -329,51 +335,79 @@ __device__ __forceinline__ void tile_coords(unsigned tile, const XformParams& P,
     z = zb / (unsigned)P.batch;
 }
 
+// Forward phases on shared memory.  Phase 1: thread s parks Y_s[p1] w_L^(s p1) at slot [s][p1]; phase 2: thread q
+// owns p1 = q + S a, reads slots [sp][p1] (all sp) and overwrites THE SAME slots with X[p1 + R p2] at [p2][p1],
+// which is the natural mode order p = p1 + R p2: the exchange buffer becomes the [mode][T] output tile in place.
 template <int R, int S, int T>
-__global__ void __launch_bounds__(T* S) fft_forward_tma_kernel(const __grid_constant__ CUtensorMap map0,
-                                                              const __grid_constant__ CUtensorMap map1,
+__device__ __forceinline__ void forward_phase1_smem(const double2 (&x)[R], int s, int c, const double2* __restrict__ tw,
+                                                    double2* exch) {
+    double2 Y[R];
+    Dft<R, +1, true, false>::run(x, Y);
+#pragma unroll
+    for (int p1 = 0; p1 < R; ++p1) {
+        const double2 w = __ldg(&tw[s * p1]);  // w_L^(s p1), s p1 < L
+        exch[(s * R + p1) * T + c] = (p1 == 0) ? Y[p1] : cmul(Y[p1], w);
+    }
+}
+template <int R, int S, int T>
+__device__ __forceinline__ void forward_phase2_smem(int s, int c, double2* exch) {
+#pragma unroll
+    for (int a = 0; a < R / S; ++a) {
+        const int p1 = s + S * a;
+        double2 y[S], X[S];
+#pragma unroll
+        for (int sp = 0; sp < S; ++sp) y[sp] = exch[(sp * R + p1) * T + c];
+        Dft<S, +1, false, false>::run(y, X);
+#pragma unroll
+        for (int p2 = 0; p2 < S; ++p2) exch[(p2 * R + p1) * T + c] = X[p2];
+    }
+}
+
+template <int R, int S, int T>
+__global__ void __launch_bounds__(T* S) fft_forward_tma_kernel(const __grid_constant__ CUtensorMap in0,
+                                                              const __grid_constant__ CUtensorMap in1,
+                                                              const __grid_constant__ CUtensorMap out0,
+                                                              const __grid_constant__ CUtensorMap out1,
                                                               const XformParams P) {
     using C = Cfg<R, S, T>;
+    constexpr int NS = C::FWD_STAGES;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
     uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));
-    double2* exch = reinterpret_cast<double2*>(sgen);
-    const uint32_t stage_addr = base + C::EXCH_BYTES;
-    const double2* stage_gen = reinterpret_cast<const double2*>(sgen + C::EXCH_BYTES);
-    const uint32_t bar = stage_addr + 2 * C::FWD_STAGE_BYTES;  // two 8-byte mbarriers
+    const uint32_t out_addr = base + NS * C::HALF_TILE_BYTES;
+    const uint32_t bar = out_addr + C::FWD_OUTS * C::FULL_TILE_BYTES;  // NS 8-byte mbarriers
 
     const int c = threadIdx.x % T, s = threadIdx.x / T;
 
     auto issue = [&](unsigned tile, int stage) {
         unsigned tx, b, z;
         tile_coords(tile, P, tx, b, z);
-        mbar_expect_tx(bar + 8 * stage, C::FWD_STAGE_BYTES);
-        tma_load_3d(stage_addr + stage * C::FWD_STAGE_BYTES, z ? &map1 : &map0, bar + 8 * stage, (int)(2 * tx * T), 0, (int)b);
+        mbar_expect_tx(bar + 8 * stage, C::HALF_TILE_BYTES);
+        tma_load_3d(base + stage * C::HALF_TILE_BYTES, z ? &in1 : &in0, bar + 8 * stage, (int)(2 * tx * T), 0, (int)b);
     };
 
     if (threadIdx.x == 0) {
-        mbar_init(bar, 1);
-        mbar_init(bar + 8, 1);
+#pragma unroll
+        for (int i = 0; i < NS; ++i) mbar_init(bar + 8 * i, 1);
         mbar_fence_init();
-        if (blockIdx.x < P.total_tiles) issue(blockIdx.x, 0);
-        if (blockIdx.x + gridDim.x < P.total_tiles) issue(blockIdx.x + gridDim.x, 1);
+#pragma unroll
+        for (int i = 0; i < NS; ++i)
+            if (blockIdx.x + i * gridDim.x < P.total_tiles) issue(blockIdx.x + i * gridDim.x, i);
     }
     __syncthreads();
 
     unsigned it = 0;
     for (unsigned tile = blockIdx.x; tile < P.total_tiles; tile += gridDim.x, ++it) {
-        const int stage = it & 1;
+        const int stage = it % NS;
         unsigned tx, b, z;
         tile_coords(tile, P, tx, b, z);
-        const size_t e = (size_t)tx * T + c;
-        const bool valid = e < P.NN;
-        mbar_wait(bar + 8 * stage, (it >> 1) & 1);
-        const double2* in = stage_gen + (size_t)stage * (C::FWD_STAGE_BYTES / 16);
+        mbar_wait(bar + 8 * stage, (it / NS) & 1);
+        const double2* in = reinterpret_cast<const double2*>(sgen + stage * C::HALF_TILE_BYTES);
         double2 x[R];
 #pragma unroll
         for (int r = 0; r < R / 2; ++r) {
             const int k = S * r + s;
-            double2 v = in[k * T + c];  // rows >= n and elements >= N^2 were zero-filled by TMA
+            double2 v = in[k * T + c];  // rows >= n and elements >= N^2 were zero-filled by TMA (Step 1's padding)
             if (P.use_scale && k < P.n) {
                 const double sc = __ldg(&P.scale_in[k]);
                 v.x *= sc;
@@ -383,93 +417,114 @@ __global__ void __launch_bounds__(T* S) fft_forward_tma_kernel(const __grid_cons
         }
 #pragma unroll
         for (int r = R / 2; r < R; ++r) x[r] = make_double2(0.0, 0.0);
-        double2* out = (z ? P.dst_freq[1] : P.dst_freq[0]) + (size_t)b * C::L * P.NN + e;
-        // phase 1 + __syncthreads (all threads have consumed the input stage) + phase 2
-        {
-            double2 Y[R];
-            Dft<R, +1, true, false>::run(x, Y);
-#pragma unroll
-            for (int p1 = 0; p1 < R; ++p1) {
-                const double2 w = __ldg(&P.tw_fwd[s * p1]);
-                exch[(p1 * S + s) * T + c] = (p1 == 0) ? Y[p1] : cmul(Y[p1], w);
-            }
-        }
-        __syncthreads();
+        const int ob = it & 1;
+        double2* exch = reinterpret_cast<double2*>(sgen + NS * C::HALF_TILE_BYTES + ob * C::FULL_TILE_BYTES);
+        if (threadIdx.x == 0) tma_store_wait_read<1>();  // the store issued two tiles ago has left buffer `ob`
+        __syncthreads();  // input stage consumed by everyone; exchange buffer `ob` is free
         if (threadIdx.x == 0) {
-            const unsigned next = tile + 2 * gridDim.x;
+            const unsigned next = tile + NS * gridDim.x;
             if (next < P.total_tiles) issue(next, stage);
         }
-#pragma unroll
-        for (int a = 0; a < R / S; ++a) {
-            const int p1 = s + S * a;
-            double2 y[S], X[S];
-#pragma unroll
-            for (int sp = 0; sp < S; ++sp) y[sp] = exch[(p1 * S + sp) * T + c];
-            Dft<S, +1, false, false>::run(y, X);
-            if (valid) {
-#pragma unroll
-                for (int p2 = 0; p2 < S; ++p2) out[(size_t)(p1 + R * p2) * P.NN] = X[p2];
-            }
+        forward_phase1_smem<R, S, T>(x, s, c, P.tw_fwd, exch);
+        __syncthreads();
+        forward_phase2_smem<R, S, T>(s, c, exch);
+        fence_proxy_async_smem();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            tma_store_3d(z ? &out1 : &out0, out_addr + ob * C::FULL_TILE_BYTES, (int)(2 * tx * T), 0, (int)b);
+            tma_store_commit();
         }
-        __syncthreads();  // exchange buffer free for the next tile
     }
+    if (threadIdx.x == 0) tma_store_wait_read<0>();
 }
 
+// Inverse (+ 1/L, truncation, unscale) and, with RETRUNC, the fused inverse -> truncate -> forward pass.
 template <int R, int S, int T, bool RETRUNC>
-__global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_constant__ CUtensorMap map, const XformParams P) {
+__global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_constant__ CUtensorMap in_map,
+                                                              const __grid_constant__ CUtensorMap out_map,
+                                                              const XformParams P) {
     using C = Cfg<R, S, T>;
+    constexpr int NS = RETRUNC ? C::RET_STAGES : C::INV_STAGES;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
     uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));
-    const uint32_t bar = base + 2 * C::INV_STAGE_BYTES;
+    const uint32_t exch_addr = base + NS * C::FULL_TILE_BYTES;
+    double2* exch = reinterpret_cast<double2*>(sgen + NS * C::FULL_TILE_BYTES);
+    const uint32_t outb_addr = exch_addr + C::FULL_TILE_BYTES;  // [order][T] output tile (plain inverse only)
+    double2* outb = reinterpret_cast<double2*>(sgen + (NS + 1) * C::FULL_TILE_BYTES);
+    const uint32_t bar = RETRUNC ? outb_addr : outb_addr + C::HALF_TILE_BYTES;
 
     const int c = threadIdx.x % T, s = threadIdx.x / T;
 
     auto issue = [&](unsigned tile, int stage) {
         unsigned tx, b, z;
         tile_coords(tile, P, tx, b, z);
-        mbar_expect_tx(bar + 8 * stage, C::INV_STAGE_BYTES);
-        tma_load_3d(base + stage * C::INV_STAGE_BYTES, &map, bar + 8 * stage, (int)(2 * tx * T), 0, (int)b);
+        mbar_expect_tx(bar + 8 * stage, C::FULL_TILE_BYTES);
+        tma_load_3d(base + stage * C::FULL_TILE_BYTES, &in_map, bar + 8 * stage, (int)(2 * tx * T), 0, (int)b);
     };
 
     if (threadIdx.x == 0) {
-        mbar_init(bar, 1);
-        mbar_init(bar + 8, 1);
+#pragma unroll
+        for (int i = 0; i < NS; ++i) mbar_init(bar + 8 * i, 1);
         mbar_fence_init();
-        if (blockIdx.x < P.total_tiles) issue(blockIdx.x, 0);
-        if (blockIdx.x + gridDim.x < P.total_tiles) issue(blockIdx.x + gridDim.x, 1);
+#pragma unroll
+        for (int i = 0; i < NS; ++i)
+            if (blockIdx.x + i * gridDim.x < P.total_tiles) issue(blockIdx.x + i * gridDim.x, i);
     }
     __syncthreads();
 
     unsigned it = 0;
     for (unsigned tile = blockIdx.x; tile < P.total_tiles; tile += gridDim.x, ++it) {
-        const int stage = it & 1;
+        const int stage = it % NS;
         unsigned tx, b, z;
         tile_coords(tile, P, tx, b, z);
-        const size_t e = (size_t)tx * T + c;
-        const bool valid = e < P.NN;
-        mbar_wait(bar + 8 * stage, (it >> 1) & 1);
-        double2* buf = reinterpret_cast<double2*>(sgen + (size_t)stage * C::INV_STAGE_BYTES);
+        mbar_wait(bar + 8 * stage, (it / NS) & 1);
+        const double2* in = reinterpret_cast<const double2*>(sgen + stage * C::FULL_TILE_BYTES);
         double2 x[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) x[r] = buf[(S * r + s) * T + c];
-        __syncthreads();  // the stage now serves as the exchange buffer
+        for (int r = 0; r < R; ++r) x[r] = in[(S * r + s) * T + c];
+        if (threadIdx.x == 0) tma_store_wait_read<0>();  // the previous tile's store has left `exch` / `outb`
+        __syncthreads();  // input stage consumed; exchange buffer free
+        if (threadIdx.x == 0) {
+            const unsigned next = tile + NS * gridDim.x;
+            if (next < P.total_tiles) issue(next, stage);
+        }
         InvRegs<R, S, T> q;
-        inverse_from_regs<R, S, T>(x, s, c, P.tw_inv, buf, q);
+        inverse_from_regs<R, S, T>(x, s, c, P.tw_inv, exch, q);
         if constexpr (RETRUNC) {
             double2 xf[R];
             retruncate_regs<R, S, T>(q, s, P.n, P.inv_L, xf);
             __syncthreads();  // phase-2 reads of the inverse are done
-            forward_from_regs<R, S, T>(xf, s, c, valid, P.dst_freq[0] + (size_t)b * C::L * P.NN + e, P.NN, P.tw_fwd, buf);
+            forward_phase1_smem<R, S, T>(xf, s, c, P.tw_fwd, exch);
+            __syncthreads();
+            forward_phase2_smem<R, S, T>(s, c, exch);
+            fence_proxy_async_smem();
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                tma_store_3d(&out_map, exch_addr, (int)(2 * tx * T), 0, (int)b);
+                tma_store_commit();
+            }
         } else {
-            if (valid) store_series<R, S, T>(q, s, P.n, P.scale_out, P.dst_series + (size_t)b * P.n * P.NN + e, P.NN);
-        }
-        __syncthreads();  // all reads of this stage are done: refill it
-        if (threadIdx.x == 0) {
-            const unsigned next = tile + 2 * gridDim.x;
-            if (next < P.total_tiles) issue(next, stage);
+            // rows k >= n of the tile are never written: the series tensor has n rows, TMA clips the rest (Step 5)
+#pragma unroll
+            for (int a = 0; a < InvRegs<R, S, T>::A; ++a)
+#pragma unroll
+                for (int k2 = 0; k2 < InvRegs<R, S, T>::K2; ++k2) {
+                    const int k = (s + S * a) + R * k2;
+                    if (k < P.n) {
+                        const double sc = __ldg(&P.scale_out[k]);  // s^-k / L
+                        outb[k * T + c] = make_double2(q.v[a][k2].x * sc, q.v[a][k2].y * sc);
+                    }
+                }
+            fence_proxy_async_smem();
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                tma_store_3d(&out_map, outb_addr, (int)(2 * tx * T), 0, (int)b);
+                tma_store_commit();
+            }
         }
     }
+    if (threadIdx.x == 0) tma_store_wait_read<0>();
 }
 
 // Spectrum of the daggered series (g is real): FFT[X^+](p) = (X~((L-p) mod L))^H.
@@ -544,33 +599,37 @@ cudaError_t run_tma(Which w, XformParams P, int nops, cudaStream_t st) {
     P.total_tiles = P.tiles_x * (unsigned)P.batch * (unsigned)nops;
     cudaError_t e;
     unsigned grid = 0;
+    // series viewed as doubles: (2 N^2 per order, n orders, batch); spectrum: (2 N^2 per mode, L modes, batch)
+    const uint64_t sdims[3] = {(uint64_t)(2 * P.NN), (uint64_t)P.n, (uint64_t)P.batch};
+    const uint64_t sstrides[2] = {(uint64_t)P.NN * 16, (uint64_t)P.n * P.NN * 16};
+    const uint32_t sbox[3] = {2 * T, (uint32_t)(C::L / 2), 1};
+    const uint64_t fdims[3] = {(uint64_t)(2 * P.NN), (uint64_t)C::L, (uint64_t)P.batch};
+    const uint64_t fstrides[2] = {(uint64_t)P.NN * 16, (uint64_t)C::L * P.NN * 16};
+    const uint32_t fbox[3] = {2 * T, (uint32_t)C::L, 1};
     if (w == W_FWD) {
-        // series viewed as doubles: (2 N^2 per order, n orders, batch); box = (2T, L/2, 1)
-        CUtensorMap maps[2];
-        const uint64_t dims[3] = {(uint64_t)(2 * P.NN), (uint64_t)P.n, (uint64_t)P.batch};
-        const uint64_t strides[2] = {(uint64_t)P.NN * 16, (uint64_t)P.n * P.NN * 16};
-        const uint32_t box[3] = {2 * T, (uint32_t)(C::L / 2), 1};
+        CUtensorMap in[2], out[2];
         for (int z = 0; z < 2; ++z) {
-            const void* src = P.src_series[z] ? P.src_series[z] : P.src_series[0];
-            if ((e = tma_encode_f64(&maps[z], src, 3, dims, strides, box, false)) != cudaSuccess) return e;
+            const void* src = P.src_series[z] ? (const void*)P.src_series[z] : (const void*)P.src_series[0];
+            const void* dst = P.dst_freq[z] ? (const void*)P.dst_freq[z] : (const void*)P.dst_freq[0];
+            if ((e = tma_encode_f64(&in[z], src, 3, sdims, sstrides, sbox, false)) != cudaSuccess) return e;
+            if ((e = tma_encode_f64(&out[z], dst, 3, fdims, fstrides, fbox, false)) != cudaSuccess) return e;
         }
         auto kern = fft_forward_tma_kernel<R, S, T>;
         if ((e = persistent_grid(kern, C::THREADS, C::FWD_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
-        kern<<<grid, C::THREADS, C::FWD_SMEM, st>>>(maps[0], maps[1], P);
+        kern<<<grid, C::THREADS, C::FWD_SMEM, st>>>(in[0], in[1], out[0], out[1], P);
     } else {
-        CUtensorMap map;
-        const uint64_t dims[3] = {(uint64_t)(2 * P.NN), (uint64_t)C::L, (uint64_t)P.batch};
-        const uint64_t strides[2] = {(uint64_t)P.NN * 16, (uint64_t)C::L * P.NN * 16};
-        const uint32_t box[3] = {2 * T, (uint32_t)C::L, 1};
-        if ((e = tma_encode_f64(&map, P.src_freq, 3, dims, strides, box, false)) != cudaSuccess) return e;
+        CUtensorMap in, out;
+        if ((e = tma_encode_f64(&in, P.src_freq, 3, fdims, fstrides, fbox, false)) != cudaSuccess) return e;
         if (w == W_INV) {
+            if ((e = tma_encode_f64(&out, P.dst_series, 3, sdims, sstrides, sbox, false)) != cudaSuccess) return e;
             auto kern = fft_inverse_tma_kernel<R, S, T, false>;
             if ((e = persistent_grid(kern, C::THREADS, C::INV_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
-            kern<<<grid, C::THREADS, C::INV_SMEM, st>>>(map, P);
+            kern<<<grid, C::THREADS, C::INV_SMEM, st>>>(in, out, P);
         } else {
+            if ((e = tma_encode_f64(&out, P.dst_freq[0], 3, fdims, fstrides, fbox, false)) != cudaSuccess) return e;
             auto kern = fft_inverse_tma_kernel<R, S, T, true>;
-            if ((e = persistent_grid(kern, C::THREADS, C::INV_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
-            kern<<<grid, C::THREADS, C::INV_SMEM, st>>>(map, P);
+            if ((e = persistent_grid(kern, C::THREADS, C::RET_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
+            kern<<<grid, C::THREADS, C::RET_SMEM, st>>>(in, out, P);
         }
     }
     return cudaGetLastError();
