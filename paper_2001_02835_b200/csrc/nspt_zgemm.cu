@@ -33,14 +33,25 @@
 namespace nspt {
 namespace {
 
-constexpr int BM = 48, BN = 48, BK = 8;
-constexpr int STAGES = 5;
-constexpr int A_STAGE_BYTES = BM * BK * 16;                    // 6144: [m][8 complex]
+constexpr int BK = 8;
 constexpr int B_BOX_BYTES = BK * 8 * 16;                       // 1024: [k][8 complex]
-constexpr int B_STAGE_BYTES = (BN / 8) * B_BOX_BYTES;          // 6144
-constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;     // 12288
-constexpr int GEMM_THREADS = 128;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8 + 1024;  // + barriers + alignment slack
+
+// Tiling of one kernel instance: a warp owns MB x NB DMMA blocks (8 MB rows x 8 NB columns), the CTA has
+// WM x WN warps, MINB CTAs share an SM, the operand ring is NSTAGES K-slices deep.
+template <int MB_, int NB_, int WM_, int WN_, int MINB_, int NSTAGES_, int LAG_ = 2>
+struct Tile {
+    static constexpr int LAG = LAG_;
+    static constexpr int MB = MB_, NB = NB_, WM = WM_, WN = WN_, MINB = MINB_, STAGES = NSTAGES_;
+    static constexpr int WARPS = WM * WN;
+    static constexpr int THREADS = 32 * WARPS;
+    static constexpr int BM = 8 * MB * WM, BN = 8 * NB * WN;
+    static constexpr int A_STAGE_BYTES = BM * BK * 16;             // [m][8 complex]
+    static constexpr int B_STAGE_BYTES = (BN / 8) * B_BOX_BYTES;   // BN/8 boxes [k][8 complex]
+    static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * STAGES * 8 + 1024;  // + barriers + alignment slack
+    static_assert((WARPS & (WARPS - 1)) == 0, "warp count must be a power of two");
+    static_assert(BM <= 256 && A_STAGE_BYTES % 1024 == 0, "A box");
+};
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -64,34 +75,30 @@ struct GemmParams {
     int accumulate, accumulate_d;
 };
 
+template <class TC>
 __device__ __forceinline__ void issue_slice(const CUtensorMap* mapA, const CUtensorMap* mapB, uint32_t stage_addr,
                                             uint32_t full_bar, int k0, int m0, int n0, int mode) {
-    mbar_expect_tx(full_bar, STAGE_BYTES);
+    mbar_expect_tx(full_bar, TC::STAGE_BYTES);
     tma_load_3d(stage_addr, mapA, full_bar, 2 * k0, m0, mode);
 #pragma unroll
-    for (int c = 0; c < BN / 8; ++c)
-        tma_load_3d(stage_addr + A_STAGE_BYTES + c * B_BOX_BYTES, mapB, full_bar, 2 * (n0 + 8 * c), k0, mode);
+    for (int c = 0; c < TC::BN / 8; ++c)
+        tma_load_3d(stage_addr + TC::A_STAGE_BYTES + c * B_BOX_BYTES, mapB, full_bar, 2 * (n0 + 8 * c), k0, mode);
 }
 
-template <bool FULL>
+template <class TC, bool FULL>
 __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUtensorMap& mapB, const GemmParams& P,
                                               uint32_t base, const uint8_t* sgen, uint32_t bar_full, uint32_t bar_empty,
                                               int warp, int lane, int nk, int m0, int n0, int mode, int nbm, int nbn,
                                               uint32_t offA0, uint32_t offA1, uint32_t offB0, uint32_t offB1,
-                                              double (&p1)[3][3][2], double (&p2)[3][3][2], double (&p3)[3][3][2]) {
+                                              double (&p1)[TC::MB][TC::NB][2], double (&p2)[TC::MB][TC::NB][2],
+                                              double (&p3)[TC::MB][TC::NB][2]) {
+    constexpr int MB = TC::MB, NB = TC::NB, STAGES = TC::STAGES, STAGE_BYTES = TC::STAGE_BYTES;
     const int N = P.N;
     const bool active = FULL || ((nbm > 0) && (nbn > 0));
     for (int it = 0; it < nk; ++it) {
-        // refill, two iterations late, by the warps in turn
-        if (it >= 2 && warp == (it & 3)) {
-            const int j = it - 2;
-            if (j + STAGES < nk && lane == 0) {
-                const int slot = j % STAGES;
-                mbar_wait(bar_empty + 8 * slot, (j / STAGES) & 1);
-                issue_slice(&mapA, &mapB, base + slot * STAGE_BYTES, bar_full + 8 * slot, (j + STAGES) * BK, m0, n0, mode);
-            }
-            __syncwarp();
-        }
+        // keep the four fragment offsets in registers (ptxas otherwise rematerialises them from the lane and
+        // CTA indices inside every sub-step, ~20 dependent integer instructions in front of the loads)
+        asm volatile("" : "+r"(offA0), "+r"(offA1), "+r"(offB0), "+r"(offB1));
         const int slot = it % STAGES;
         mbar_wait(bar_full + 8 * slot, (it / STAGES) & 1);
         if (active) {
@@ -100,23 +107,23 @@ __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUt
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
                 if (s < nsub) {
-                    double2 a[3], b[3];
-                    double as[3], bs[3];
+                    double2 a[MB], b[NB];
+                    double as[MB], bs[NB];
 #pragma unroll
-                    for (int bm = 0; bm < 3; ++bm) {
+                    for (int bm = 0; bm < MB; ++bm) {
                         a[bm] = *reinterpret_cast<const double2*>(st + (s ? offA1 : offA0) + bm * 1024);
                         as[bm] = a[bm].x + a[bm].y;
                     }
 #pragma unroll
-                    for (int bn = 0; bn < 3; ++bn) {
+                    for (int bn = 0; bn < NB; ++bn) {
                         b[bn] = *reinterpret_cast<const double2*>(st + (s ? offB1 : offB0) + bn * B_BOX_BYTES);
                         bs[bn] = b[bn].x + b[bn].y;
                     }
 #pragma unroll
-                    for (int bm = 0; bm < 3; ++bm) {
+                    for (int bm = 0; bm < MB; ++bm) {
                         if (FULL || bm < nbm) {
 #pragma unroll
-                            for (int bn = 0; bn < 3; ++bn) {
+                            for (int bn = 0; bn < NB; ++bn) {
                                 if (FULL || bn < nbn) {
                                     dmma(p1[bm][bn][0], p1[bm][bn][1], a[bm].x, b[bn].x);
                                     dmma(p2[bm][bn][0], p2[bm][bn][1], a[bm].y, b[bn].y);
@@ -130,13 +137,26 @@ __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUt
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
+        if (it + 1 >= TC::LAG && warp == ((it + 1) & (TC::WARPS - 1))) {
+            // refill of the slot released LAG iterations ago, by the warps in turn: by then even the slowest warp
+            // has released it, so the wait below does not block (LAG = 1 or a refill by the last arriver costs 5 %)
+            const int j = it + 1 - TC::LAG;
+            if (j + STAGES < nk && lane == 0) {
+                const int sl = j % STAGES;
+                mbar_wait(bar_empty + 8 * sl, (j / STAGES) & 1);
+                issue_slice<TC>(&mapA, &mapB, base + sl * STAGE_BYTES, bar_full + 8 * sl, (j + STAGES) * BK, m0, n0, mode);
+            }
+            __syncwarp();
+        }
     }
-
 }
 
-__global__ void __launch_bounds__(GEMM_THREADS, 3)
+template <class TC>
+__global__ void __launch_bounds__(TC::THREADS, TC::MINB)
 zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
                         const GemmParams P) {
+    constexpr int MB = TC::MB, NB = TC::NB, STAGES = TC::STAGES, STAGE_BYTES = TC::STAGE_BYTES;
+    constexpr int BM = TC::BM, BN = TC::BN;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));  // same address, generic-shared pointer for loads
@@ -155,34 +175,34 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(bar_full + 8 * s, 1);
-            mbar_init(bar_empty + 8 * s, 4);
+            mbar_init(bar_empty + 8 * s, TC::WARPS);
         }
         mbar_fence_init();
         const int pre = nk < STAGES ? nk : STAGES;
         for (int it = 0; it < pre; ++it)
-            issue_slice(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, it * BK, m0, n0, mode);
+            issue_slice<TC>(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, it * BK, m0, n0, mode);
     }
     __syncthreads();
 
     const int g = lane >> 2, t = lane & 3;
-    // Quadrant of the CTA tile this warp owns.  Edge tiles give the quadrants unequal work (out-of-range
-    // 8-blocks are skipped) and warp w always runs on scheduler w of its SM, each with its own DMMA pipe:
-    // rotating the assignment with the CTA index spreads the light quadrants over the four schedulers.
-    const int quad = (warp + blockIdx.x) & 3;
-    const int wm = quad >> 1, wn = quad & 1;
-    const int mw = 24 * wm, nw = 24 * wn;  // warp offsets inside the CTA tile
+    // Part of the CTA tile this warp owns.  Edge tiles give the warps unequal work (out-of-range 8-blocks are
+    // skipped) and warp w always runs on scheduler w % 4 of its SM, each with its own DMMA pipe: rotating the
+    // assignment with the CTA index spreads the light parts over the four schedulers.
+    const int quad = (warp + blockIdx.x) & (TC::WARPS - 1);
+    const int wm = quad / TC::WN, wn = quad % TC::WN;
+    const int mw = 8 * MB * wm, nw = 8 * NB * wn;  // warp offsets inside the CTA tile
     // number of 8-row / 8-column blocks of this warp that intersect the matrix
     int nbm = (N - (m0 + mw) + 7) >> 3;
-    nbm = nbm < 0 ? 0 : (nbm > 3 ? 3 : nbm);
+    nbm = nbm < 0 ? 0 : (nbm > MB ? MB : nbm);
     int nbn = (N - (n0 + nw) + 7) >> 3;
-    nbn = nbn < 0 ? 0 : (nbn > 3 ? 3 : nbn);
+    nbn = nbn < 0 ? 0 : (nbn > NB ? NB : nbn);
     const bool active = (nbm > 0) && (nbn > 0);
 
-    double p1[3][3][2], p2[3][3][2], p3[3][3][2];
+    double p1[MB][NB][2], p2[MB][NB][2], p3[MB][NB][2];
 #pragma unroll
-    for (int i = 0; i < 3; ++i)
+    for (int i = 0; i < MB; ++i)
 #pragma unroll
-        for (int j = 0; j < 3; ++j) {
+        for (int j = 0; j < NB; ++j) {
             p1[i][j][0] = p1[i][j][1] = 0.0;
             p2[i][j][0] = p2[i][j][1] = 0.0;
             p3[i][j][0] = p3[i][j][1] = 0.0;
@@ -191,17 +211,18 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
     // per-lane byte offsets of the fragment loads inside a stage (sub-step 0; sub-step 1 is derived)
     const uint32_t offA0 = (uint32_t)((mw + g) * 128 + (((2 * t) ^ g) << 4));           // + bm*1024
     const uint32_t offA1 = offA0 ^ 16u;                                                   // k-slot 2t+1
-    const uint32_t offB0 = (uint32_t)(A_STAGE_BYTES + (3 * wn) * B_BOX_BYTES + (2 * t) * 128 + ((g ^ (2 * t)) << 4));
+    const uint32_t offB0 =
+        (uint32_t)(TC::A_STAGE_BYTES + (NB * wn) * B_BOX_BYTES + (2 * t) * 128 + ((g ^ (2 * t)) << 4));  // + bn*1024
     const uint32_t offB1 = (offB0 + 128u) ^ 16u;                                          // row 2t+1
 
-    // Warps whose 3 x 3 blocks all intersect the matrix (all but those on the last tile row / column) run
+    // Warps whose MB x NB blocks all intersect the matrix (all but those on the last tile row / column) run
     // an unpredicated copy of the loop: predicated mma.sync costs a WARPSYNC and issue bubbles per group.
-    if (nbm == 3 && nbn == 3)
-        gemm_mainloop<true>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, mode, 3, 3, offA0, offA1,
-                            offB0, offB1, p1, p2, p3);
+    if (nbm == MB && nbn == NB)
+        gemm_mainloop<TC, true>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, mode, MB, NB, offA0,
+                                offA1, offB0, offB1, p1, p2, p3);
     else
-        gemm_mainloop<false>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, mode, nbm, nbn, offA0,
-                             offA1, offB0, offB1, p1, p2, p3);
+        gemm_mainloop<TC, false>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, mode, nbm, nbn,
+                                 offA0, offA1, offB0, offB1, p1, p2, p3);
 
     if (!active) return;
     // ---------------------------------------------------------------- epilogue
@@ -210,11 +231,11 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
     const int pm = mode % P.L;
     double2* Dm = P.D ? P.D + (size_t)(mode - pm + ((P.L - pm) % P.L)) * P.NN : nullptr;
 #pragma unroll
-    for (int bm = 0; bm < 3; ++bm) {
+    for (int bm = 0; bm < MB; ++bm) {
         const int m = m0 + mw + 8 * bm + g;
         if (bm < nbm && m < N) {
 #pragma unroll
-            for (int bn = 0; bn < 3; ++bn) {
+            for (int bn = 0; bn < NB; ++bn) {
                 const int n = n0 + nw + 8 * bn + 2 * t;
                 if (bn < nbn && n < N) {
                     const double cr0 = p1[bm][bn][0] - p2[bm][bn][0];
@@ -338,13 +359,30 @@ cudaError_t tma_encode_f64(CUtensorMap* map, const void* base, int rank, const u
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-cudaError_t zgemm_init() {
-    static bool done = false;
-    if (done) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(zgemm_modes_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-    if (e == cudaSuccess) done = true;
-    return e;
+cudaError_t zgemm_init() { return cudaSuccess; }
+
+namespace {
+
+template <class TC>
+cudaError_t launch_dmma(const FreqLayout& f, int modes, const double* A, const double* B, GemmParams P, cudaStream_t st) {
+    static bool attr_done = false;
+    cudaError_t e;
+    if (!attr_done) {
+        e = cudaFuncSetAttribute(zgemm_modes_dmma_kernel<TC>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    P.tiles_m = (f.N + TC::BM - 1) / TC::BM;
+    P.tiles_n = (f.N + TC::BN - 1) / TC::BN;
+    CUtensorMap mapA, mapB;
+    if ((e = encode_operand(&mapA, A, f, modes, TC::BM)) != cudaSuccess) return e;
+    if ((e = encode_operand(&mapB, B, f, modes, BK)) != cudaSuccess) return e;
+    const unsigned grid = (unsigned)(modes * P.tiles_m * P.tiles_n);
+    zgemm_modes_dmma_kernel<TC><<<grid, TC::THREADS, TC::SMEM_BYTES, st>>>(mapA, mapB, P);
+    return cudaGetLastError();
 }
+
+}  // namespace
 
 cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out,
                                int variant, cudaStream_t st) {
@@ -356,27 +394,26 @@ cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, 
     P.NN = f.NN;
     P.N = f.N;
     P.L = f.L;
-    P.tiles_m = (f.N + BM - 1) / BM;
-    P.tiles_n = (f.N + BN - 1) / BN;
+    P.tiles_m = P.tiles_n = 0;
     P.alpha_re = out.alpha.re;
     P.alpha_im = out.alpha.im;
     P.beta_re = out.beta.re;
     P.beta_im = out.beta.im;
     P.accumulate = out.accumulate ? 1 : 0;
     P.accumulate_d = out.accumulate_d ? 1 : 0;
-    if (variant == 0) {
-        dim3 grid((f.N + 15) / 16, (f.N + 15) / 16, modes);
-        zgemm_modes_ref_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(A), reinterpret_cast<const double2*>(B), P);
-        return cudaGetLastError();
+    switch (variant) {
+        case 0: {
+            dim3 grid((f.N + 15) / 16, (f.N + 15) / 16, modes);
+            zgemm_modes_ref_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(A),
+                                                         reinterpret_cast<const double2*>(B), P);
+            return cudaGetLastError();
+        }
+        // 48 x 48 CTA tile, 4 warps of 24 x 24, 3 CTAs per SM, 5-deep ring.  Measured alternatives on B200 at N = 225,
+        // L = 128 (331 us): 64 x 48 / 8 warps of 16 x 24 / 2 CTAs 341 us; 48 x 64 / 8 warps of 24 x 16 354 us; 32 x 48 /
+        // 4 warps / 4 CTAs 338 us; 6-deep ring 331 us; 2 CTAs with an 8-deep ring 359 us.
+        case 1: return launch_dmma<Tile<3, 3, 2, 2, 3, 5>>(f, modes, A, B, P, st);
+        default: return cudaErrorInvalidValue;
     }
-    cudaError_t e = zgemm_init();
-    if (e != cudaSuccess) return e;
-    CUtensorMap mapA, mapB;
-    if ((e = encode_operand(&mapA, A, f, modes, BM)) != cudaSuccess) return e;
-    if ((e = encode_operand(&mapB, B, f, modes, BK)) != cudaSuccess) return e;
-    const unsigned grid = (unsigned)(modes * P.tiles_m * P.tiles_n);
-    zgemm_modes_dmma_kernel<<<grid, GEMM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, P);
-    return cudaGetLastError();
 }
 
 }  // namespace nspt
