@@ -12,6 +12,9 @@ from .nspt_oracle import (  # noqa: F401
     series_mul_rows,
     dagger,
     staple,
+    series_exp,
+    exp_bound,
+    force,
     product_bound,
     staple_bound,
     per_order_error,

@@ -10,6 +10,12 @@ What is defined here, with the passage each follows:
       S_mu = U_mu * [ sum_{nu != mu} ( z_mu,nu  U_nu * U_mu^+ * U_nu^+
                                        - z_mu,nu^*  U_nu^+ * U_mu^+ * U_nu ) ]
   left-to-right association, truncation after every product (readings c6, c9).
+* ``series_exp(X)``         -- exp(X) = sum_{m>=0} X^{*m} / m!  of a series with X^(0) = 0, every power a chain of
+  star-products of eq. 2.5 (the link update U <- exp(i eps P) * U of the NSPT integrator,
+  PAPER.md:50-55; readings c15, c17).  The sum stops at m = Ntrunc exactly because
+  X^{*m} starts at g^m.
+* ``force(S, c)``           -- F^(k) = i c [ S^(k) - S^(k)+ - Tr(S^(k) - S^(k)+)/N ], PAPER.md:50 (eq. 2.3),
+  with the coefficient c ("beta" after the paper's time rescaling, reading c10) left to the caller.
 * ``product_bound`` / ``staple_bound`` / ``per_order_error`` -- the error metric of the north
   star: per order k, ||C_test^(k) - C_oracle^(k)||_F / bound_k with
   bound_k = sum_{j<=k} ||A^(j)||_F ||B^(k-j)||_F   (readings c11, c12).
@@ -156,6 +162,56 @@ def staple(U, z):
             X += z[mu, nu] * t1 - np.conj(z[mu, nu]) * t2
         S.append(series_mul(U[mu], X))
     return S
+
+
+def series_exp(X) -> np.ndarray:
+    """exp(X) = sum_{m=0}^{Ntrunc} X^{*m} / m!  for a series with X^(0) = 0 (a non-zero X^(0) is an error).
+
+    Written out as the definition: the powers X^{*m} = X * X^{*(m-1)} are formed one after the other
+    with the star-product of eq. 2.5 and added with weight 1/m!.  X^{*m} has no orders below g^m, so
+    the sum ends at m = Ntrunc with nothing dropped."""
+    X = _as_series(X, "X")
+    n, N, _ = X.shape
+    if np.any(X[0] != 0):
+        raise ValueError("series_exp needs X^(0) = 0")
+    E = np.zeros_like(X)
+    E[0] = np.eye(N)
+    power = E.copy()          # X^{*0} = 1
+    fact = 1.0
+    for m in range(1, n):
+        power = series_mul(X, power)
+        fact *= m
+        E += power / fact
+    return E
+
+
+def exp_bound(X) -> np.ndarray:
+    """Tolerance denominator for series_exp: the scalar series exp(x), x_k = ||X^(k)||_F, which
+    majorises every term of the definition (sub-multiplicativity of the Frobenius norm), plus
+    sqrt(N) at order 0 for the identity."""
+    x = _order_norms(X)
+    n = len(x)
+    e = np.zeros(n)
+    e[0] = 1.0
+    power = e.copy()
+    fact = 1.0
+    for m in range(1, n):
+        power = _scalar_conv(x, power)
+        fact *= m
+        e += power / fact
+    e[0] = np.sqrt(np.asarray(X).shape[1])
+    return e
+
+
+def force(S, c: float) -> np.ndarray:
+    """F^(k) = i c [ S^(k) - S^(k)+ - Tr(S^(k) - S^(k)+)/N 1 ]   (eq. 2.3; c real)."""
+    S = _as_series(S, "S")
+    n, N, _ = S.shape
+    F = np.empty_like(S)
+    for k in range(n):
+        D = S[k] - S[k].conj().T
+        F[k] = 1j * c * (D - (np.trace(D) / N) * np.eye(N))
+    return F
 
 
 # ----------------------------------------------------------------------------- error metric

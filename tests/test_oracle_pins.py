@@ -396,3 +396,147 @@ def test_error_metric_definition():
     D[1] += 1e-6
     err = oracle.per_order_error(D, C, want)
     assert err[0] == 0 and err[2] == 0 and np.isclose(err[1], 3e-6 / want[1])
+
+
+# ----------------------------------------------------------------------------- series exponential and force
+# (the steps on either side of the staple in one NSPT update)
+
+def test_exp_of_log_series_is_one_plus_g():
+    # N = 1: X = log(1+g) = sum_{k>=1} (-1)^(k+1) g^k / k  =>  exp(X) = 1 + g exactly
+    n = 24
+    X = np.zeros((n, 1, 1), dtype=np.complex128)
+    for k in range(1, n):
+        X[k, 0, 0] = (-1.0) ** (k + 1) / k
+    E = oracle.series_exp(X)
+    want = np.zeros(n)
+    want[0] = want[1] = 1.0
+    assert np.abs(E[:, 0, 0] - want).max() < 5e-15
+
+
+def test_exp_of_g_times_scalar_is_taylor_series():
+    n = 16
+    X = np.zeros((n, 1, 1), dtype=np.complex128)
+    X[1, 0, 0] = 0.75 - 0.5j
+    E = oracle.series_exp(X)
+    want = np.array([(0.75 - 0.5j) ** k / math.factorial(k) for k in range(n)])
+    assert np.abs(E[:, 0, 0] - want).max() < 1e-15
+
+
+def test_exp_of_commuting_diagonal_series_matches_scalar_recurrence():
+    # for commuting coefficients E' = X' E holds, i.e. k e_k = sum_j j x_j e_{k-j}: an independent formula
+    rng = np.random.default_rng(70)
+    n, N = 10, 4
+    x = rng.standard_normal((n, N)) + 1j * rng.standard_normal((n, N))
+    x[0] = 0
+    X = np.zeros((n, N, N), dtype=np.complex128)
+    for k in range(n):
+        X[k] = np.diag(x[k])
+    E = oracle.series_exp(X)
+    e = np.zeros((n, N), dtype=np.complex128)
+    e[0] = 1
+    for k in range(1, n):
+        e[k] = sum(j * x[j] * e[k - j] for j in range(1, k + 1)) / k
+    for k in range(n):
+        assert np.abs(E[k] - np.diag(e[k])).max() < 1e-12 * max(1.0, np.abs(e[k]).max())
+
+
+def test_exp_low_orders_noncommuting_by_hand():
+    # X = g A + g^2 B, [A, B] != 0: orders 0..3 of exp(X) written out by hand
+    A = np.array([[0, 1], [2, 0]], dtype=np.complex128)
+    B = np.array([[1, 0], [3, -1j]], dtype=np.complex128)
+    X = np.zeros((4, 2, 2), dtype=np.complex128)
+    X[1], X[2] = A, B
+    E = oracle.series_exp(X)
+    assert np.allclose(E[0], np.eye(2), atol=0)
+    assert np.allclose(E[1], A, atol=1e-15)
+    assert np.allclose(E[2], B + A @ A / 2, atol=1e-15)
+    assert np.allclose(E[3], (A @ B + B @ A) / 2 + A @ A @ A / 6, atol=1e-15)
+    assert not np.allclose(A @ B, B @ A)
+
+
+def test_exp_of_nilpotent_generator_terminates():
+    M = np.array([[0, 3, 1], [0, 0, -2], [0, 0, 0]], dtype=np.complex128)
+    X = np.zeros((6, 3, 3), dtype=np.complex128)
+    X[1] = M
+    E = oracle.series_exp(X)
+    assert np.array_equal(E[0], np.eye(3)) and np.array_equal(E[1], M)
+    assert np.allclose(E[2], M @ M / 2, atol=0) and np.abs(E[3:]).max() == 0
+
+
+def test_exp_inverse_and_unitarity():
+    rng = np.random.default_rng(71)
+    n, N = 9, 5
+    X = np.zeros((n, N, N), dtype=np.complex128)
+    for k in range(1, n):
+        X[k] = 1j * wl.hermitian_traceless(N, rng)       # anti-Hermitian => exp(X) unitary order by order
+    E = oracle.series_exp(X)
+    one = identity_series(N, n - 1)
+    assert np.abs(oracle.series_mul(E, oracle.series_exp(-X)) - one).max() < 1e-13
+    assert np.abs(oracle.series_mul(E, oracle.dagger(E)) - one).max() < 1e-13
+
+
+def test_exp_evaluated_at_numeric_g_matches_matrix_exponential():
+    from scipy.linalg import expm
+    rng = np.random.default_rng(72)
+    n, N, g0 = 14, 4, 0.05
+    X = 0.5 * wl.gaussian_series(N, n - 1, rng)
+    X[0] = 0
+    E = oracle.series_exp(X)
+    Xg = sum(g0 ** k * X[k] for k in range(n))
+    Eg = sum(g0 ** k * E[k] for k in range(n))
+    assert np.abs(Eg - expm(Xg)).max() < 1e-14        # truncation error ~ g0^14
+
+
+def test_exp_agrees_with_the_input_generator():
+    # workloads._input_series_exp is a different arrangement (Horner, stacked products); both must give exp(X)
+    rng = np.random.default_rng(73)
+    n, N = 8, 6
+    X = np.zeros((n, N, N), dtype=np.complex128)
+    for k in range(1, n):
+        X[k] = 1j * wl.hermitian_traceless(N, rng)
+    E = oracle.series_exp(X)
+    assert oracle.per_order_error(wl._input_series_exp(X), E, oracle.exp_bound(X)).max() < 1e-14
+
+
+def test_exp_rejects_zeroth_order():
+    X = np.zeros((3, 2, 2), dtype=np.complex128)
+    X[0, 0, 0] = 1.0
+    with pytest.raises(ValueError):
+        oracle.series_exp(X)
+
+
+def test_force_by_hand_2x2():
+    # S = [[1+2i, 3], [4i, 5-i]]: S - S^+ = [[4i, 3+4i], [-3+4i, -2i]], Tr = 2i, /N = i
+    S = np.zeros((1, 2, 2), dtype=np.complex128)
+    S[0] = [[1 + 2j, 3], [4j, 5 - 1j]]
+    F = oracle.force(S, 2.0)
+    want = 2j * np.array([[4j - 1j, 3 + 4j], [-3 + 4j, -2j - 1j]])
+    assert np.allclose(F[0], want, atol=0)
+
+
+def test_force_is_hermitian_traceless_and_kills_hermitian_input():
+    rng = np.random.default_rng(74)
+    n, N = 5, 7
+    S = wl.gaussian_series(N, n - 1, rng)
+    F = oracle.force(S, 1.7)
+    for k in range(n):
+        assert np.abs(F[k] - F[k].conj().T).max() < 1e-15
+        assert abs(np.trace(F[k])) < 1e-14
+    H = S + np.conj(np.transpose(S, (0, 2, 1)))
+    assert np.abs(oracle.force(H, 3.0)).max() == 0
+    iden = np.zeros((1, N, N), dtype=np.complex128)
+    iden[0] = 1j * np.eye(N)                                # S - S^+ = 2i 1 is pure trace
+    assert np.abs(oracle.force(iden, 1.0)).max() == 0
+
+
+def test_force_matches_scalar_loops():
+    rng = np.random.default_rng(75)
+    n, N, c = 3, 4, -0.6
+    S = wl.gaussian_series(N, n - 1, rng)
+    F = oracle.force(S, c)
+    for k in range(n):
+        tr = sum(complex(S[k, i, i]) - complex(S[k, i, i]).conjugate() for i in range(N))
+        for i in range(N):
+            for j in range(N):
+                d = complex(S[k, i, j]) - complex(S[k, j, i]).conjugate() - (tr / N if i == j else 0)
+                assert abs(F[k, i, j] - 1j * c * d) < 1e-15
