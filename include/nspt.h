@@ -55,7 +55,7 @@ enum {
     NSPT_EARCH = -4    /* current device is not compute capability 10.x */
 };
 
-enum { NSPT_OP_SERIES_MUL = 0, NSPT_OP_STAPLE = 1 };
+enum { NSPT_OP_SERIES_MUL = 0, NSPT_OP_STAPLE = 1, NSPT_OP_SERIES_EXP = 2 };
 
 /* Largest supported truncation order: the transform length L = smallest power of two
  * >= 2*Ntrunc+1 must be <= 256 (Ntrunc <= 127; the paper uses Ntrunc <= 63). */
@@ -94,7 +94,27 @@ int nspt_series_mul_batched(const nspt_c128* A, const nspt_c128* B, nspt_c128* C
 int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4],
                 int N, int Ntrunc);
 
-/* Host-buffer forms of the three calls above: same semantics, HOST pointers for the series,
+/*
+ * E = exp(X) = sum_{m=0}^{Ntrunc} X^{*m} / m!, every power a chain of the star-product above, for a series
+ * whose coefficient of g^0 vanishes; X^(0) is NOT read and is taken as zero (with X^(0) = 0 the power
+ * X^{*m} starts at g^m, so the sum is finite and exact).  This is the exponential of the link update
+ * U <- exp(i eps P) * U of the NSPT integrator ("solved with a symplectic integrator";
+ * U-dot = i P * U, eq. 2.3), and of U = exp(i sum_k g^k H_k).  Ntrunc - 1 star-products (Horner form, X
+ * transformed once, intermediate results kept in frequency space).  Device pointers, (Ntrunc+1)*N*N elements;
+ * E may alias X.
+ */
+int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc);
+
+/*
+ * The force of eq. 2.3 from a staple series, order by order:
+ *     F^(k) = i c [ S^(k) - S^(k)+ - Tr(S^(k) - S^(k)+)/N ],   k = 0..Ntrunc,
+ * Hermitian and traceless.  c is the real coefficient the paper writes as beta; what is left of it after the
+ * paper's rescaling of the fictitious time is not recoverable from the text, so the caller supplies it.
+ * Device pointers, (Ntrunc+1)*N*N elements; F must NOT alias S (NSPT_EINVAL if F == S).
+ */
+int nspt_force(const nspt_c128* S, nspt_c128* F, double c, int N, int Ntrunc);
+
+/* Host-buffer forms of nspt_series_mul, nspt_series_mul_batched and nspt_staple: same semantics, HOST pointers for the series,
  * host<->device copies on the library stream inside the call, stream synchronised on return. */
 int nspt_series_mul_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc);
 int nspt_series_mul_batched_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C,
@@ -114,7 +134,7 @@ int nspt_set_stream(void* cuda_stream);
 int nspt_set_order_scale(double s);
 
 /* Bytes of device workspace a call needs (op = NSPT_OP_SERIES_MUL with its batch, or
- * NSPT_OP_STAPLE, batch ignored). */
+ * NSPT_OP_STAPLE / NSPT_OP_SERIES_EXP, batch ignored).  nspt_force needs none. */
 int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out);
 
 /* Give the library a caller-owned device workspace (256-byte aligned).  Calls that need more

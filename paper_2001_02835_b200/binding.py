@@ -19,11 +19,11 @@ _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libnspt.so"
 
 NSPT_OK, NSPT_EINVAL, NSPT_ENOMEM, NSPT_ECUDA, NSPT_EARCH = 0, -1, -2, -3, -4
-NSPT_OP_SERIES_MUL, NSPT_OP_STAPLE = 0, 1
+NSPT_OP_SERIES_MUL, NSPT_OP_STAPLE, NSPT_OP_SERIES_EXP = 0, 1, 2
 STAGES = {"fft_forward": 0, "zgemm_modes": 1, "fft_inverse": 2, "fft_retruncate": 3, "other": 4}
 
 EXPORTS = [
-    "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple",
+    "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_series_exp", "nspt_force",
     "nspt_series_mul_host", "nspt_series_mul_batched_host", "nspt_staple_host",
     "nspt_set_stream", "nspt_set_order_scale", "nspt_workspace_bytes", "nspt_set_workspace",
     "nspt_set_gemm_variant", "nspt_probe_fp64_peak", "nspt_profile", "nspt_profile_read", "nspt_launch_count",
@@ -47,6 +47,8 @@ _vp, _int, _dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
 _lib.nspt_series_mul.argtypes = [_vp, _vp, _vp, _int, _int]
 _lib.nspt_series_mul_batched.argtypes = [_vp, _vp, _vp, _int, _int, _int]
 _lib.nspt_staple.argtypes = [ctypes.POINTER(_vp), _vp, ctypes.POINTER(_vp), _int, _int]
+_lib.nspt_series_exp.argtypes = [_vp, _vp, _int, _int]
+_lib.nspt_force.argtypes = [_vp, _vp, _dbl, _int, _int]
 _lib.nspt_series_mul_host.argtypes = [_vp, _vp, _vp, _int, _int]
 _lib.nspt_series_mul_batched_host.argtypes = [_vp, _vp, _vp, _int, _int, _int]
 _lib.nspt_staple_host.argtypes = [ctypes.POINTER(_vp), _vp, ctypes.POINTER(_vp), _int, _int]
@@ -158,6 +160,30 @@ def nspt_staple(U, z, S=None):
     Sp = (_vp * 4)(*[s.data_ptr() for s in S])
     _check(_lib.nspt_staple(Up, zz.ctypes.data, Sp, N, Ntrunc), "nspt_staple")
     return S
+
+
+def nspt_series_exp(X, E=None):
+    """E = exp(X) = sum_m X^{*m}/m! for a series with X^(0) = 0 (X^(0) is not read).  Device tensors."""
+    torch = _torch()
+    X = _dev_series(X, "X")
+    _, Ntrunc, N = _shape(X, False)
+    if E is None:
+        E = torch.empty_like(X)
+    _dev_series(E, "E")
+    _check(_lib.nspt_series_exp(X.data_ptr(), E.data_ptr(), N, Ntrunc), "nspt_series_exp")
+    return E
+
+
+def nspt_force(S, c: float, F=None):
+    """F^(k) = i c [S^(k) - S^(k)+ - Tr(S^(k) - S^(k)+)/N] (eq. 2.3).  Device tensors; F must not alias S."""
+    torch = _torch()
+    S = _dev_series(S, "S")
+    _, Ntrunc, N = _shape(S, False)
+    if F is None:
+        F = torch.empty_like(S)
+    _dev_series(F, "F")
+    _check(_lib.nspt_force(S.data_ptr(), F.data_ptr(), float(c), N, Ntrunc), "nspt_force")
+    return F
 
 
 # ------------------------------------------------------------------------------ host calls

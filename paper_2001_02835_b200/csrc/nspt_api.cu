@@ -290,6 +290,64 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
     return NSPT_OK;
 }
 
+// exp(X) = sum_m X^{*m}/m! by Horner in frequency space (reading c17):
+//     T_n = 1 + X/n,   T_m = 1 + (X * T_{m+1})/m  (m = n-1 .. 1),   exp(X) = T_1,     n = Ntrunc,
+// X~ is transformed once; every step is one mode-wise product whose epilogue scales by 1/m and adds the
+// identity series (the unit matrix at every mode), followed by a re-truncation pass (a length-L cyclic
+// transform protects one product only); the last step goes straight to the inverse transform.
+int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc) {
+    NSPT_TRY(check_dims(N, Ntrunc, 1));
+    if (!X || !E || !aligned16(X) || !aligned16(E)) return NSPT_EINVAL;
+    NSPT_TRY(check_arch());
+    const FreqLayout f = make_layout(N, Ntrunc);
+    if (!fft_length_supported(f.L)) return NSPT_EINVAL;
+    PlanTables t;
+    NSPT_TRY(get_plan(f.L, f.n, g.order_scale, &t));
+    char* ws = nullptr;
+    NSPT_TRY(get_workspace(ws_bytes_for(f, 1, NSPT_OP_SERIES_EXP), &ws));
+    const size_t sb = spectrum_bytes(f, 1);
+    double* Xt = reinterpret_cast<double*>(ws);
+    double* Tt = reinterpret_cast<double*>(ws + sb);
+    double* Pt = reinterpret_cast<double*>(ws + 2 * sb);
+    {   // X~ with the coefficient of g^0 taken as zero
+        StageTimer tm;
+        NSPT_TRY(tm.begin(ST_FWD));
+        NSPT_CUDA(launch_fft_forward(f, t, 1, X, Xt, nullptr, nullptr, g.stream, true));
+        NSPT_TRY(tm.end());
+    }
+    const int n = Ntrunc > 0 ? Ntrunc : 1;
+    {   // T_n = 1 + X/n
+        StageTimer tm;
+        NSPT_TRY(tm.begin(ST_OTHER));
+        NSPT_CUDA(launch_freq_scale_identity(f, 1, Xt, Tt, 1.0 / n, g.stream));
+        NSPT_TRY(tm.end());
+    }
+    double* cur = Tt;
+    double* other = Pt;
+    for (int m = n - 1; m >= 1; --m) {
+        GemmOut o;
+        o.C = other;
+        o.alpha = Cplx{1.0 / m, 0.0};
+        o.diag = 1.0;
+        NSPT_TRY(k_gemm(f, 1, Xt, cur, o));
+        if (m > 1) NSPT_TRY(k_retrunc(f, t, 1, other, other));
+        double* tmp = cur;
+        cur = other;
+        other = tmp;
+    }
+    return k_inverse(f, t, 1, cur, E);
+}
+
+int force_device(const nspt_c128* S, nspt_c128* F, double c, int N, int Ntrunc) {
+    NSPT_TRY(check_dims(N, Ntrunc, 1));
+    if (!S || !F || S == F || !aligned16(S) || !aligned16(F) || !std::isfinite(c)) return NSPT_EINVAL;
+    NSPT_TRY(check_arch());
+    StageTimer tm;
+    NSPT_TRY(tm.begin(ST_OTHER));
+    NSPT_CUDA(launch_force(S, F, c, N, Ntrunc + 1, g.stream));
+    return tm.end();
+}
+
 int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4], int N, int Ntrunc) {
     NSPT_TRY(check_dims(N, Ntrunc, 1));
     if (!U || !z || !S) return NSPT_EINVAL;
@@ -387,6 +445,16 @@ int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* c
     return staple_device(U, z, S, N, Ntrunc);
 }
 
+int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    return series_exp_device(X, E, N, Ntrunc);
+}
+
+int nspt_force(const nspt_c128* S, nspt_c128* F, double c, int N, int Ntrunc) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    return force_device(S, F, c, N, Ntrunc);
+}
+
 int nspt_series_mul_batched_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc, int batch) {
     std::lock_guard<std::mutex> lk(g.mu);
     NSPT_TRY(check_dims(N, Ntrunc, batch));
@@ -449,8 +517,8 @@ int nspt_set_order_scale(double s) {
 
 int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out) {
     if (!out) return NSPT_EINVAL;
-    if (op != NSPT_OP_SERIES_MUL && op != NSPT_OP_STAPLE) return NSPT_EINVAL;
-    if (op == NSPT_OP_STAPLE) batch = 1;
+    if (op != NSPT_OP_SERIES_MUL && op != NSPT_OP_STAPLE && op != NSPT_OP_SERIES_EXP) return NSPT_EINVAL;
+    if (op != NSPT_OP_SERIES_MUL) batch = 1;
     NSPT_TRY(check_dims(N, Ntrunc, batch));
     const FreqLayout f = make_layout(N, Ntrunc);
     if (!fft_length_supported(f.L)) return NSPT_EINVAL;

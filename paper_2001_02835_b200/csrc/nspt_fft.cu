@@ -143,6 +143,7 @@ struct XformParams {
     const double* scale_out;
     double inv_L;
     int use_scale;
+    int skip_order0;               // forward only: treat the coefficient of g^0 as zero (series exponential)
 };
 
 // ---- forward phases: registers x[r] = coefficient of order S*r + s (r < R/2 non-zero) -> spectrum.
@@ -273,7 +274,7 @@ __global__ void __launch_bounds__(T) fft_forward_small_kernel(const XformParams 
     for (int r = 0; r < R; ++r) x[r] = make_double2(0.0, 0.0);
 #pragma unroll
     for (int r = 0; r < RH; ++r) {
-        if (valid && r < P.n) {
+        if (valid && r < P.n && !(P.skip_order0 && r == 0)) {
             double2 v = __ldg(&in[(size_t)r * P.NN]);
             if (P.use_scale) {
                 const double sc = __ldg(&P.scale_in[r]);
@@ -413,6 +414,7 @@ __global__ void __launch_bounds__(T* S) fft_forward_tma_kernel(const __grid_cons
                 v.x *= sc;
                 v.y *= sc;
             }
+            if (P.skip_order0 && k == 0) v = make_double2(0.0, 0.0);
             x[r] = v;
         }
 #pragma unroll
@@ -554,6 +556,20 @@ __global__ void __launch_bounds__(256) freq_dagger_kernel(const double2* __restr
     }
 }
 
+// dst(p) = alpha * src(p) + 1 for every mode p: alpha X + (identity series), whose spectrum is the unit matrix
+// at every mode.  First Horner step of the series exponential.
+__global__ void __launch_bounds__(256) freq_scale_identity_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
+                                                                 int N, size_t NN, double alpha) {
+    const size_t e = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (e >= NN) return;
+    const size_t o = (size_t)blockIdx.y * NN + e;
+    double2 v = src[o];
+    v.x *= alpha;
+    v.y *= alpha;
+    if (e / N == e % N) v.x += 1.0;
+    dst[o] = v;
+}
+
 // ------------------------------------------------------------------------------------ host side
 enum Which { W_FWD, W_INV, W_RET };
 
@@ -662,6 +678,7 @@ XformParams base_params(const FreqLayout& f, const PlanTables& t, int batch) {
     P.scale_out = t.scale_out;
     P.inv_L = t.inv_L;
     P.use_scale = 0;
+    P.skip_order0 = 0;
     return P;
 }
 
@@ -670,8 +687,9 @@ XformParams base_params(const FreqLayout& f, const PlanTables& t, int batch) {
 bool fft_length_supported(int L) { return L >= 1 && L <= 256 && (L & (L - 1)) == 0; }
 
 cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int batch, const nspt_c128* src0,
-                               double* dst0, const nspt_c128* src1, double* dst1, cudaStream_t st) {
+                               double* dst0, const nspt_c128* src1, double* dst1, cudaStream_t st, bool skip_order0) {
     XformParams P = base_params(f, t, batch);
+    P.skip_order0 = skip_order0 ? 1 : 0;
     P.src_series[0] = reinterpret_cast<const double2*>(src0);
     P.src_series[1] = reinterpret_cast<const double2*>(src1);
     P.dst_freq[0] = reinterpret_cast<double2*>(dst0);
@@ -700,6 +718,14 @@ cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src
     dim3 grid((f.N + 31) / 32, (f.N + 31) / 32, (unsigned)(batch * f.L));
     freq_dagger_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst), f.N,
                                              f.NN, f.L);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_freq_scale_identity(const FreqLayout& f, int batch, const double* src, double* dst, double alpha,
+                                       cudaStream_t st) {
+    dim3 grid((unsigned)((f.NN + 255) / 256), (unsigned)(batch * f.L));
+    freq_scale_identity_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst),
+                                                     f.N, f.NN, alpha);
     return cudaGetLastError();
 }
 

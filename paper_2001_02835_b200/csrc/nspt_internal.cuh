@@ -57,7 +57,8 @@ struct Cplx { double re, im; };
 // Forward: up to two operands per launch (src1 may be null). series -> spectrum.
 cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int batch,
                                const nspt_c128* src0, double* dst0,
-                               const nspt_c128* src1, double* dst1, cudaStream_t st);
+                               const nspt_c128* src1, double* dst1, cudaStream_t st,
+                               bool skip_order0 = false);
 // Inverse + 1/L + truncation (+ unscale): spectrum -> series.
 cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int batch,
                                const double* src, nspt_c128* dst, cudaStream_t st);
@@ -67,11 +68,18 @@ cudaError_t launch_fft_retruncate(const FreqLayout& f, const PlanTables& t, int 
 // Spectrum of the daggered series: Xd~(p) = (X~((L - p) mod L))^H.
 cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src, double* dst,
                                cudaStream_t st);
+// dst(p) = alpha * src(p) + 1 (unit matrix) for every mode: spectrum of alpha X + identity series.
+cudaError_t launch_freq_scale_identity(const FreqLayout& f, int batch, const double* src, double* dst, double alpha,
+                                       cudaStream_t st);
 bool fft_length_supported(int L);
+
+// ---- force projection (nspt_md.cu) -------------------------------------------------------------
+// F^(k) = i c [ S^(k) - S^(k)+ - Tr(S^(k) - S^(k)+)/N ] for k < n (eq. 2.3).  F must not alias S.
+cudaError_t launch_force(const nspt_c128* S, nspt_c128* F, double c, int N, int n, cudaStream_t st);
 
 // ---- mode-wise matrix product (nspt_zgemm.cu) -----------------------------------------------
 // For all batch*L modes p, with M(p) = A~(p) B~(p):
-//     C(p)             (+)= alpha * M(p)        if C is not null  (accumulate selects +=)
+//     C(p)             (+)= alpha * M(p) + diag*1   if C is not null  (accumulate selects +=)
 //     D((L-p) mod L)   (+)= beta  * M(p)^H      if D is not null  (accumulate_d selects +=)
 // The second form adds the spectrum of the DAGGERED product series, FFT[X^+](p') = (X~((L-p') mod L))^H.
 struct GemmOut {
@@ -81,6 +89,7 @@ struct GemmOut {
     double* D = nullptr;
     Cplx beta{1.0, 0.0};
     bool accumulate_d = false;
+    double diag = 0.0;   // added to the diagonal of C(p) after alpha (the identity series in frequency space)
 };
 cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B,
                                const GemmOut& out, int variant, cudaStream_t st);

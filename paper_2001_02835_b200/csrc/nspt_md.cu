@@ -1,0 +1,64 @@
+// nspt_md.cu -- the force projection that follows the staple in the NSPT update (eq. 2.3):
+//     F^(k) = i c [ S^(k) - S^(k)+ - Tr(S^(k) - S^(k)+)/N ],   k = 0..Ntrunc,
+// per order a traceless-Hermitian projection of the staple coefficient.  HBM-bound (each element of S is read
+// twice, once transposed through shared memory, and F is written once): 48 N^2 bytes per order.
+// With S^(k)_ij = a_ij + i b_ij and t = sum_i b_ii:
+//     F_ij = -c (b_ij + b_ji) + i c (a_ij - a_ji)  +  delta_ij 2 c t / N.
+#include "nspt_internal.cuh"
+
+namespace nspt {
+namespace {
+
+__global__ void __launch_bounds__(256) force_kernel(const double2* __restrict__ S, double2* __restrict__ F, int N, size_t NN,
+                                                   double c) {
+    __shared__ double2 tile[32][33];
+    __shared__ double red[8];
+    const int k = blockIdx.z;
+    const double2* s = S + (size_t)k * NN;
+    double2* f = F + (size_t)k * NN;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;  // 32 x 8
+    const int i0 = blockIdx.y * 32, j0 = blockIdx.x * 32;
+    const bool diag_tile = (i0 == j0);
+    // t = sum_i Im S_ii, needed by the diagonal tiles only (N values, L2-resident)
+    double t = 0.0;
+    if (diag_tile) {
+        for (int i = threadIdx.x; i < N; i += 256) t += s[(size_t)i * N + i].y;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (tx == 0) red[ty] = t;
+    }
+    // transposed tile: tile[r][tx] = S[j0 + r][i0 + tx]
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int j = j0 + r, i = i0 + tx;
+        tile[r][tx] = (j < N && i < N) ? s[(size_t)j * N + i] : make_double2(0.0, 0.0);
+    }
+    __syncthreads();
+    if (diag_tile) {
+        t = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) t += red[w];
+    }
+    const double shift = 2.0 * c * t / (double)N;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int i = i0 + r, j = j0 + tx;
+        if (i < N && j < N) {
+            const double2 a = s[(size_t)i * N + j];  // S_ij
+            const double2 b = tile[tx][r];           // S_ji
+            double2 o = make_double2(-c * (a.y + b.y), c * (a.x - b.x));
+            if (i == j) o.x += shift;
+            f[(size_t)i * N + j] = o;
+        }
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_force(const nspt_c128* S, nspt_c128* F, double c, int N, int n, cudaStream_t st) {
+    dim3 grid((N + 31) / 32, (N + 31) / 32, (unsigned)n);
+    force_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(S), reinterpret_cast<double2*>(F), N, (size_t)N * N, c);
+    return cudaGetLastError();
+}
+
+}  // namespace nspt

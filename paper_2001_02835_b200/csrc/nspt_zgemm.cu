@@ -73,6 +73,7 @@ struct GemmParams {
     double alpha_re, alpha_im;
     double beta_re, beta_im;
     int accumulate, accumulate_d;
+    double diag;   // added to the diagonal of C after alpha
 };
 
 template <class TC>
@@ -246,6 +247,8 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
                     if (Cm) {
                         double2 o0 = make_double2(P.alpha_re * cr0 - P.alpha_im * ci0, P.alpha_re * ci0 + P.alpha_im * cr0);
                         double2 o1 = make_double2(P.alpha_re * cr1 - P.alpha_im * ci1, P.alpha_re * ci1 + P.alpha_im * cr1);
+                        if (m == n) o0.x += P.diag;
+                        if (m == n + 1) o1.x += P.diag;
                         double2* d = Cm + (size_t)m * N + n;
                         if (P.accumulate) {
                             const double2 old0 = d[0];
@@ -305,6 +308,7 @@ zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict_
     }
     if (P.C) {
         double2 out = make_double2(P.alpha_re * cr - P.alpha_im * ci, P.alpha_re * ci + P.alpha_im * cr);
+        if (i == j) out.x += P.diag;
         double2* c = P.C + (size_t)mode * P.NN + (size_t)i * N + j;
         if (P.accumulate) {
             out.x += c->x;
@@ -401,6 +405,7 @@ cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, 
     P.beta_im = out.beta.im;
     P.accumulate = out.accumulate ? 1 : 0;
     P.accumulate_d = out.accumulate_d ? 1 : 0;
+    P.diag = out.diag;
     switch (variant) {
         case 0: {
             dim3 grid((f.N + 15) / 16, (f.N + 15) / 16, modes);

@@ -340,3 +340,117 @@ def test_config5_sweep_points_sampled_rows(nspt, N, Ntrunc):
     d = got[:, rows, :] - ref
     err = np.sqrt((np.abs(d) ** 2).sum(axis=(1, 2))) / bound
     assert err.max() <= TOL, f"{err.max():.3e}"
+
+
+# ----------------------------------------------------------------------------- series exponential and force
+# (SURVEY.md 8f NEXT-1).  Tolerance for exp: per order, 1e-11 of the scalar-series bound exp(||X^(k)||)
+# (oracle.exp_bound), the same normwise criterion as the product's.
+
+def anti_hermitian_series(N, Ntrunc, seed):
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(seed)
+    X = np.zeros((Ntrunc + 1, N, N), dtype=np.complex128)
+    for k in range(1, Ntrunc + 1):
+        X[k] = 1j * wl.hermitian_traceless(N, rng)
+    return X
+
+
+def gpu_exp(nspt, X):
+    import torch
+    E = nspt.nspt_series_exp(to_dev(X))
+    torch.cuda.synchronize()
+    return E.cpu().numpy()
+
+
+@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (1, 1), (1, 9), (3, 2), (9, 7), (25, 15), (57, 9), (50, 20), (33, 31)])
+def test_series_exp_matches_oracle(nspt, N, Ntrunc):
+    import oracle
+    X = anti_hermitian_series(N, Ntrunc, seed=[60, N, Ntrunc])
+    ref = oracle.series_exp(X)
+    got = gpu_exp(nspt, X)
+    err = oracle.per_order_error(got, ref, oracle.exp_bound(X))
+    assert np.isfinite(got).all() and err.max() <= TOL, f"{err.max():.3e}"
+
+
+def test_series_exp_generic_series_and_reference_gemm(nspt):
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    X = 0.3 * wl.gaussian_series(20, 11, np.random.default_rng(61))
+    X[0] = 0
+    ref = oracle.series_exp(X)
+    for variant in (0, 1):
+        nspt.nspt_set_gemm_variant(variant)
+        err = oracle.per_order_error(gpu_exp(nspt, X), ref, oracle.exp_bound(X))
+        assert err.max() <= TOL
+    nspt.nspt_set_gemm_variant(1)
+
+
+def test_series_exp_ignores_zeroth_order_and_may_alias(nspt):
+    import torch
+    import oracle
+    X = anti_hermitian_series(12, 6, seed=62)
+    ref = oracle.series_exp(X)
+    Xd = X.copy()
+    Xd[0] = 7.0 - 3.0j                                  # documented: X^(0) is not read
+    d = to_dev(Xd)
+    nspt.nspt_series_exp(d, d)                          # in place
+    torch.cuda.synchronize()
+    assert oracle.per_order_error(d.cpu().numpy(), ref, oracle.exp_bound(X)).max() <= TOL
+
+
+def test_series_exp_integer_nilpotent_bit_exact(nspt):
+    # X = g M with M strictly upper triangular integers: exp(X) = 1 + g M + g^2 M^2/2 + g^3 M^3/6 exactly
+    M = np.array([[0, 6, 2, -12], [0, 0, -6, 6], [0, 0, 0, 12], [0, 0, 0, 0]], dtype=np.complex128)
+    X = np.zeros((8, 4, 4), dtype=np.complex128)
+    X[1] = M
+    got = gpu_exp(nspt, X)
+    want = np.zeros_like(X)
+    want[0], want[1], want[2], want[3] = np.eye(4), M, M @ M / 2, M @ M @ M / 6
+    assert np.array_equal(np.round(got.real), want.real) and np.array_equal(np.round(got.imag), want.imag)
+    assert np.abs(got - want).max() < 1e-11
+
+
+def test_series_exp_is_unitary_at_config_size(nspt):
+    # N = 225, N_trunc = 31 (configs[1] shape): exp of an anti-Hermitian series is unitary order by order;
+    # checked with the library's own product and sampled rows of the oracle product.
+    import torch
+    import oracle
+    X = anti_hermitian_series(225, 31, seed=63)
+    E = nspt.nspt_series_exp(to_dev(X))
+    Ed = E.conj().transpose(1, 2).contiguous()
+    P = nspt.nspt_series_mul(E, Ed)
+    torch.cuda.synchronize()
+    P = P.cpu().numpy()
+    En = E.cpu().numpy()
+    one = np.zeros_like(P)
+    one[0] = np.eye(225)
+    bound = oracle.product_bound(En, En)
+    assert oracle.per_order_error(P, one, bound).max() <= TOL
+    rows = [0, 100, 224]
+    ref = oracle.series_mul_rows(En, oracle.dagger(En), rows)
+    assert np.abs(ref - one[:, rows, :]).max() < 1e-10
+
+
+@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (2, 3), (31, 4), (32, 1), (33, 2), (225, 7)])
+def test_force_matches_oracle(nspt, N, Ntrunc):
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    S = wl.gaussian_series(N, Ntrunc, np.random.default_rng([64, N, Ntrunc]))
+    c = 1.25
+    F = nspt.nspt_force(to_dev(S), c)
+    torch.cuda.synchronize()
+    got = F.cpu().numpy()
+    ref = oracle.force(S, c)
+    scale = np.sqrt((np.abs(S) ** 2).sum(axis=(1, 2)))
+    err = np.sqrt((np.abs(got - ref) ** 2).sum(axis=(1, 2))) / scale
+    assert err.max() <= 1e-14, f"{err.max():.3e}"
+    # off-diagonal entries involve one addition and one multiplication in the same order: bit-exact
+    off = ~np.eye(N, dtype=bool)
+    assert np.array_equal(got[:, off], ref[:, off])
+
+
+def test_force_rejects_aliasing(nspt):
+    S = to_dev(np.zeros((2, 4, 4), dtype=np.complex128))
+    with pytest.raises(nspt.NsptError):
+        nspt.nspt_force(S, 1.0, S)
