@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- series star-products per second on B200 (BASELINE.json metric), one JSON line.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg2|staple|batched4]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg2|staple|batched4|sweep]
     python bench.py --impl reference ...        # the CPU oracle as the reference arm
 
 A step is one pass of the whole hot path over one synthetic input: for the default workload
@@ -51,6 +51,8 @@ WORKLOADS = {
     "batched4": ("batched", 225, 31, 4, 2),
     "staple": ("staple", 225, 31, 1, 4),
     "small": ("product", 9, 7, 1, 0),
+    "sweep": ("sweep", 225, 31, 1, 5),
+    "exp": ("exp", 225, 31, 1, 6),
 }
 
 
@@ -229,6 +231,130 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------ config 5 sweep
+
+def device_unitary_series(nspt, torch, N, Ntrunc, seed, dev):
+    """U = exp(i sum_{k>=1} g^k H_k), H_k Hermitian traceless with E|H_ij|^2 = 1/N (the config-2 recipe), built on
+    the device: generators from torch's generator, exponential by the library's own nspt_series_exp.  Used for
+    TIMING inputs of the sweep only (the numpy generation costs minutes at N_trunc = 127); the parity of every
+    sweep point is tests/test_gpu_parity.py::test_config5_sweep_points_sampled_rows with numpy-generated inputs."""
+    g = torch.Generator(device=dev)
+    g.manual_seed(int(seed))
+    G = torch.randn(Ntrunc + 1, N, N, dtype=torch.complex128, device=dev, generator=g)   # re, im ~ N(0, 1/2)
+    H = (G + G.conj().transpose(1, 2)) / (2.0 * N) ** 0.5
+    tr = torch.diagonal(H, dim1=1, dim2=2).sum(dim=1) / N
+    H = H - tr[:, None, None] * torch.eye(N, dtype=torch.complex128, device=dev)
+    X = (1j * H).contiguous()
+    X[0] = 0
+    return nspt.nspt_series_exp(X)
+
+
+def run_sweep(args):
+    """BASELINE.json configs[4]: time per product over N_trunc in {7..127} at N = 225 and N in {16..400} at
+    N_trunc = 31, FFT-CONV on the GPU against the naive O(N_trunc^2) convolution (the oracle, host cores)."""
+    import torch
+    rank, local, world = dist_env()
+    if rank != 0:
+        return 0
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    from paper_2001_02835_b200 import build as nspt_build
+    nspt_build.build()
+    from paper_2001_02835_b200 import binding as nspt
+    from paper_2001_02835_b200 import workloads as wl
+    stream = torch.cuda.Stream(device=dev)
+    nspt.nspt_set_stream(stream.cuda_stream)
+    nspt.nspt_set_order_scale(1.0)
+    nspt.nspt_set_gemm_variant(1)
+    fp64_peak = nspt.nspt_probe_fp64_peak()
+    peaks = {}
+    pfile = ROOT / "MEASURED_PEAKS.json"
+    if pfile.exists():
+        try:
+            peaks = json.loads(pfile.read_text())
+        except Exception:
+            peaks = {}
+    hbm = peaks.get("hbm_gbs", 6650.0)
+    W, K = max(3, args.warmup), args.steps
+    points = sorted(set(wl.sweep_points() + [(225, 31)]), key=lambda p: (p[0] != 225, p[0], p[1]))
+    rows_out = []
+    launches0 = nspt.nspt_launch_count()
+    sampler = ClockSampler(local).start()
+    headline = None
+    for (N, Ntrunc) in points:
+        n, L = Ntrunc + 1, transform_length(Ntrunc)
+        per_set = 3 * n * N * N * 16
+        R = max(2, int(np.ceil(2 * L2_BYTES / per_set)))
+        R = min(R, 64)
+        with torch.cuda.stream(stream):
+            A0 = device_unitary_series(nspt, torch, N, Ntrunc, 1000 * N + Ntrunc, dev)
+            B0 = device_unitary_series(nspt, torch, N, Ntrunc, 1000 * N + Ntrunc + 500, dev)
+            sets = [(A0.roll(r, dims=-1).contiguous() if r else A0, B0.roll(r, dims=-2).contiguous() if r else B0,
+                     torch.empty_like(A0)) for r in range(R)]
+            for i in range(W):
+                nspt.nspt_series_mul(*sets[i % R])
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            stream.synchronize()
+            ev0.record(stream)
+            for i in range(K):
+                nspt.nspt_series_mul(*sets[i % R])
+            ev1.record(stream)
+            stream.synchronize()
+            us = ev0.elapsed_time(ev1) / K * 1e3
+            nspt.nspt_profile(True)
+            for name in nspt.STAGES:
+                nspt.nspt_profile_read(name)
+            for i in range(K):
+                nspt.nspt_series_mul(*sets[i % R])
+            st = {name: nspt.nspt_profile_read(name) for name in ("fft_forward", "zgemm_modes", "fft_inverse")}
+            nspt.nspt_profile(False)
+        t_gemm = 8.0 * N ** 3 * L / (fp64_peak * 1e12)
+        t_fft = 9.0 * n * N * N * 16 / (hbm * 1e9)
+        row = {"N": N, "N_trunc": Ntrunc, "L": L, "us_per_product": us, "products_per_s": 1e6 / us,
+               "fft_forward_us": st["fft_forward"][0] / K * 1e3, "zgemm_modes_us": st["zgemm_modes"][0] / K * 1e3,
+               "fft_inverse_us": st["fft_inverse"][0] / K * 1e3,
+               "fftconv_roofline_us": max(t_gemm, t_fft) * 1e6, "bound": "fp64" if t_gemm >= t_fft else "hbm",
+               "fftconv_roofline_frac": max(t_gemm, t_fft) * 1e6 / us, "buffer_sets": R}
+        if not args.no_cpu_baseline:
+            import oracle
+            A = A0.cpu().numpy()
+            B = B0.cpu().numpy()
+            # naive O(N_trunc^2) convolution (eq. 2.5) on the host cores: a row sample sized for ~1 s, scaled to a product
+            flops = 8.0 * N ** 3 * n * (n + 1) / 2
+            nrows = int(max(1, min(N, round(N * 30e9 / flops))))
+            rows = np.linspace(0, N - 1, nrows).astype(np.int32)
+            t0 = time.perf_counter()
+            ref = oracle.series_mul_rows(A, B, rows)
+            dt = (time.perf_counter() - t0) * N / nrows
+            with torch.cuda.stream(stream):
+                C = nspt.nspt_series_mul(A0, B0)
+            stream.synchronize()
+            got = C[:, torch.from_numpy(rows.astype(np.int64)).to(dev), :].cpu().numpy()
+            bound = oracle.product_bound(A, B) * np.sqrt(nrows / N)
+            err = (np.sqrt((np.abs(got - ref) ** 2).sum(axis=(1, 2))) / bound).max()
+            row.update({"naive_oracle_s_per_product": dt, "naive_rows_sampled": nrows, "cores": oracle.num_threads(),
+                        "fftconv_gpu_vs_naive_cpu": dt / (us * 1e-6), "parity_sampled_rows_err_over_bound": float(err)})
+        rows_out.append(row)
+        if (N, Ntrunc) == (225, 31):
+            headline = row
+        del sets, A0, B0
+        torch.cuda.empty_cache()
+    clocks = sampler.stop()
+    line = {
+        "metric": METRIC, "value": headline["products_per_s"], "unit": "products/s", "n_gpus": 1, "steps": K, "warmup": W,
+        "ms_per_step": headline["us_per_product"] * 1e-3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "scaling sweep of A*B (BASELINE.json configs[4]): N_trunc in {7,15,31,63,127} at N=225 and N in "
+                               "{16,49,100,225,400} at N_trunc=31; value is the shared point N=225, N_trunc=31; timing inputs are "
+                               "unitary series generated on the device with nspt_series_exp",
+                   "l2": "each point rotates over buffer sets larger than 2 x L2 (up to 64 sets)"},
+        "clocks": clocks, "gpu_launches": nspt.nspt_launch_count() - launches0,
+        "fp64_peak_tflops": fp64_peak, "hbm_peak_GB_s": hbm, "sweep": rows_out,
+    }
+    print(json.dumps(line))
+    return 0
+
+
 # ------------------------------------------------------------------------------------ CUDA arm
 
 def run_cuda(args):
@@ -249,7 +375,7 @@ def run_cuda(args):
     kind, N, Ntrunc, batch, seed = WORKLOADS[args.workload]
     L = transform_length(Ntrunc)
     n = Ntrunc + 1
-    inp = make_inputs(kind, N, Ntrunc, batch, seed)
+    inp = make_inputs(kind, N, Ntrunc, batch, seed) if kind != "exp" else {}
 
     stream = torch.cuda.Stream(device=dev)
     nspt.nspt_set_stream(stream.cuda_stream)
@@ -258,7 +384,26 @@ def run_cuda(args):
 
     series_bytes = n * N * N * 16 * batch
     with torch.cuda.stream(stream):
-        if kind == "staple":
+        if kind == "exp":
+            # series exponential of an anti-Hermitian series (the link-update exponential)
+            per_set = 2 * series_bytes
+            R = max(2, int(np.ceil(2 * L2_BYTES / per_set)))
+            gen = torch.Generator(device=dev)
+            gen.manual_seed(seed)
+            sets = []
+            for r in range(R):
+                G = torch.randn(n, N, N, dtype=torch.complex128, device=dev, generator=gen)
+                H = (G + G.conj().transpose(1, 2)) / (2.0 * N) ** 0.5
+                X = (1j * H).contiguous()
+                X[0] = 0
+                sets.append((X, torch.empty_like(X)))
+
+            def step(i):
+                X, E = sets[i % R]
+                nspt.nspt_series_exp(X, E)
+            products_per_step = max(Ntrunc - 1, 0)
+            units_name = "exponentials"
+        elif kind == "staple":
             per_set = 8 * series_bytes
             R = max(2, int(np.ceil(2 * L2_BYTES / per_set)))
             U0 = [torch.from_numpy(u).to(dev) for u in inp["U"]]
@@ -321,7 +466,7 @@ def run_cuda(args):
     ms_local = ev0.elapsed_time(ev1)
     launches = nspt.nspt_launch_count() - launches0
     clocks = sampler.stop()
-    value, ms_total = aggregate_throughput(K * (products_per_step if kind != "staple" else 1), ms_local, world, dev)
+    value, ms_total = aggregate_throughput(K * (products_per_step if kind not in ("staple", "exp") else 1), ms_local, world, dev)
 
     # ---- timed region 2: the same K steps with the stage profiler on -> per-kernel durations
     nspt.nspt_profile(True)
@@ -342,7 +487,10 @@ def run_cuda(args):
         fp64_peak = nspt.nspt_probe_fp64_peak()
         gemm = stage_ms.get("zgemm_modes")
         flops_per_launch = 8.0 * N ** 3 * L * batch
-        achieved = flops_per_launch / (gemm["ms_per_launch"] * 1e-3) * 1e-12 if gemm else None
+        # a launch may carry several independent products (staple): flops of all mode-wise products of a step
+        # over the summed duration of the step's GEMM launches
+        gemm_products_per_step = products_per_step if kind in ("staple", "exp") else 1
+        achieved = (gemm_products_per_step * flops_per_launch * K / (gemm["ms_total"] * 1e-3) * 1e-12) if gemm else None
         traffic = read_traffic(args.workload, "zgemm_modes")
         peaks = {}
         pfile = ROOT / "MEASURED_PEAKS.json"
@@ -354,9 +502,9 @@ def run_cuda(args):
         hbm = peaks.get("hbm_gbs", 6650.0)
         hbm_src = "MEASURED_PEAKS.json" if "hbm_gbs" in peaks else "fallback 6.65 TB/s"
         fft_bytes = {  # algorithmic bytes per launch
-            "fft_forward": 2 * (n + L) * N * N * 16 * batch,      # two operands: read n*e, write L*e each
+            "fft_forward": (1 if kind == "exp" else 2) * (n + L) * N * N * 16 * batch,      # per operand: read n*e, write L*e
             "fft_inverse": (L + n) * N * N * 16 * batch,
-            "fft_retruncate": 2 * L * N * N * 16,
+            "fft_retruncate": 2 * L * N * N * 16 * (9 if kind == "staple" else 1),   # staple: 18 spectra in 2 launches
         }
         stages_out = {}
         for name, st in stage_ms.items():
@@ -372,12 +520,19 @@ def run_cuda(args):
             "bound": "tensor", "kernel": "zgemm_modes_dmma_kernel (FP64 tensor pipe, DMMA.8x8x4)",
             "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
             "frac": (achieved / fp64_peak) if achieved else None, "traffic": traffic,
-            "flops_basis": "conventional 8*N^3*L per launch; the kernel executes 6*N^3*L (3-multiplication complex product)",
+            "flops_basis": "conventional 8*N^3*L per mode-wise product (all products of a step / summed GEMM launch time); the kernel executes 6*N^3*L (3-multiplication complex product)",
             "achieved_executed": (achieved * 0.75) if achieved else None,
             "peak_source": "nspt_probe_fp64_peak: DMMA m8n8k4 chain, measured in this run (MEASURED_PEAKS.json has no FP64 entry)",
             "hbm_peak_GB_s": hbm, "hbm_peak_source": hbm_src,
         }
-        if kind != "staple":
+        if kind == "exp":
+            step_s = ms_local / K * 1e-3
+            line_extra["exp_roofline"] = {
+                "definition": "N_trunc-1 mode-wise products (Horner form of sum_m X^m/m!) of 8*N^3*L flops each at FP64 peak",
+                "t_roof_ms": products_per_step * t_gemm_roof * 1e3, "products_executed": products_per_step,
+                "frac": products_per_step * t_gemm_roof / step_s if step_s else None,
+            }
+        elif kind != "staple":
             step_s = ms_local / K * 1e-3
             line_extra["fftconv_roofline"] = {
                 "definition": "slower of 8*N^3*L flops at FP64 peak and 9*n*16*N^2 bytes at HBM peak (SURVEY.md 8d)",
@@ -431,7 +586,7 @@ def run_cuda(args):
 
     # ---- CPU baseline: the oracle on this box's cores (rank 0, single-GPU runs only)
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and kind != "exp":
         import oracle
         if kind == "staple":
             # one of the 52 products of the literal staple, scaled
@@ -469,9 +624,10 @@ def run_cuda(args):
         "batched4": "batch of 4 star-products, N=225, N_trunc=31 (the four P_mu*U_mu of a link update)",
         "staple": "full TEK staple S_mu, mu=1..4, N=225, N_trunc=31, k=4 twist (BASELINE.json configs[3]); 36 mode-wise products per step (literal eq. 2.3: 52)",
         "small": "single star-product A*B, N=9, N_trunc=7 (BASELINE.json configs[0])",
+        "exp": "series exponential exp(X), X anti-Hermitian series, N=225, N_trunc=31 (link-update exponential; 30 mode-wise products)",
     }[args.workload]
     line = {
-        "metric": METRIC if kind != "staple" else "tek_staples_per_sec",
+        "metric": {"staple": "tek_staples_per_sec", "exp": "series_exponentials_per_sec"}.get(kind, METRIC),
         "value": value, "unit": f"{units_name}/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
@@ -500,7 +656,11 @@ def main():
         args.steps = args.steps if args.steps is not None else 5
         args.warmup = args.warmup if args.warmup is not None else 1
         return run_reference(args)
-    args.steps = args.steps if args.steps is not None else (200 if args.workload != "staple" else 10)
+    if args.workload == "sweep":
+        args.steps = args.steps if args.steps is not None else 50
+        args.warmup = args.warmup if args.warmup is not None else 3
+        return run_sweep(args)
+    args.steps = args.steps if args.steps is not None else (200 if args.workload not in ("staple", "exp") else 10)
     args.warmup = args.warmup if args.warmup is not None else 5
     return run_cuda(args)
 

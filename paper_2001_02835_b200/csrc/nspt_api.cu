@@ -134,10 +134,12 @@ int get_plan(int L, int n, double s, PlanTables* out) {
 // ---- workspace -----------------------------------------------------------------------------
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-size_t spectrum_bytes(const FreqLayout& f, int batch) { return align_up(f.spectrum_doubles(batch) * 8, 1024); }
+// Spectra are packed back to back (a whole number of N x N matrices apart) so that one tensor map can address
+// several of them by mode offset; 16-byte alignment is all the TMA maps need.
+size_t spectrum_bytes(const FreqLayout& f, int batch) { return f.spectrum_doubles(batch) * 8; }
 
 size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
-    if (op == NSPT_OP_STAPLE) return 15 * spectrum_bytes(f, 1);
+    if (op == NSPT_OP_STAPLE) return 30 * spectrum_bytes(f, 1);
     return 3 * spectrum_bytes(f, batch);
 }
 
@@ -260,6 +262,12 @@ int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, con
     NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, out, g.gemm_variant, g.stream));
     return tm.end();
 }
+int k_gemm_groups(const FreqLayout& f, const GemmGroup* groups, int ngroups) {
+    StageTimer tm;
+    NSPT_TRY(tm.begin(ST_GEMM));
+    NSPT_CUDA(launch_zgemm_groups(f, 1, groups, ngroups, g.gemm_variant, g.stream));
+    return tm.end();
+}
 int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, double* C) {
     GemmOut out;
     out.C = C;
@@ -365,9 +373,20 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     double* Ut[4] = {spec(0), spec(1), spec(2), spec(3)};      // U~_mu
     double* Ud[4] = {spec(4), spec(5), spec(6), spec(7)};      // spectrum of U_mu^+
     double* St[4] = {spec(8), spec(9), spec(10), spec(11)};    // S~_mu, accumulated in frequency space
-    double* W = spec(12);                                      // U_mu * U_nu^+
-    double* Y = spec(13);                                      // U_mu^+ * U_nu
-    double* T = spec(14);                                      // U_nu * W
+    // per unordered pair p = (mu < nu): W_p = U_mu * U_nu^+, Y_p = U_mu^+ * U_nu, T_p = U_nu * W_p
+    double* W[6];
+    double* Y[6];
+    double* T[6];
+    int pmu[6], pnu[6], np = 0;
+    for (int mu = 0; mu < 4; ++mu)
+        for (int nu = mu + 1; nu < 4; ++nu) {
+            pmu[np] = mu;
+            pnu[np] = nu;
+            W[np] = spec(12 + np);
+            Y[np] = spec(18 + np);
+            T[np] = spec(24 + np);
+            ++np;
+        }
     // Eq. 2.3 with U_mu distributed over the sum (the truncated series form a ring, so this is exact):
     //     S_mu = sum_{nu != mu} ( z_{mu nu} P_{mu nu} - z_{mu nu}^* R_{mu nu} ),
     //     P_{mu nu} = U_mu U_nu U_mu^+ U_nu^+,     R_{mu nu} = U_mu U_nu^+ U_mu^+ U_nu       (all products are *).
@@ -376,48 +395,70 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     // Six mode-wise products per pair, 36 in all (the literal form needs 52).  The daggers of PRODUCTS are
     // taken by the GEMM epilogue (conjugate-transposed accumulate into the mirrored mode), the sums over
     // nu are accumulated in frequency space, and each S_mu is inverse-transformed once.
+    // Products that do not depend on one another share a launch (8 launches for the 36 products): a single
+    // product at L = 64 is 3.6 waves of CTAs and loses a tenth of its time to the last, partly filled wave.
     // All four links are transformed before any output is written (S may alias U).
     NSPT_TRY(k_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1]));
     NSPT_TRY(k_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3]));
-    for (int mu = 0; mu < 4; ++mu) NSPT_TRY(k_dagger(f, 1, Ut[mu], Ud[mu]));
+    NSPT_TRY(k_dagger(f, 4, Ut[0], Ud[0]));
+    {   // W_p and Y_p for the six pairs: twelve products, one launch; then one re-truncation pass over all twelve
+        GemmGroup gr[12];
+        for (int p = 0; p < 6; ++p) {
+            gr[p].A = Ut[pmu[p]];
+            gr[p].B = Ud[pnu[p]];
+            gr[p].out.C = W[p];
+            gr[6 + p].A = Ud[pmu[p]];
+            gr[6 + p].B = Ut[pnu[p]];
+            gr[6 + p].out.C = Y[p];
+        }
+        NSPT_TRY(k_gemm_groups(f, gr, 12));
+        NSPT_TRY(k_retrunc(f, t, 12, W[0], W[0]));   // W[0..5], Y[0..5] are contiguous
+    }
+    {   // T_p = U_nu W_p: six products, one launch, one re-truncation pass
+        GemmGroup gr[6];
+        for (int p = 0; p < 6; ++p) {
+            gr[p].A = Ut[pnu[p]];
+            gr[p].B = W[p];
+            gr[p].out.C = T[p];
+        }
+        NSPT_TRY(k_gemm_groups(f, gr, 6));
+        NSPT_TRY(k_retrunc(f, t, 6, T[0], T[0]));
+    }
+    // Accumulation into S~: three rounds, each a perfect matching of the four directions, so that the products of
+    // one launch write different S~_mu.  Round r: pairs (0, r+1) and the complementary pair.
     bool touched[4] = {false, false, false, false};
-    for (int mu = 0; mu < 4; ++mu) {
-        for (int nu = mu + 1; nu < 4; ++nu) {
+    const int match[3][2] = {{0, 5}, {1, 4}, {2, 3}};   // pair indices: (0,1)+(2,3), (0,2)+(1,3), (0,3)+(1,2)
+    for (int r = 0; r < 3; ++r) {
+        GemmGroup ga[4], gb[2];
+        for (int q = 0; q < 2; ++q) {
+            const int p = match[r][q], mu = pmu[p], nu = pnu[p];
             const Cplx zmn{z[4 * mu + nu].re, z[4 * mu + nu].im};
             const Cplx znm{z[4 * nu + mu].re, z[4 * nu + mu].im};
-            NSPT_TRY(k_gemm(f, 1, Ut[mu], Ud[nu], W));
-            NSPT_TRY(k_retrunc(f, t, 1, W, W));
-            NSPT_TRY(k_gemm(f, 1, Ud[mu], Ut[nu], Y));
-            NSPT_TRY(k_retrunc(f, t, 1, Y, Y));
-            {   // S_mu -= z_{mu nu}^* R_{mu nu},  R_{mu nu} = W Y
-                GemmOut o;
-                o.C = St[mu];
-                o.alpha = Cplx{-zmn.re, zmn.im};
-                o.accumulate = touched[mu];
-                NSPT_TRY(k_gemm(f, 1, W, Y, o));
-                touched[mu] = true;
-            }
-            {   // S_nu -= z_{nu mu}^* R_{nu mu},  R_{nu mu} = (Y W)^+
-                GemmOut o;
-                o.D = St[nu];
-                o.beta = Cplx{-znm.re, znm.im};
-                o.accumulate_d = touched[nu];
-                NSPT_TRY(k_gemm(f, 1, Y, W, o));
-                touched[nu] = true;
-            }
-            NSPT_TRY(k_gemm(f, 1, Ut[nu], W, T));
-            NSPT_TRY(k_retrunc(f, t, 1, T, T));
-            {   // S_nu += z_{nu mu} P_{nu mu},  S_mu += z_{mu nu} P_{nu mu}^+,  P_{nu mu} = T U_mu^+
-                GemmOut o;
-                o.C = St[nu];
-                o.alpha = znm;
-                o.accumulate = true;
-                o.D = St[mu];
-                o.beta = zmn;
-                o.accumulate_d = true;
-                NSPT_TRY(k_gemm(f, 1, T, Ud[mu], o));
-            }
+            // S_mu -= z_{mu nu}^* R_{mu nu},  R_{mu nu} = W Y
+            ga[2 * q].A = W[p];
+            ga[2 * q].B = Y[p];
+            ga[2 * q].out.C = St[mu];
+            ga[2 * q].out.alpha = Cplx{-zmn.re, zmn.im};
+            ga[2 * q].out.accumulate = touched[mu];
+            // S_nu -= z_{nu mu}^* R_{nu mu},  R_{nu mu} = (Y W)^+
+            ga[2 * q + 1].A = Y[p];
+            ga[2 * q + 1].B = W[p];
+            ga[2 * q + 1].out.D = St[nu];
+            ga[2 * q + 1].out.beta = Cplx{-znm.re, znm.im};
+            ga[2 * q + 1].out.accumulate_d = touched[nu];
+            // S_nu += z_{nu mu} P_{nu mu},  S_mu += z_{mu nu} P_{nu mu}^+,  P_{nu mu} = T U_mu^+
+            gb[q].A = T[p];
+            gb[q].B = Ud[mu];
+            gb[q].out.C = St[nu];
+            gb[q].out.alpha = znm;
+            gb[q].out.accumulate = true;
+            gb[q].out.D = St[mu];
+            gb[q].out.beta = zmn;
+            gb[q].out.accumulate_d = true;
         }
+        NSPT_TRY(k_gemm_groups(f, ga, 4));
+        for (int q = 0; q < 2; ++q) touched[pmu[match[r][q]]] = touched[pnu[match[r][q]]] = true;
+        NSPT_TRY(k_gemm_groups(f, gb, 2));
     }
     for (int mu = 0; mu < 4; ++mu) NSPT_TRY(k_inverse(f, t, 1, St[mu], S[mu]));
     return NSPT_OK;

@@ -93,6 +93,15 @@ struct GemmOut {
 };
 cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B,
                                const GemmOut& out, int variant, cudaStream_t st);
+// Up to 12 independent products of the same shape in ONE launch (their outputs must not overlap).  The operands
+// of all groups must lie a whole number of N x N matrices apart (spectra of one workspace do).
+struct GemmGroup {
+    const double* A = nullptr;
+    const double* B = nullptr;
+    GemmOut out;
+};
+cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup* groups, int ngroups, int variant,
+                                cudaStream_t st);
 cudaError_t zgemm_init();   // resolves the driver entry point for tensor maps
 
 }  // namespace nspt

@@ -64,32 +64,44 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
         : "d"(a), "d"(b));
 }
 
-struct GemmParams {
-    double2* C;   // direct target:   C(p)            (+)= alpha * A(p) B(p)          (may be null)
+// One product of a launch: modes [aoff, aoff + nmodes) of the A tensor map times modes [boff, ...) of the B map.
+struct GemmGroupDev {
+    double2* C;   // direct target:   C(p)            (+)= alpha * A(p) B(p) + diag   (may be null)
     double2* D;   // daggered target: D((L-p) mod L)  (+)= beta * (A(p) B(p))^H       (may be null)
+    int aoff, boff;
+    double alpha_re, alpha_im;
+    double beta_re, beta_im;
+    double diag;   // added to the diagonal of C after alpha
+    int accumulate, accumulate_d;
+};
+constexpr int MAX_GROUPS = 12;
+
+// Independent products of the same shape share one launch (the staple has up to twelve at a time): the grid is
+// ngroups x nmodes x tiles, so a launch of g products has g times the waves and 1/g of the tail of a single one.
+struct GemmParams {
     size_t NN;
     int N, L;
     int tiles_m, tiles_n;
-    double alpha_re, alpha_im;
-    double beta_re, beta_im;
-    int accumulate, accumulate_d;
-    double diag;   // added to the diagonal of C after alpha
+    int nmodes;    // modes per group (batch * L)
+    int ngroups;
+    GemmGroupDev g[MAX_GROUPS];
 };
 
 template <class TC>
 __device__ __forceinline__ void issue_slice(const CUtensorMap* mapA, const CUtensorMap* mapB, uint32_t stage_addr,
-                                            uint32_t full_bar, int k0, int m0, int n0, int mode) {
+                                            uint32_t full_bar, int k0, int m0, int n0, int modeA, int modeB) {
     mbar_expect_tx(full_bar, TC::STAGE_BYTES);
-    tma_load_3d(stage_addr, mapA, full_bar, 2 * k0, m0, mode);
+    tma_load_3d(stage_addr, mapA, full_bar, 2 * k0, m0, modeA);
 #pragma unroll
     for (int c = 0; c < TC::BN / 8; ++c)
-        tma_load_3d(stage_addr + TC::A_STAGE_BYTES + c * B_BOX_BYTES, mapB, full_bar, 2 * (n0 + 8 * c), k0, mode);
+        tma_load_3d(stage_addr + TC::A_STAGE_BYTES + c * B_BOX_BYTES, mapB, full_bar, 2 * (n0 + 8 * c), k0, modeB);
 }
 
 template <class TC, bool FULL>
 __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUtensorMap& mapB, const GemmParams& P,
                                               uint32_t base, const uint8_t* sgen, uint32_t bar_full, uint32_t bar_empty,
-                                              int warp, int lane, int nk, int m0, int n0, int mode, int nbm, int nbn,
+                                              int warp, int lane, int nk, int m0, int n0, int modeA, int modeB, int nbm,
+                                              int nbn,
                                               uint32_t offA0, uint32_t offA1, uint32_t offB0, uint32_t offB1,
                                               double (&p1)[TC::MB][TC::NB][2], double (&p2)[TC::MB][TC::NB][2],
                                               double (&p3)[TC::MB][TC::NB][2]) {
@@ -145,7 +157,8 @@ __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUt
             if (j + STAGES < nk && lane == 0) {
                 const int sl = j % STAGES;
                 mbar_wait(bar_empty + 8 * sl, (j / STAGES) & 1);
-                issue_slice<TC>(&mapA, &mapB, base + sl * STAGE_BYTES, bar_full + 8 * sl, (j + STAGES) * BK, m0, n0, mode);
+                issue_slice<TC>(&mapA, &mapB, base + sl * STAGE_BYTES, bar_full + 8 * sl, (j + STAGES) * BK, m0, n0, modeA,
+                                modeB);
             }
             __syncwarp();
         }
@@ -166,11 +179,15 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tiles = P.tiles_m * P.tiles_n;
-    const int mode = blockIdx.x / tiles;
-    const int tile = blockIdx.x % tiles;
+    const int grp = blockIdx.x / (tiles * P.nmodes);
+    const int rest = blockIdx.x % (tiles * P.nmodes);
+    const int mode = rest / tiles;    // mode inside the group
+    const int tile = rest % tiles;
     const int m0 = (tile / P.tiles_n) * BM, n0 = (tile % P.tiles_n) * BN;
     const int N = P.N;
     const int nk = (N + BK - 1) / BK;
+    const GemmGroupDev& G = P.g[grp];
+    const int modeA = G.aoff + mode, modeB = G.boff + mode;
 
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -181,7 +198,7 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
         mbar_fence_init();
         const int pre = nk < STAGES ? nk : STAGES;
         for (int it = 0; it < pre; ++it)
-            issue_slice<TC>(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, it * BK, m0, n0, mode);
+            issue_slice<TC>(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, it * BK, m0, n0, modeA, modeB);
     }
     __syncthreads();
 
@@ -219,18 +236,21 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
     // Warps whose MB x NB blocks all intersect the matrix (all but those on the last tile row / column) run
     // an unpredicated copy of the loop: predicated mma.sync costs a WARPSYNC and issue bubbles per group.
     if (nbm == MB && nbn == NB)
-        gemm_mainloop<TC, true>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, mode, MB, NB, offA0,
-                                offA1, offB0, offB1, p1, p2, p3);
+        gemm_mainloop<TC, true>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, modeA, modeB, MB, NB,
+                                offA0, offA1, offB0, offB1, p1, p2, p3);
     else
-        gemm_mainloop<TC, false>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, mode, nbm, nbn,
-                                 offA0, offA1, offB0, offB1, p1, p2, p3);
+        gemm_mainloop<TC, false>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, modeA, modeB, nbm,
+                                 nbn, offA0, offA1, offB0, offB1, p1, p2, p3);
 
     if (!active) return;
     // ---------------------------------------------------------------- epilogue
-    double2* Cm = P.C ? P.C + (size_t)mode * P.NN : nullptr;
+    double2* Cm = G.C ? G.C + (size_t)mode * P.NN : nullptr;
     // spectrum of the daggered series: FFT[X^+](p') = (X~(p))^H with p' = (L - p) mod L, same batch element
     const int pm = mode % P.L;
-    double2* Dm = P.D ? P.D + (size_t)(mode - pm + ((P.L - pm) % P.L)) * P.NN : nullptr;
+    double2* Dm = G.D ? G.D + (size_t)(mode - pm + ((P.L - pm) % P.L)) * P.NN : nullptr;
+    const double alpha_re = G.alpha_re, alpha_im = G.alpha_im, beta_re = G.beta_re, beta_im = G.beta_im;
+    const int accumulate = G.accumulate, accumulate_d = G.accumulate_d;
+    const double diag = G.diag;
 #pragma unroll
     for (int bm = 0; bm < MB; ++bm) {
         const int m = m0 + mw + 8 * bm + g;
@@ -245,12 +265,12 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
                     const double ci1 = p3[bm][bn][1] - p1[bm][bn][1] - p2[bm][bn][1];
                     const bool second = (n + 1 < N);
                     if (Cm) {
-                        double2 o0 = make_double2(P.alpha_re * cr0 - P.alpha_im * ci0, P.alpha_re * ci0 + P.alpha_im * cr0);
-                        double2 o1 = make_double2(P.alpha_re * cr1 - P.alpha_im * ci1, P.alpha_re * ci1 + P.alpha_im * cr1);
-                        if (m == n) o0.x += P.diag;
-                        if (m == n + 1) o1.x += P.diag;
+                        double2 o0 = make_double2(alpha_re * cr0 - alpha_im * ci0, alpha_re * ci0 + alpha_im * cr0);
+                        double2 o1 = make_double2(alpha_re * cr1 - alpha_im * ci1, alpha_re * ci1 + alpha_im * cr1);
+                        if (m == n) o0.x += diag;
+                        if (m == n + 1) o1.x += diag;
                         double2* d = Cm + (size_t)m * N + n;
-                        if (P.accumulate) {
+                        if (accumulate) {
                             const double2 old0 = d[0];
                             o0.x += old0.x;
                             o0.y += old0.y;
@@ -265,11 +285,11 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
                     }
                     if (Dm) {
                         // beta * conj(c): the eight lanes g = 0..7 of a quarter-warp write 128 contiguous bytes
-                        double2 o0 = make_double2(P.beta_re * cr0 + P.beta_im * ci0, P.beta_im * cr0 - P.beta_re * ci0);
-                        double2 o1 = make_double2(P.beta_re * cr1 + P.beta_im * ci1, P.beta_im * cr1 - P.beta_re * ci1);
+                        double2 o0 = make_double2(beta_re * cr0 + beta_im * ci0, beta_im * cr0 - beta_re * ci0);
+                        double2 o1 = make_double2(beta_re * cr1 + beta_im * ci1, beta_im * cr1 - beta_re * ci1);
                         double2* d0 = Dm + (size_t)n * N + m;
                         double2* d1 = d0 + N;
-                        if (P.accumulate_d) {
+                        if (accumulate_d) {
                             const double2 old0 = *d0;
                             o0.x += old0.x;
                             o0.y += old0.y;
@@ -291,14 +311,14 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
 // Reference kernel (variant 0): one thread per output element, conventional 4-multiplication
 // complex product with plain FMAs.  For debugging the tensor-core kernel; never the default.
 __global__ void __launch_bounds__(256)
-zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict__ B, const GemmParams P) {
+zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict__ B, const GemmGroupDev G, int N, size_t NN,
+                       int L) {
     const int mode = blockIdx.z;
     const int j = blockIdx.x * 16 + (threadIdx.x & 15);
     const int i = blockIdx.y * 16 + (threadIdx.x >> 4);
-    const int N = P.N;
     if (i >= N || j >= N) return;
-    const double2* Am = A + (size_t)mode * P.NN;
-    const double2* Bm = B + (size_t)mode * P.NN;
+    const double2* Am = A + (size_t)mode * NN;
+    const double2* Bm = B + (size_t)mode * NN;
     double cr = 0.0, ci = 0.0;
     for (int k = 0; k < N; ++k) {
         const double2 a = Am[(size_t)i * N + k];
@@ -306,21 +326,21 @@ zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict_
         cr += a.x * b.x - a.y * b.y;
         ci += a.x * b.y + a.y * b.x;
     }
-    if (P.C) {
-        double2 out = make_double2(P.alpha_re * cr - P.alpha_im * ci, P.alpha_re * ci + P.alpha_im * cr);
-        if (i == j) out.x += P.diag;
-        double2* c = P.C + (size_t)mode * P.NN + (size_t)i * N + j;
-        if (P.accumulate) {
+    if (G.C) {
+        double2 out = make_double2(G.alpha_re * cr - G.alpha_im * ci, G.alpha_re * ci + G.alpha_im * cr);
+        if (i == j) out.x += G.diag;
+        double2* c = G.C + (size_t)mode * NN + (size_t)i * N + j;
+        if (G.accumulate) {
             out.x += c->x;
             out.y += c->y;
         }
         *c = out;
     }
-    if (P.D) {
-        const int pm = mode % P.L;
-        double2 out = make_double2(P.beta_re * cr + P.beta_im * ci, P.beta_im * cr - P.beta_re * ci);
-        double2* d = P.D + (size_t)(mode - pm + ((P.L - pm) % P.L)) * P.NN + (size_t)j * N + i;
-        if (P.accumulate_d) {
+    if (G.D) {
+        const int pm = mode % L;
+        double2 out = make_double2(G.beta_re * cr + G.beta_im * ci, G.beta_im * cr - G.beta_re * ci);
+        double2* d = G.D + (size_t)(mode - pm + ((L - pm) % L)) * NN + (size_t)j * N + i;
+        if (G.accumulate_d) {
             out.x += d->x;
             out.y += d->y;
         }
@@ -368,7 +388,8 @@ cudaError_t zgemm_init() { return cudaSuccess; }
 namespace {
 
 template <class TC>
-cudaError_t launch_dmma(const FreqLayout& f, int modes, const double* A, const double* B, GemmParams P, cudaStream_t st) {
+cudaError_t launch_dmma(const FreqLayout& f, const double* baseA, int modesA, const double* baseB, int modesB, GemmParams P,
+                        cudaStream_t st) {
     static bool attr_done = false;
     cudaError_t e;
     if (!attr_done) {
@@ -379,46 +400,85 @@ cudaError_t launch_dmma(const FreqLayout& f, int modes, const double* A, const d
     P.tiles_m = (f.N + TC::BM - 1) / TC::BM;
     P.tiles_n = (f.N + TC::BN - 1) / TC::BN;
     CUtensorMap mapA, mapB;
-    if ((e = encode_operand(&mapA, A, f, modes, TC::BM)) != cudaSuccess) return e;
-    if ((e = encode_operand(&mapB, B, f, modes, BK)) != cudaSuccess) return e;
-    const unsigned grid = (unsigned)(modes * P.tiles_m * P.tiles_n);
+    if ((e = encode_operand(&mapA, baseA, f, modesA, TC::BM)) != cudaSuccess) return e;
+    if ((e = encode_operand(&mapB, baseB, f, modesB, BK)) != cudaSuccess) return e;
+    const unsigned grid = (unsigned)(P.ngroups * P.nmodes * P.tiles_m * P.tiles_n);
     zgemm_modes_dmma_kernel<TC><<<grid, TC::THREADS, TC::SMEM_BYTES, st>>>(mapA, mapB, P);
     return cudaGetLastError();
 }
 
+GemmGroupDev to_dev(const GemmOut& out) {
+    GemmGroupDev g{};
+    g.C = reinterpret_cast<double2*>(out.C);
+    g.D = reinterpret_cast<double2*>(out.D);
+    g.alpha_re = out.alpha.re;
+    g.alpha_im = out.alpha.im;
+    g.beta_re = out.beta.re;
+    g.beta_im = out.beta.im;
+    g.diag = out.diag;
+    g.accumulate = out.accumulate ? 1 : 0;
+    g.accumulate_d = out.accumulate_d ? 1 : 0;
+    return g;
+}
+
 }  // namespace
 
-cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out,
-                               int variant, cudaStream_t st) {
+cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup* groups, int ngroups, int variant,
+                                cudaStream_t st) {
     const int modes = batch * f.L;
-    if (!out.C && !out.D) return cudaErrorInvalidValue;
-    GemmParams P;
-    P.C = reinterpret_cast<double2*>(out.C);
-    P.D = reinterpret_cast<double2*>(out.D);
+    if (ngroups < 1 || ngroups > MAX_GROUPS) return cudaErrorInvalidValue;
+    for (int i = 0; i < ngroups; ++i)
+        if (!groups[i].A || !groups[i].B || (!groups[i].out.C && !groups[i].out.D)) return cudaErrorInvalidValue;
+    if (variant == 0) {
+        for (int i = 0; i < ngroups; ++i) {
+            dim3 grid((f.N + 15) / 16, (f.N + 15) / 16, modes);
+            zgemm_modes_ref_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(groups[i].A),
+                                                         reinterpret_cast<const double2*>(groups[i].B), to_dev(groups[i].out),
+                                                         f.N, f.NN, f.L);
+            cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+        }
+        return cudaSuccess;
+    }
+    if (variant != 1) return cudaErrorInvalidValue;
+    // one tensor map per operand side spans every group's spectrum: the groups address it by mode offset, so
+    // their operands must sit a whole number of N x N matrices apart (spectra of one workspace always do)
+    const double* baseA = groups[0].A;
+    const double* baseB = groups[0].B;
+    for (int i = 1; i < ngroups; ++i) {
+        if (groups[i].A < baseA) baseA = groups[i].A;
+        if (groups[i].B < baseB) baseB = groups[i].B;
+    }
+    GemmParams P{};
     P.NN = f.NN;
     P.N = f.N;
     P.L = f.L;
-    P.tiles_m = P.tiles_n = 0;
-    P.alpha_re = out.alpha.re;
-    P.alpha_im = out.alpha.im;
-    P.beta_re = out.beta.re;
-    P.beta_im = out.beta.im;
-    P.accumulate = out.accumulate ? 1 : 0;
-    P.accumulate_d = out.accumulate_d ? 1 : 0;
-    P.diag = out.diag;
-    switch (variant) {
-        case 0: {
-            dim3 grid((f.N + 15) / 16, (f.N + 15) / 16, modes);
-            zgemm_modes_ref_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(A),
-                                                         reinterpret_cast<const double2*>(B), P);
-            return cudaGetLastError();
-        }
-        // 48 x 48 CTA tile, 4 warps of 24 x 24, 3 CTAs per SM, 5-deep ring.  Measured alternatives on B200 at N = 225,
-        // L = 128 (331 us): 64 x 48 / 8 warps of 16 x 24 / 2 CTAs 341 us; 48 x 64 / 8 warps of 24 x 16 354 us; 32 x 48 /
-        // 4 warps / 4 CTAs 338 us; 6-deep ring 331 us; 2 CTAs with an 8-deep ring 359 us.
-        case 1: return launch_dmma<Tile<3, 3, 2, 2, 3, 5>>(f, modes, A, B, P, st);
-        default: return cudaErrorInvalidValue;
+    P.nmodes = modes;
+    P.ngroups = ngroups;
+    const size_t mat = f.NN * 2;  // doubles per mode
+    long long maxA = 0, maxB = 0;
+    for (int i = 0; i < ngroups; ++i) {
+        const size_t da = (size_t)(groups[i].A - baseA), db = (size_t)(groups[i].B - baseB);
+        if (da % mat || db % mat) return cudaErrorInvalidValue;
+        P.g[i] = to_dev(groups[i].out);
+        P.g[i].aoff = (int)(da / mat);
+        P.g[i].boff = (int)(db / mat);
+        if ((long long)(da / mat) > maxA) maxA = (long long)(da / mat);
+        if ((long long)(db / mat) > maxB) maxB = (long long)(db / mat);
     }
+    // 48 x 48 CTA tile, 4 warps of 24 x 24, 3 CTAs per SM, 5-deep ring.  Measured alternatives on B200 at N = 225,
+    // L = 128 (331 us): 64 x 48 / 8 warps of 16 x 24 / 2 CTAs 341 us; 48 x 64 / 8 warps of 24 x 16 354 us; 32 x 48 /
+    // 4 warps / 4 CTAs 338 us; 6-deep ring 331 us; 2 CTAs with an 8-deep ring 359 us.
+    return launch_dmma<Tile<3, 3, 2, 2, 3, 5>>(f, baseA, (int)maxA + modes, baseB, (int)maxB + modes, P, st);
+}
+
+cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out,
+                               int variant, cudaStream_t st) {
+    GemmGroup g;
+    g.A = A;
+    g.B = B;
+    g.out = out;
+    return launch_zgemm_groups(f, batch, &g, 1, variant, st);
 }
 
 }  // namespace nspt
