@@ -685,9 +685,12 @@ cudaError_t dispatch(int L, Which w, const XformParams& P, int nops, cudaStream_
         case 8: return run_small<8, 128>(w, P, nops, st);
         case 16: return run_tma<4, 4, 32>(w, P, nops, st);
         case 32: return run_tma<8, 4, 32>(w, P, nops, st);
-        case 64: return run_tma<8, 8, 16>(w, P, nops, st);
-        case 128: return run_tma<16, 8, 16>(w, P, nops, st);
-        case 256: return run_tma<16, 16, 8>(w, P, nops, st);
+        // The forward pass (1 byte read : 2 written) gains from wider rows per TMA box -- measured at N = 225: L = 64
+        // 32.8 -> 32.0 us, L = 128 63.9 -> 60.2 us, L = 256 140 -> 129 us -- while the inverse and re-truncation passes lose
+        // with them (L = 128: 34.2 -> 37.2 us, L = 256: 58.5 -> 68.9 us) and keep the narrower tiles.
+        case 64: return w == W_FWD ? run_tma<8, 8, 32>(w, P, nops, st) : run_tma<8, 8, 16>(w, P, nops, st);
+        case 128: return w == W_FWD ? run_tma<16, 8, 32>(w, P, nops, st) : run_tma<16, 8, 16>(w, P, nops, st);
+        case 256: return w == W_FWD ? run_tma<16, 16, 16>(w, P, nops, st) : run_tma<16, 16, 8>(w, P, nops, st);
         default: return cudaErrorInvalidValue;
     }
 }
