@@ -404,6 +404,10 @@ __global__ void __launch_bounds__(T* S) fft_forward_tma_kernel(const __grid_cons
 #pragma unroll
         for (int i = 0; i < NS; ++i) mbar_init(bar + 8 * i, 1);
         mbar_fence_init();
+    }
+    pdl_wait();      // everything above overlaps the tail of the previous kernel of the stream
+    pdl_trigger();
+    if (threadIdx.x == 0) {
 #pragma unroll
         for (int i = 0; i < NS; ++i)
             if (blockIdx.x + i * gridDim.x < P.total_tiles) issue(blockIdx.x + i * gridDim.x, i);
@@ -482,6 +486,10 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
 #pragma unroll
         for (int i = 0; i < NS; ++i) mbar_init(bar + 8 * i, 1);
         mbar_fence_init();
+    }
+    pdl_wait();      // everything above overlaps the tail of the previous kernel of the stream
+    pdl_trigger();
+    if (threadIdx.x == 0) {
 #pragma unroll
         for (int i = 0; i < NS; ++i)
             if (blockIdx.x + i * gridDim.x < P.total_tiles) issue(blockIdx.x + i * gridDim.x, i);
@@ -658,7 +666,7 @@ cudaError_t run_tma(Which w, XformParams P, int nops, cudaStream_t st) {
         }
         auto kern = fft_forward_tma_kernel<R, S, T>;
         if ((e = persistent_grid(kern, C::THREADS, C::FWD_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
-        kern<<<grid, C::THREADS, C::FWD_SMEM, st>>>(in[0], in[1], out[0], out[1], P);
+        return launch_pdl(kern, grid, C::THREADS, C::FWD_SMEM, st, in[0], in[1], out[0], out[1], P);
     } else {
         CUtensorMap in, out;
         if ((e = tma_encode_f64(&in, P.src_freq, 3, fdims, fstrides, fbox, false)) != cudaSuccess) return e;
@@ -666,12 +674,12 @@ cudaError_t run_tma(Which w, XformParams P, int nops, cudaStream_t st) {
             if ((e = tma_encode_f64(&out, P.dst_series, 3, sdims, sstrides, sbox, false)) != cudaSuccess) return e;
             auto kern = fft_inverse_tma_kernel<R, S, T, false>;
             if ((e = persistent_grid(kern, C::THREADS, C::INV_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
-            kern<<<grid, C::THREADS, C::INV_SMEM, st>>>(in, out, P);
+            return launch_pdl(kern, grid, C::THREADS, C::INV_SMEM, st, in, out, P);
         } else {
             if ((e = tma_encode_f64(&out, P.dst_freq[0], 3, fdims, fstrides, fbox, false)) != cudaSuccess) return e;
             auto kern = fft_inverse_tma_kernel<R, S, T, true>;
             if ((e = persistent_grid(kern, C::THREADS, C::RET_SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
-            kern<<<grid, C::THREADS, C::RET_SMEM, st>>>(in, out, P);
+            return launch_pdl(kern, grid, C::THREADS, C::RET_SMEM, st, in, out, P);
         }
     }
     return cudaGetLastError();

@@ -196,6 +196,10 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
             mbar_init(bar_empty + 8 * s, TC::WARPS);
         }
         mbar_fence_init();
+    }
+    pdl_wait();      // the set-up above overlaps the tail of the previous kernel of the stream
+    pdl_trigger();
+    if (threadIdx.x == 0) {
         const int pre = nk < STAGES ? nk : STAGES;
         for (int it = 0; it < pre; ++it)
             issue_slice<TC>(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, it * BK, m0, n0, modeA, modeB);
@@ -403,8 +407,7 @@ cudaError_t launch_dmma(const FreqLayout& f, const double* baseA, int modesA, co
     if ((e = encode_operand(&mapA, baseA, f, modesA, TC::BM)) != cudaSuccess) return e;
     if ((e = encode_operand(&mapB, baseB, f, modesB, BK)) != cudaSuccess) return e;
     const unsigned grid = (unsigned)(P.ngroups * P.nmodes * P.tiles_m * P.tiles_n);
-    zgemm_modes_dmma_kernel<TC><<<grid, TC::THREADS, TC::SMEM_BYTES, st>>>(mapA, mapB, P);
-    return cudaGetLastError();
+    return launch_pdl(zgemm_modes_dmma_kernel<TC>, grid, TC::THREADS, TC::SMEM_BYTES, st, mapA, mapB, P);
 }
 
 GemmGroupDev to_dev(const GemmOut& out) {
