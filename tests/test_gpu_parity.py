@@ -454,3 +454,88 @@ def test_force_rejects_aliasing(nspt):
     S = to_dev(np.zeros((2, 4, 4), dtype=np.complex128))
     with pytest.raises(nspt.NsptError):
         nspt.nspt_force(S, 1.0, S)
+
+
+# ----------------------------------------------------------------------------- context state across calls
+
+def test_order_scale_is_transparent_for_staple_and_exp(nspt):
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    U, z = wl.config_staple(9, 15, seed=80, twist_k=1)
+    X = anti_hermitian_series(10, 9, seed=81)
+    ref_exp = oracle.series_exp(X)
+    try:
+        for s in (0.9, 1.1):
+            nspt.nspt_set_order_scale(s)
+            check_staple(nspt, U, z)
+            got = gpu_exp(nspt, X)
+            assert oracle.per_order_error(got, ref_exp, oracle.exp_bound(X)).max() <= TOL
+    finally:
+        nspt.nspt_set_order_scale(1.0)
+
+
+def test_caller_workspace_for_staple_and_exp(nspt):
+    import torch
+    from paper_2001_02835_b200 import workloads as wl
+    import oracle
+    U, z = wl.config_staple(9, 7, seed=82, twist_k=1)
+    X = anti_hermitian_series(9, 7, seed=83)
+    need_s = nspt.nspt_workspace_bytes(9, 7, 1, nspt.NSPT_OP_STAPLE)
+    need_e = nspt.nspt_workspace_bytes(9, 7, 1, nspt.NSPT_OP_SERIES_EXP)
+    assert need_s == 30 * 16 * 81 * 16 and need_e == 3 * 16 * 81 * 16       # 30 and 3 spectra of L = 16 modes
+    ws = torch.empty(need_s, dtype=torch.uint8, device="cuda")
+    try:
+        nspt.nspt_set_workspace(ws.data_ptr(), need_s)
+        check_staple(nspt, U, z)
+        got = gpu_exp(nspt, X)
+        assert oracle.per_order_error(got, oracle.series_exp(X), oracle.exp_bound(X)).max() <= TOL
+        nspt.nspt_set_workspace(ws.data_ptr(), need_s - 16)
+        with pytest.raises(nspt.NsptError) as ei:
+            nspt.nspt_staple([to_dev(u) for u in U], z)
+        assert ei.value.code == nspt.NSPT_ENOMEM
+    finally:
+        nspt.nspt_set_workspace(None, 0)
+
+
+def test_alternating_shapes_and_calls_back_to_back(nspt):
+    # plans, tensor maps and the workspace are rebuilt per call; nothing may leak from one shape to the next,
+    # and kernels launched with programmatic stream serialization must still see their predecessor's output
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(84)
+    cases = [(33, 31), (9, 7), (57, 9), (12, 63), (33, 31), (5, 3), (20, 127)]
+    data = [(wl.gaussian_series(N, nt, rng), wl.gaussian_series(N, nt, rng)) for N, nt in cases]
+    dev = [(to_dev(a), to_dev(b)) for a, b in data]
+    outs = [nspt.nspt_series_mul(a, b) for a, b in dev]          # all enqueued before any synchronisation
+    torch.cuda.synchronize()
+    for (A, B), C in zip(data, outs):
+        err = oracle.per_order_error(C.cpu().numpy(), oracle.series_mul(A, B), oracle.product_bound(A, B))
+        assert err.max() <= TOL
+
+
+def test_chained_products_on_the_stream(nspt):
+    # (A*B)*C computed with the output of one call feeding the next, no synchronisation in between
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(85)
+    A, B, C = (wl.gaussian_series(40, 15, rng) for _ in range(3))
+    dA, dB, dC = to_dev(A), to_dev(B), to_dev(C)
+    T = nspt.nspt_series_mul(dA, dB)
+    nspt.nspt_series_mul(T, dC, T)
+    torch.cuda.synchronize()
+    AB = oracle.series_mul(A, B)
+    ref = oracle.series_mul(AB, C)
+    bound = oracle.product_bound(AB, C)
+    assert oracle.per_order_error(T.cpu().numpy(), ref, bound).max() <= 2 * TOL
+
+
+def test_release_and_reuse(nspt):
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(86)
+    A, B = wl.gaussian_series(17, 5, rng), wl.gaussian_series(17, 5, rng)
+    check_product(nspt, A, B)
+    nspt.nspt_release()
+    check_product(nspt, A, B)
