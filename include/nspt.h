@@ -115,7 +115,8 @@ int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc);
 int nspt_force(const nspt_c128* S, nspt_c128* F, double c, int N, int Ntrunc);
 
 /* Host-buffer forms of nspt_series_mul, nspt_series_mul_batched and nspt_staple: same semantics, HOST pointers for the series,
- * host<->device copies on the library stream inside the call, stream synchronised on return. */
+ * host<->device copies inside the call, everything synchronised on return.  For batch > 1 the batched form overlaps the
+ * copy-in of element b+1, the product of element b and the copy-out of element b-1 on internal copy streams. */
 int nspt_series_mul_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc);
 int nspt_series_mul_batched_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C,
                                  int N, int Ntrunc, int batch);

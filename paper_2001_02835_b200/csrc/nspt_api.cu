@@ -38,9 +38,11 @@ struct Context {
     size_t user_ws_bytes = 0;
     void* own_ws = nullptr;
     size_t own_ws_bytes = 0;
-    // staging for the _host calls
+    // staging for the _host calls; copy streams and events of the pipelined batched call
     void* stage_dev = nullptr;
     size_t stage_dev_bytes = 0;
+    cudaStream_t h2d = nullptr, d2h = nullptr;
+    std::vector<cudaEvent_t> copy_events;
     std::vector<Plan> plans;
     // profiling
     bool profiling = false;
@@ -524,10 +526,39 @@ int nspt_series_mul_batched_host(const nspt_c128* A, const nspt_c128* B, nspt_c1
     nspt_c128* dA = reinterpret_cast<nspt_c128*>(dev);
     nspt_c128* dB = reinterpret_cast<nspt_c128*>(dev + slot);
     nspt_c128* dC = reinterpret_cast<nspt_c128*>(dev + 2 * slot);
-    NSPT_CUDA(cudaMemcpyAsync(dA, A, bytes, cudaMemcpyHostToDevice, g.stream));
-    NSPT_CUDA(cudaMemcpyAsync(dB, B, bytes, cudaMemcpyHostToDevice, g.stream));
-    NSPT_TRY(series_mul_device(dA, dB, dC, N, Ntrunc, batch));
-    NSPT_CUDA(cudaMemcpyAsync(C, dC, bytes, cudaMemcpyDeviceToHost, g.stream));
+    if (batch == 1) {
+        NSPT_CUDA(cudaMemcpyAsync(dA, A, bytes, cudaMemcpyHostToDevice, g.stream));
+        NSPT_CUDA(cudaMemcpyAsync(dB, B, bytes, cudaMemcpyHostToDevice, g.stream));
+        NSPT_TRY(series_mul_device(dA, dB, dC, N, Ntrunc, 1));
+        NSPT_CUDA(cudaMemcpyAsync(C, dC, bytes, cudaMemcpyDeviceToHost, g.stream));
+        NSPT_CUDA(cudaStreamSynchronize(g.stream));
+        return NSPT_OK;
+    }
+    // batch > 1: the products are independent, so element b+1 is copied in (one copy stream) while element b is
+    // multiplied (library stream) and element b-1 is copied out (second copy stream, PCIe is full duplex).
+    if (!g.h2d) NSPT_CUDA(cudaStreamCreateWithFlags(&g.h2d, cudaStreamNonBlocking));
+    if (!g.d2h) NSPT_CUDA(cudaStreamCreateWithFlags(&g.d2h, cudaStreamNonBlocking));
+    while (g.copy_events.size() < (size_t)(2 * batch + 1)) {
+        cudaEvent_t e;
+        NSPT_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        g.copy_events.push_back(e);
+    }
+    const size_t one = bytes / batch;
+    const size_t elems = one / sizeof(nspt_c128);
+    // the copy-in stream must not overtake earlier work of the library stream that may still read the staging area
+    NSPT_CUDA(cudaEventRecord(g.copy_events[2 * batch], g.stream));
+    NSPT_CUDA(cudaStreamWaitEvent(g.h2d, g.copy_events[2 * batch], 0));
+    for (int b = 0; b < batch; ++b) {
+        NSPT_CUDA(cudaMemcpyAsync(dA + b * elems, A + b * elems, one, cudaMemcpyHostToDevice, g.h2d));
+        NSPT_CUDA(cudaMemcpyAsync(dB + b * elems, B + b * elems, one, cudaMemcpyHostToDevice, g.h2d));
+        NSPT_CUDA(cudaEventRecord(g.copy_events[2 * b], g.h2d));
+        NSPT_CUDA(cudaStreamWaitEvent(g.stream, g.copy_events[2 * b], 0));
+        NSPT_TRY(series_mul_device(dA + b * elems, dB + b * elems, dC + b * elems, N, Ntrunc, 1));
+        NSPT_CUDA(cudaEventRecord(g.copy_events[2 * b + 1], g.stream));
+        NSPT_CUDA(cudaStreamWaitEvent(g.d2h, g.copy_events[2 * b + 1], 0));
+        NSPT_CUDA(cudaMemcpyAsync(C + b * elems, dC + b * elems, one, cudaMemcpyDeviceToHost, g.d2h));
+    }
+    NSPT_CUDA(cudaStreamSynchronize(g.d2h));
     NSPT_CUDA(cudaStreamSynchronize(g.stream));
     return NSPT_OK;
 }
@@ -639,6 +670,11 @@ int nspt_release(void) {
     if (g.stage_dev) cudaFree(g.stage_dev);
     g.stage_dev = nullptr;
     g.stage_dev_bytes = 0;
+    for (cudaEvent_t e : g.copy_events) cudaEventDestroy(e);
+    g.copy_events.clear();
+    if (g.h2d) cudaStreamDestroy(g.h2d);
+    if (g.d2h) cudaStreamDestroy(g.d2h);
+    g.h2d = g.d2h = nullptr;
     for (ProfEvent& e : g.prof_used) {
         cudaEventDestroy(e.a);
         cudaEventDestroy(e.b);

@@ -174,6 +174,16 @@ def test_host_entry_points(nspt):
     Cb = np.empty_like(Ab)
     nspt.nspt_series_mul_batched_host(Ab, Bb, Cb)
     assert oracle.per_order_error(Cb[1], oracle.series_mul(B, A), oracle.product_bound(B, A)).max() <= TOL
+    # batch > 1 is pipelined over copy streams inside the call: every element must still be its own product
+    X = [wl.gaussian_series(31, 7, rng) for _ in range(5)]
+    A5, B5 = np.stack(X), np.stack(X[::-1])
+    C5 = np.empty_like(A5)
+    for _ in range(2):
+        C5[:] = 0
+        nspt.nspt_series_mul_batched_host(A5, B5, C5)
+        for b in range(5):
+            ref = oracle.series_mul(A5[b], B5[b])
+            assert oracle.per_order_error(C5[b], ref, oracle.product_bound(A5[b], B5[b])).max() <= TOL
 
 
 def test_order_scale_is_transparent(nspt):
