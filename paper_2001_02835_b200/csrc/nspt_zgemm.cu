@@ -65,6 +65,12 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 }
 
 // One product of a launch: modes [aoff, aoff + nmodes) of the A tensor map times modes [boff, ...) of the B map.
+// *dst += v without reading it back (RED.E.ADD.F64)
+__device__ __forceinline__ void red_add(double2& dst, double2 v) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&dst.x), "d"(v.x) : "memory");
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&dst.y), "d"(v.y) : "memory");
+}
+
 struct GemmGroupDev {
     double2* C;   // direct target:   C(p)            (+)= alpha * A(p) B(p) + diag   (may be null)
     double2* D;   // daggered target: D((L-p) mod L)  (+)= beta * (A(p) B(p))^H       (may be null)
@@ -275,17 +281,14 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
                         if (m == n + 1) o1.x += diag;
                         double2* d = Cm + (size_t)m * N + n;
                         if (accumulate) {
-                            const double2 old0 = d[0];
-                            o0.x += old0.x;
-                            o0.y += old0.y;
-                            if (second) {
-                                const double2 old1 = d[1];
-                                o1.x += old1.x;
-                                o1.y += old1.y;
-                            }
+                            // fire-and-forget reductions: every element receives exactly one contribution per launch
+                            // (deterministic), and nothing waits for the old value to come back from L2 / HBM
+                            red_add(d[0], o0);
+                            if (second) red_add(d[1], o1);
+                        } else {
+                            d[0] = o0;
+                            if (second) d[1] = o1;
                         }
-                        d[0] = o0;
-                        if (second) d[1] = o1;
                     }
                     if (Dm) {
                         // beta * conj(c): the eight lanes g = 0..7 of a quarter-warp write 128 contiguous bytes
@@ -294,17 +297,12 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
                         double2* d0 = Dm + (size_t)n * N + m;
                         double2* d1 = d0 + N;
                         if (accumulate_d) {
-                            const double2 old0 = *d0;
-                            o0.x += old0.x;
-                            o0.y += old0.y;
-                            if (second) {
-                                const double2 old1 = *d1;
-                                o1.x += old1.x;
-                                o1.y += old1.y;
-                            }
+                            red_add(*d0, o0);
+                            if (second) red_add(*d1, o1);
+                        } else {
+                            *d0 = o0;
+                            if (second) *d1 = o1;
                         }
-                        *d0 = o0;
-                        if (second) *d1 = o1;
                     }
                 }
             }
