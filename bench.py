@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- series star-products per second on B200 (BASELINE.json metric), one JSON line.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg2|staple|batched4|sweep]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg2|staple|batched4|exp|exp4|sweep]
     python bench.py --impl reference ...        # the CPU oracle as the reference arm
 
 A step is one pass of the whole hot path over one synthetic input: for the default workload
@@ -53,6 +53,7 @@ WORKLOADS = {
     "small": ("product", 9, 7, 1, 0),
     "sweep": ("sweep", 225, 31, 1, 5),
     "exp": ("exp", 225, 31, 1, 6),
+    "exp4": ("exp", 225, 31, 4, 6),
 }
 
 
@@ -392,15 +393,20 @@ def run_cuda(args):
             gen.manual_seed(seed)
             sets = []
             for r in range(R):
-                G = torch.randn(n, N, N, dtype=torch.complex128, device=dev, generator=gen)
-                H = (G + G.conj().transpose(1, 2)) / (2.0 * N) ** 0.5
+                G = torch.randn(batch, n, N, N, dtype=torch.complex128, device=dev, generator=gen)
+                H = (G + G.conj().transpose(2, 3)) / (2.0 * N) ** 0.5
                 X = (1j * H).contiguous()
-                X[0] = 0
+                X[:, 0] = 0
+                if batch == 1:
+                    X = X[0].contiguous()
                 sets.append((X, torch.empty_like(X)))
 
             def step(i):
                 X, E = sets[i % R]
-                nspt.nspt_series_exp(X, E)
+                if batch == 1:
+                    nspt.nspt_series_exp(X, E)
+                else:
+                    nspt.nspt_series_exp_batched(X, E)
             products_per_step = max(Ntrunc - 1, 0)
             units_name = "exponentials"
         elif kind == "staple":
@@ -466,7 +472,8 @@ def run_cuda(args):
     ms_local = ev0.elapsed_time(ev1)
     launches = nspt.nspt_launch_count() - launches0
     clocks = sampler.stop()
-    value, ms_total = aggregate_throughput(K * (products_per_step if kind not in ("staple", "exp") else 1), ms_local, world, dev)
+    units_per_step = 1 if kind == "staple" else (batch if kind == "exp" else products_per_step)
+    value, ms_total = aggregate_throughput(K * units_per_step, ms_local, world, dev)
 
     # ---- timed region 2: the same K steps with the stage profiler on -> per-kernel durations
     nspt.nspt_profile(True)
@@ -625,6 +632,7 @@ def run_cuda(args):
         "staple": "full TEK staple S_mu, mu=1..4, N=225, N_trunc=31, k=4 twist (BASELINE.json configs[3]); 36 mode-wise products per step (literal eq. 2.3: 52)",
         "small": "single star-product A*B, N=9, N_trunc=7 (BASELINE.json configs[0])",
         "exp": "series exponential exp(X), X anti-Hermitian series, N=225, N_trunc=31 (link-update exponential; 30 mode-wise products)",
+        "exp4": "batch of 4 series exponentials (the four links of an update), N=225, N_trunc=31; 30 batched mode-wise products",
     }[args.workload]
     line = {
         "metric": {"staple": "tek_staples_per_sec", "exp": "series_exponentials_per_sec"}.get(kind, METRIC),
@@ -660,7 +668,7 @@ def main():
         args.steps = args.steps if args.steps is not None else 50
         args.warmup = args.warmup if args.warmup is not None else 3
         return run_sweep(args)
-    args.steps = args.steps if args.steps is not None else (200 if args.workload not in ("staple", "exp") else 10)
+    args.steps = args.steps if args.steps is not None else (200 if args.workload not in ("staple", "exp", "exp4") else 10)
     args.warmup = args.warmup if args.warmup is not None else 5
     return run_cuda(args)
 

@@ -104,6 +104,8 @@ int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* c
  * E may alias X.
  */
 int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc);
+/* batch independent exponentials E_b = exp(X_b) (the four links of an update); element b at offset b*(Ntrunc+1)*N*N. */
+int nspt_series_exp_batched(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int batch);
 
 /*
  * The force of eq. 2.3 from a staple series, order by order:
@@ -134,8 +136,8 @@ int nspt_set_stream(void* cuda_stream);
  * (s^l)(s^(k-l)) = s^k.  s = 1 (default) switches it off.  s must be finite and > 0. */
 int nspt_set_order_scale(double s);
 
-/* Bytes of device workspace a call needs (op = NSPT_OP_SERIES_MUL with its batch, or
- * NSPT_OP_STAPLE / NSPT_OP_SERIES_EXP, batch ignored).  nspt_force needs none. */
+/* Bytes of device workspace a call needs (op = NSPT_OP_SERIES_MUL or
+ * NSPT_OP_SERIES_EXP with theirs, or NSPT_OP_STAPLE, batch ignored).  nspt_force needs none.  batch <= 65535. */
 int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out);
 
 /* Give the library a caller-owned device workspace (256-byte aligned).  Calls that need more

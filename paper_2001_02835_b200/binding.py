@@ -23,7 +23,7 @@ NSPT_OP_SERIES_MUL, NSPT_OP_STAPLE, NSPT_OP_SERIES_EXP = 0, 1, 2
 STAGES = {"fft_forward": 0, "zgemm_modes": 1, "fft_inverse": 2, "fft_retruncate": 3, "other": 4}
 
 EXPORTS = [
-    "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_series_exp", "nspt_force",
+    "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_series_exp", "nspt_series_exp_batched", "nspt_force",
     "nspt_series_mul_host", "nspt_series_mul_batched_host", "nspt_staple_host",
     "nspt_set_stream", "nspt_set_order_scale", "nspt_workspace_bytes", "nspt_set_workspace",
     "nspt_set_gemm_variant", "nspt_probe_fp64_peak", "nspt_profile", "nspt_profile_read", "nspt_launch_count",
@@ -48,6 +48,7 @@ _lib.nspt_series_mul.argtypes = [_vp, _vp, _vp, _int, _int]
 _lib.nspt_series_mul_batched.argtypes = [_vp, _vp, _vp, _int, _int, _int]
 _lib.nspt_staple.argtypes = [ctypes.POINTER(_vp), _vp, ctypes.POINTER(_vp), _int, _int]
 _lib.nspt_series_exp.argtypes = [_vp, _vp, _int, _int]
+_lib.nspt_series_exp_batched.argtypes = [_vp, _vp, _int, _int, _int]
 _lib.nspt_force.argtypes = [_vp, _vp, _dbl, _int, _int]
 _lib.nspt_series_mul_host.argtypes = [_vp, _vp, _vp, _int, _int]
 _lib.nspt_series_mul_batched_host.argtypes = [_vp, _vp, _vp, _int, _int, _int]
@@ -171,6 +172,18 @@ def nspt_series_exp(X, E=None):
         E = torch.empty_like(X)
     _dev_series(E, "E")
     _check(_lib.nspt_series_exp(X.data_ptr(), E.data_ptr(), N, Ntrunc), "nspt_series_exp")
+    return E
+
+
+def nspt_series_exp_batched(X, E=None):
+    """E_b = exp(X_b) for a stack of series, shape (batch, Ntrunc+1, N, N)."""
+    torch = _torch()
+    X = _dev_series(X, "X")
+    batch, Ntrunc, N = _shape(X, True)
+    if E is None:
+        E = torch.empty_like(X)
+    _dev_series(E, "E")
+    _check(_lib.nspt_series_exp_batched(X.data_ptr(), E.data_ptr(), N, Ntrunc, batch), "nspt_series_exp_batched")
     return E
 
 

@@ -81,7 +81,7 @@ int check_arch() {
 
 int check_dims(int N, int Ntrunc, int batch) {
     if (N < 1 || Ntrunc < 0 || batch < 1) return NSPT_EINVAL;
-    if (Ntrunc > NSPT_MAX_NTRUNC) return NSPT_EINVAL;
+    if (Ntrunc > NSPT_MAX_NTRUNC || batch > 65535) return NSPT_EINVAL;
     if ((long long)N * N > (1ll << 40)) return NSPT_EINVAL;
     return NSPT_OK;
 }
@@ -322,8 +322,8 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
 // X~ is transformed once; every step is one mode-wise product whose epilogue scales by 1/m and adds the
 // identity series (the unit matrix at every mode), followed by a re-truncation pass (a length-L cyclic
 // transform protects one product only); the last step goes straight to the inverse transform.
-int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc) {
-    NSPT_TRY(check_dims(N, Ntrunc, 1));
+int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int batch) {
+    NSPT_TRY(check_dims(N, Ntrunc, batch));
     if (!X || !E || !aligned16(X) || !aligned16(E)) return NSPT_EINVAL;
     NSPT_TRY(check_arch());
     const FreqLayout f = make_layout(N, Ntrunc);
@@ -331,22 +331,22 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc) {
     PlanTables t;
     NSPT_TRY(get_plan(f.L, f.n, g.order_scale, &t));
     char* ws = nullptr;
-    NSPT_TRY(get_workspace(ws_bytes_for(f, 1, NSPT_OP_SERIES_EXP), &ws));
-    const size_t sb = spectrum_bytes(f, 1);
+    NSPT_TRY(get_workspace(ws_bytes_for(f, batch, NSPT_OP_SERIES_EXP), &ws));
+    const size_t sb = spectrum_bytes(f, batch);
     double* Xt = reinterpret_cast<double*>(ws);
     double* Tt = reinterpret_cast<double*>(ws + sb);
     double* Pt = reinterpret_cast<double*>(ws + 2 * sb);
     {   // X~ with the coefficient of g^0 taken as zero
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_FWD));
-        NSPT_CUDA(launch_fft_forward(f, t, 1, X, Xt, nullptr, nullptr, g.stream, true));
+        NSPT_CUDA(launch_fft_forward(f, t, batch, X, Xt, nullptr, nullptr, g.stream, true));
         NSPT_TRY(tm.end());
     }
     const int n = Ntrunc > 0 ? Ntrunc : 1;
     {   // T_n = 1 + X/n
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_OTHER));
-        NSPT_CUDA(launch_freq_scale_identity(f, 1, Xt, Tt, 1.0 / n, g.stream));
+        NSPT_CUDA(launch_freq_scale_identity(f, batch, Xt, Tt, 1.0 / n, g.stream));
         NSPT_TRY(tm.end());
     }
     double* cur = Tt;
@@ -356,13 +356,13 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc) {
         o.C = other;
         o.alpha = Cplx{1.0 / m, 0.0};
         o.diag = 1.0;
-        NSPT_TRY(k_gemm(f, 1, Xt, cur, o));
-        if (m > 1) NSPT_TRY(k_retrunc(f, t, 1, other, other));
+        NSPT_TRY(k_gemm(f, batch, Xt, cur, o));
+        if (m > 1) NSPT_TRY(k_retrunc(f, t, batch, other, other));
         double* tmp = cur;
         cur = other;
         other = tmp;
     }
-    return k_inverse(f, t, 1, cur, E);
+    return k_inverse(f, t, batch, cur, E);
 }
 
 int force_device(const nspt_c128* S, nspt_c128* F, double c, int N, int Ntrunc) {
@@ -507,7 +507,12 @@ int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* c
 
 int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc) {
     std::lock_guard<std::mutex> lk(g.mu);
-    return series_exp_device(X, E, N, Ntrunc);
+    return series_exp_device(X, E, N, Ntrunc, 1);
+}
+
+int nspt_series_exp_batched(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int batch) {
+    std::lock_guard<std::mutex> lk(g.mu);
+    return series_exp_device(X, E, N, Ntrunc, batch);
 }
 
 int nspt_force(const nspt_c128* S, nspt_c128* F, double c, int N, int Ntrunc) {
@@ -607,7 +612,7 @@ int nspt_set_order_scale(double s) {
 int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out) {
     if (!out) return NSPT_EINVAL;
     if (op != NSPT_OP_SERIES_MUL && op != NSPT_OP_STAPLE && op != NSPT_OP_SERIES_EXP) return NSPT_EINVAL;
-    if (op != NSPT_OP_SERIES_MUL) batch = 1;
+    if (op == NSPT_OP_STAPLE) batch = 1;
     NSPT_TRY(check_dims(N, Ntrunc, batch));
     const FreqLayout f = make_layout(N, Ntrunc);
     if (!fft_length_supported(f.L)) return NSPT_EINVAL;

@@ -395,6 +395,17 @@ def test_series_exp_generic_series_and_reference_gemm(nspt):
     nspt.nspt_set_gemm_variant(1)
 
 
+def test_series_exp_batched_matches_oracle(nspt):
+    import torch
+    import oracle
+    X = np.stack([anti_hermitian_series(21, 12, seed=[65, b]) for b in range(3)])
+    E = nspt.nspt_series_exp_batched(to_dev(X))
+    torch.cuda.synchronize()
+    E = E.cpu().numpy()
+    for b in range(3):
+        assert oracle.per_order_error(E[b], oracle.series_exp(X[b]), oracle.exp_bound(X[b])).max() <= TOL
+
+
 def test_series_exp_ignores_zeroth_order_and_may_alias(nspt):
     import torch
     import oracle
