@@ -99,9 +99,10 @@ int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* c
  * whose coefficient of g^0 vanishes; X^(0) is NOT read and is taken as zero (with X^(0) = 0 the power
  * X^{*m} starts at g^m, so the sum is finite and exact).  This is the exponential of the link update
  * U <- exp(i eps P) * U of the NSPT integrator ("solved with a symplectic integrator";
- * U-dot = i P * U, eq. 2.3), and of U = exp(i sum_k g^k H_k).  Ntrunc - 1 star-products (Horner form, X
- * transformed once, intermediate results kept in frequency space).  Device pointers, (Ntrunc+1)*N*N elements;
- * E may alias X.
+ * U-dot = i P * U, eq. 2.3), and of U = exp(i sum_k g^k H_k).  For Ntrunc >= 6 the sum is evaluated in the
+ * Paterson-Stockmeyer arrangement, (s-1)+(r-1) star-products with s = ceil(sqrt(Ntrunc+1)), r = ceil((Ntrunc+1)/s)
+ * (10 at Ntrunc = 31); below that by Horner with Ntrunc-1 products.  X is transformed once and all intermediate
+ * results stay in frequency space.  Device pointers, (Ntrunc+1)*N*N elements; E may alias X.
  */
 int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc);
 /* batch independent exponentials E_b = exp(X_b) (the four links of an update); element b at offset b*(Ntrunc+1)*N*N. */

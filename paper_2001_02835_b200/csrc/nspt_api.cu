@@ -157,8 +157,25 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 // several of them by mode offset; 16-byte alignment is all the TMA maps need.
 size_t spectrum_bytes(const FreqLayout& f, int batch) { return f.spectrum_doubles(batch) * 8; }
 
+// Paterson-Stockmeyer split of exp(X) = sum_{m <= n} X^m / m!: powers X^1..X^s and r = ceil((n+1)/s) block polynomials
+// (series_exp_device).  Below n = 6 the plain Horner form is used (s = 0).
+void exp_split(int Ntrunc, int* s, int* r) {
+    *s = 0;
+    *r = 0;
+    if (Ntrunc < 6) return;
+    int q = 1;
+    while (q * q < Ntrunc + 1) ++q;
+    *s = q;                                  // <= 12 for Ntrunc <= 127
+    *r = (Ntrunc + 1 + q - 1) / q;           // <= 12
+}
+
 size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
     if (op == NSPT_OP_STAPLE) return 30 * spectrum_bytes(f, 1);
+    if (op == NSPT_OP_SERIES_EXP) {
+        int s, r;
+        exp_split(f.n - 1, &s, &r);
+        return (size_t)(s ? s + r : 3) * spectrum_bytes(f, batch);
+    }
     return 3 * spectrum_bytes(f, batch);
 }
 
@@ -281,10 +298,10 @@ int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, con
     NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, out, g.gemm_variant, g.stream));
     return tm.end();
 }
-int k_gemm_groups(const FreqLayout& f, const GemmGroup* groups, int ngroups) {
+int k_gemm_groups(const FreqLayout& f, const GemmGroup* groups, int ngroups, int batch = 1) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_GEMM));
-    NSPT_CUDA(launch_zgemm_groups(f, 1, groups, ngroups, g.gemm_variant, g.stream));
+    NSPT_CUDA(launch_zgemm_groups(f, batch, groups, ngroups, g.gemm_variant, g.stream));
     return tm.end();
 }
 int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, double* C) {
@@ -317,11 +334,16 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
     return NSPT_OK;
 }
 
-// exp(X) = sum_m X^{*m}/m! by Horner in frequency space (reading c17):
-//     T_n = 1 + X/n,   T_m = 1 + (X * T_{m+1})/m  (m = n-1 .. 1),   exp(X) = T_1,     n = Ntrunc,
-// X~ is transformed once; every step is one mode-wise product whose epilogue scales by 1/m and adds the
-// identity series (the unit matrix at every mode), followed by a re-truncation pass (a length-L cyclic
-// transform protects one product only); the last step goes straight to the inverse transform.
+// exp(X) = sum_{m <= n} X^{*m}/m!, n = Ntrunc, in frequency space (reading c17).  X~ is transformed once, every
+// product is followed by a re-truncation pass (a length-L cyclic transform protects one product only), and the last
+// product goes straight to the inverse transform.
+//   n >= 6: Paterson-Stockmeyer.  With s = ceil(sqrt(n+1)), r = ceil((n+1)/s):
+//       exp(X) = sum_{j<r} (X^s)^j B_j(X),   B_j(X) = sum_{i<s} X^i / (s j + i)!   (terms beyond m = n dropped),
+//     the powers X^2..X^s by doubling (X^2; X^3, X^4; X^5..X^8; ...: each wave ONE grouped launch and one batched
+//     re-truncation), all B_j by one elementwise pass over the powers, then Horner in X^s: r-1 products whose
+//     epilogue accumulates acc * X^s onto B_j.  s - 1 + r - 1 products instead of n - 1 (10 instead of 30 at n = 31).
+//   n < 6: plain Horner, T_n = 1 + X/n, T_m = 1 + (X * T_{m+1})/m, exp(X) = T_1; the GEMM epilogue scales by 1/m and
+//     adds the identity series (the unit matrix at every mode).
 int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int batch) {
     NSPT_TRY(check_dims(N, Ntrunc, batch));
     if (!X || !E || !aligned16(X) || !aligned16(E)) return NSPT_EINVAL;
@@ -341,6 +363,48 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
         NSPT_TRY(tm.begin(ST_FWD));
         NSPT_CUDA(launch_fft_forward(f, t, batch, X, Xt, nullptr, nullptr, g.stream, true));
         NSPT_TRY(tm.end());
+    }
+    int ps, pr;
+    exp_split(Ntrunc, &ps, &pr);
+    if (ps) {
+        auto pw = [&](int i) { return reinterpret_cast<double*>(ws + (size_t)(i - 1) * sb); };     // spectrum of X^i, i = 1..s
+        auto bj = [&](int j) { return reinterpret_cast<double*>(ws + (size_t)(ps + j) * sb); };    // B_j, later the Horner sums
+        // powers by doubling: with X^1..X^h known, X^(h+i) = X^h * X^i for i = 1..min(h, s-h)
+        for (int h = 1; h < ps;) {
+            const int cnt = (ps - h) < h ? (ps - h) : h;
+            GemmGroup gr[12];
+            for (int i = 1; i <= cnt; ++i) {
+                gr[i - 1].A = pw(h);
+                gr[i - 1].B = pw(i);
+                gr[i - 1].out.C = pw(h + i);
+            }
+            NSPT_TRY(k_gemm_groups(f, gr, cnt, batch));
+            NSPT_TRY(k_retrunc(f, t, cnt * batch, pw(h + 1), pw(h + 1)));   // the new powers are contiguous
+            h += cnt;
+        }
+        {   // all block polynomials in one pass over X^1..X^(s-1)
+            double coef[144];
+            for (int j = 0; j < pr; ++j)
+                for (int i = 0; i < ps; ++i) {
+                    const int m = ps * j + i;
+                    long double fct = 1.0L;
+                    for (int q = 2; q <= m; ++q) fct *= q;
+                    coef[j * ps + i] = (m <= Ntrunc) ? (double)(1.0L / fct) : 0.0;
+                }
+            StageTimer tm;
+            NSPT_TRY(tm.begin(ST_OTHER));
+            NSPT_CUDA(launch_freq_block_polys(f, batch, pw(1), bj(0), ps, pr, coef, g.stream));
+            NSPT_TRY(tm.end());
+        }
+        // Horner in X^s: acc = B_{r-1}; acc = acc * X^s + B_j for j = r-2 .. 0 (the product is accumulated onto B_j)
+        for (int j = pr - 2; j >= 0; --j) {
+            GemmOut o;
+            o.C = bj(j);
+            o.accumulate = true;
+            NSPT_TRY(k_gemm(f, batch, bj(j + 1), pw(ps), o));
+            if (j > 0) NSPT_TRY(k_retrunc(f, t, batch, bj(j), bj(j)));
+        }
+        return k_inverse(f, t, batch, bj(0), E);
     }
     const int n = Ntrunc > 0 ? Ntrunc : 1;
     {   // T_n = 1 + X/n

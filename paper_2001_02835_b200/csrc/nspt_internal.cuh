@@ -78,6 +78,10 @@ cudaError_t fft_init_tables(const double* w256_re_im);
 // ---- force projection (nspt_md.cu) -------------------------------------------------------------
 // F^(k) = i c [ S^(k) - S^(k)+ - Tr(S^(k) - S^(k)+)/N ] for k < n (eq. 2.3).  F must not alias S.
 cudaError_t launch_force(const nspt_c128* S, nspt_c128* F, double c, int N, int n, cudaStream_t st);
+// Block polynomials B_j = coef[j][0] 1 + sum_{i=1}^{s-1} coef[j][i] P_i (j < r) of spectra packed back to back:
+// powers = P_1, P_2, ... (s-1 of them), polys = B_0 .. B_{r-1}; s, r <= 12.  Used by the series exponential.
+cudaError_t launch_freq_block_polys(const FreqLayout& f, int batch, const double* powers, double* polys, int s, int r,
+                                    const double* coef, cudaStream_t st);
 
 // ---- mode-wise matrix product (nspt_zgemm.cu) -----------------------------------------------
 // For all batch*L modes p, with M(p) = A~(p) B~(p):

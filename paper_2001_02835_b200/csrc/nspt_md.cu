@@ -53,7 +53,54 @@ __global__ void __launch_bounds__(256) force_kernel(const double2* __restrict__ 
     }
 }
 
+// Block polynomials of the Paterson-Stockmeyer form of exp(X) in frequency space (nspt_api.cu, series_exp_device):
+//     B_j(p) = c[j][0] 1 + sum_{i=1}^{s-1} c[j][i] P_i(p),   j = 0..r-1,
+// P_i = spectrum of the power X^{*i} (spectra `stride` doubles apart, P_1 first), B_j written `stride` apart.  One pass:
+// every element of the s-1 powers is read once and the r results are written once.
+struct PolyCoef {
+    double c[12][12];
+};
+
+__global__ void __launch_bounds__(256) freq_block_polys_kernel(const double2* __restrict__ pw, double2* __restrict__ out,
+                                                              size_t stride_c, size_t total, int N, size_t NN, int s, int r,
+                                                              const PolyCoef K) {
+    const size_t e = (size_t)blockIdx.x * 256 + threadIdx.x;   // element of one (batched) spectrum
+    if (e >= total) return;
+    const size_t el = e % NN;
+    const bool on_diag = (el / N == el % N);
+    double2 acc[12];
+#pragma unroll
+    for (int j = 0; j < 12; ++j) acc[j] = make_double2((on_diag && j < r) ? K.c[j][0] : 0.0, 0.0);
+    for (int i = 1; i < s; ++i) {
+        const double2 v = pw[(size_t)(i - 1) * stride_c + e];
+#pragma unroll
+        for (int j = 0; j < 12; ++j) {
+            if (j < r) {
+                const double w = K.c[j][i];
+                acc[j].x += w * v.x;
+                acc[j].y += w * v.y;
+            }
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 12; ++j)
+        if (j < r) out[(size_t)j * stride_c + e] = acc[j];
+}
+
 }  // namespace
+
+cudaError_t launch_freq_block_polys(const FreqLayout& f, int batch, const double* powers, double* polys, int s, int r,
+                                    const double* coef /* r x s, row-major */, cudaStream_t st) {
+    if (s < 1 || s > 12 || r < 1 || r > 12) return cudaErrorInvalidValue;
+    PolyCoef K{};
+    for (int j = 0; j < r; ++j)
+        for (int i = 0; i < s; ++i) K.c[j][i] = coef[j * s + i];
+    const size_t total = (size_t)batch * f.L * f.NN;
+    const unsigned grid = (unsigned)((total + 255) / 256);
+    freq_block_polys_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(powers), reinterpret_cast<double2*>(polys),
+                                                  total, total, f.N, f.NN, s, r, K);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_force(const nspt_c128* S, nspt_c128* F, double c, int N, int n, cudaStream_t st) {
     dim3 grid((N + 31) / 32, (N + 31) / 32, (unsigned)n);

@@ -48,6 +48,8 @@ def test_single_rank_aggregate_is_identity():
     assert ms == 3.5 and value == pytest.approx(2000.0)
     assert bench.transform_length(7) == 16 and bench.transform_length(63) == 128
     assert bench.transform_length(0) == 1 and bench.transform_length(8) == 32 and bench.transform_length(127) == 256
+    # products of the series exponential: Horner below N_trunc = 6, Paterson-Stockmeyer above
+    assert [bench.exp_products(n) for n in (0, 1, 5, 6, 31, 63, 127)] == [0, 0, 4, 4, 10, 14, 21]
 
 
 def test_reference_arm_prints_one_json_line():

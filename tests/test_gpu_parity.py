@@ -372,7 +372,8 @@ def gpu_exp(nspt, X):
     return E.cpu().numpy()
 
 
-@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (1, 1), (1, 9), (3, 2), (9, 7), (25, 15), (57, 9), (50, 20), (33, 31)])
+@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (1, 1), (1, 9), (3, 2), (4, 5), (4, 6), (9, 7), (5, 8), (25, 15), (57, 9),
+                                      (50, 20), (33, 31), (10, 35), (6, 63), (3, 127)])
 def test_series_exp_matches_oracle(nspt, N, Ntrunc):
     import oracle
     X = anti_hermitian_series(N, Ntrunc, seed=[60, N, Ntrunc])
@@ -504,7 +505,7 @@ def test_caller_workspace_for_staple_and_exp(nspt):
     X = anti_hermitian_series(9, 7, seed=83)
     need_s = nspt.nspt_workspace_bytes(9, 7, 1, nspt.NSPT_OP_STAPLE)
     need_e = nspt.nspt_workspace_bytes(9, 7, 1, nspt.NSPT_OP_SERIES_EXP)
-    assert need_s == 30 * 16 * 81 * 16 and need_e == 3 * 16 * 81 * 16       # 30 and 3 spectra of L = 16 modes
+    assert need_s == 30 * 16 * 81 * 16 and need_e == 6 * 16 * 81 * 16       # 30 and 3 + 3 spectra of L = 16 modes
     ws = torch.empty(need_s, dtype=torch.uint8, device="cuda")
     try:
         nspt.nspt_set_workspace(ws.data_ptr(), need_s)
