@@ -289,7 +289,8 @@ def run_sweep(args):
             peaks = {}
     hbm = peaks.get("hbm_gbs", 6650.0)
     W, K = max(3, args.warmup), args.steps
-    points = sorted(set(wl.sweep_points() + [(225, 31)]), key=lambda p: (p[0] != 225, p[0], p[1]))
+    # BASELINE.json configs[4] plus the paper's other matrix sizes (Table 3) at N_trunc = 31
+    points = sorted(set(wl.sweep_points() + [(225, 31), (121, 31), (169, 31), (289, 31)]), key=lambda p: (p[0] != 225, p[0], p[1]))
     rows_out = []
     launches0 = nspt.nspt_launch_count()
     sampler = ClockSampler(local).start()
@@ -358,7 +359,7 @@ def run_sweep(args):
         "ms_per_step": headline["us_per_product"] * 1e-3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "scaling sweep of A*B (BASELINE.json configs[4]): N_trunc in {7,15,31,63,127} at N=225 and N in "
-                               "{16,49,100,225,400} at N_trunc=31; value is the shared point N=225, N_trunc=31; timing inputs are "
+                               "{16,49,100,225,400} at N_trunc=31, plus the paper's other sizes N in {121,169,289}; value is the shared point N=225, N_trunc=31; timing inputs are "
                                "unitary series generated on the device with nspt_series_exp",
                    "l2": "each point rotates over buffer sets larger than 2 x L2 (up to 64 sets)"},
         "clocks": clocks, "gpu_launches": nspt.nspt_launch_count() - launches0,

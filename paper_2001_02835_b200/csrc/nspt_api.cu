@@ -768,6 +768,6 @@ const char* nspt_strerror(int code) {
     }
 }
 
-int nspt_version(void) { return 100; }
+int nspt_version(void) { return 200; }
 
 }  // extern "C"
