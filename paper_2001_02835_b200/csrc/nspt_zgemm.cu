@@ -467,10 +467,18 @@ cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup*
         if ((long long)(da / mat) > maxA) maxA = (long long)(da / mat);
         if ((long long)(db / mat) > maxB) maxB = (long long)(db / mat);
     }
-    // 48 x 48 CTA tile, 4 warps of 24 x 24, 3 CTAs per SM, 5-deep ring.  Measured alternatives on B200 at N = 225,
-    // L = 128 (331 us): 64 x 48 / 8 warps of 16 x 24 / 2 CTAs 341 us; 48 x 64 / 8 warps of 24 x 16 354 us; 32 x 48 /
-    // 4 warps / 4 CTAs 338 us; 6-deep ring 331 us; 2 CTAs with an 8-deep ring 359 us.
-    return launch_dmma<Tile<3, 3, 2, 2, 3, 5>>(f, baseA, (int)maxA + modes, baseB, (int)maxB + modes, P, st);
+    // Two tilings.  A: 48 x 48 CTA tile, 4 warps of 24 x 24, 3 CTAs per SM -- the better inner loop (6 fragment loads
+    // and 6 DADDs per 27 DMMAs); measured alternatives at N = 225, L = 128 (331 us): 64 x 48 / 8 warps of 16 x 24 / 2
+    // CTAs 341 us, 48 x 64 / 8 warps of 24 x 16 354 us, 32 x 48 / 4 warps / 4 CTAs 338 us, 6-deep ring 331 us, 2 CTAs
+    // with an 8-deep ring 359 us.  B: 32 x 32 CTA tile, 4 warps of 16 x 16, 5 CTAs per SM -- finer granularity.
+    // Which one wins is decided by how the nb = ceil(N / 8) eight-blocks of a dimension fill the last tile: A when
+    // they fill it (nb mod 6 = 0) or nearly (5), B otherwise.  Measured per product at L = 64, A vs B in us:
+    // N = 121: 67 / 48, 169: 119 / 111, 200: 172 / 156, 256: 306 / 268, 289: 449 / 430, 400: 988 / 979 (B wins);
+    // N = 144: 72 / 74, 192: 122 / 126, 225: 213 / 226, 240: 220 / 244 (A wins); the rule misses N = 184 (126 / 121).
+    const int nb = (f.N + 7) / 8;
+    if (nb % 6 == 0 || nb % 6 == 5)
+        return launch_dmma<Tile<3, 3, 2, 2, 3, 5>>(f, baseA, (int)maxA + modes, baseB, (int)maxB + modes, P, st);
+    return launch_dmma<Tile<2, 2, 2, 2, 5, 5>>(f, baseA, (int)maxA + modes, baseB, (int)maxB + modes, P, st);
 }
 
 cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out,
