@@ -472,11 +472,11 @@ cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup*
     // CTAs 341 us, 48 x 64 / 8 warps of 24 x 16 354 us, 32 x 48 / 4 warps / 4 CTAs 338 us, 6-deep ring 331 us, 2 CTAs
     // with an 8-deep ring 359 us.  B: 32 x 32 CTA tile, 4 warps of 16 x 16, 5 CTAs per SM -- finer granularity.
     // Which one wins is decided by how the nb = ceil(N / 8) eight-blocks of a dimension fill the last tile: A when
-    // they fill it (nb mod 6 = 0) or nearly (5), B otherwise.  Measured per product at L = 64, A vs B in us:
+    // they fill it (nb mod 6 = 0) or nearly (5, from nb = 29 up), B otherwise.  Measured per product at L = 64, A vs B in us:
     // N = 121: 67 / 48, 169: 119 / 111, 200: 172 / 156, 256: 306 / 268, 289: 449 / 430, 400: 988 / 979 (B wins);
-    // N = 144: 72 / 74, 192: 122 / 126, 225: 213 / 226, 240: 220 / 244 (A wins); the rule misses N = 184 (126 / 121).
+    // N = 144: 72 / 74, 192: 122 / 126, 225: 213 / 226, 240: 220 / 244 (A wins); N = 184 (nb = 23): 126 / 121, hence nb >= 29 for the 'nearly' case.
     const int nb = (f.N + 7) / 8;
-    if (nb % 6 == 0 || nb % 6 == 5)
+    if (nb % 6 == 0 || (nb % 6 == 5 && nb >= 29))
         return launch_dmma<Tile<3, 3, 2, 2, 3, 5>>(f, baseA, (int)maxA + modes, baseB, (int)maxB + modes, P, st);
     return launch_dmma<Tile<2, 2, 2, 2, 5, 5>>(f, baseA, (int)maxA + modes, baseB, (int)maxB + modes, P, st);
 }
