@@ -29,6 +29,10 @@
  * inputs are transformed into the workspace before any output is written); partial overlap
  * is undefined.  In nspt_staple S[mu] may alias U[mu] for the same reason.
  *
+ * CUDA graphs.  After one call of the same shape (which builds the plan tables and sizes the workspace) the
+ * device entry points neither allocate nor synchronise, so they can be captured into a CUDA graph on the library
+ * stream.  The large kernels are launched with programmatic stream serialization.
+ *
  * Errors.  Every call returns 0 (NSPT_OK) or a negative code; nothing throws, aborts or
  * prints.  Kernel faults are asynchronous and surface at the caller's next synchronisation.
  *

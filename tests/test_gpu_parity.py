@@ -561,3 +561,35 @@ def test_release_and_reuse(nspt):
     check_product(nspt, A, B)
     nspt.nspt_release()
     check_product(nspt, A, B)
+
+
+def test_calls_can_be_captured_in_a_cuda_graph(nspt):
+    # after one warm-up call of the same shape (plans, workspace) the device entry points neither allocate nor
+    # synchronise, so a chain of them can be captured on the library stream and replayed
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(87)
+    A, B = wl.gaussian_series(57, 15, rng), wl.gaussian_series(57, 15, rng)
+    dA, dB = to_dev(A), to_dev(B)
+    dC = torch.empty_like(dA)
+    s = torch.cuda.Stream()
+    try:
+        with torch.cuda.stream(s):
+            nspt.nspt_set_stream(s.cuda_stream)
+            nspt.nspt_series_mul(dA, dB, dC)
+            s.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=s):
+                nspt.nspt_set_stream(torch.cuda.current_stream().cuda_stream)
+                nspt.nspt_series_mul(dA, dB, dC)
+                nspt.nspt_series_mul(dC, dB, dC)
+            for _ in range(2):
+                dC.zero_()
+                graph.replay()
+            s.synchronize()
+    finally:
+        nspt.use_current_stream()
+    AB = oracle.series_mul(A, B)
+    err = oracle.per_order_error(dC.cpu().numpy(), oracle.series_mul(AB, B), oracle.product_bound(AB, B))
+    assert err.max() <= 2 * TOL
