@@ -199,9 +199,12 @@ struct InvRegs {
     double2 v[A][K2];
 };
 
-template <int R, int S, int T>
+// The twiddles w^(+-s k1), k1 < R, of a thread do not change from tile to tile: the persistent kernels load them
+// once into registers (twr) instead of once per tile from the global table (18 % of the inverse pass's warp samples
+// were waiting for those loads).  TWREG selects the register copy.
+template <int R, int S, int T, bool TWREG = false>
 __device__ __forceinline__ void inverse_from_regs(double2 (&x)[R], int s, int c, const double2* __restrict__ tw,
-                                                  double2* sm, InvRegs<R, S, T>& out) {
+                                                  double2* sm, InvRegs<R, S, T>& out, const double2* twr = nullptr) {
     double2 Y[R];
     Dft<R, -1, false, false>::run(x, Y);
     if constexpr (S == 1) {
@@ -210,7 +213,11 @@ __device__ __forceinline__ void inverse_from_regs(double2 (&x)[R], int s, int c,
     } else {
 #pragma unroll
         for (int k1 = 0; k1 < R; ++k1) {
-            const double2 w = __ldg(&tw[s * k1]);  // (the constant table measured slower here: 40 vs 34 us at L = 128)
+            double2 w;
+            if constexpr (TWREG)
+                w = twr[k1];
+            else
+                w = __ldg(&tw[s * k1]);  // (the constant table measured slower here: 40 vs 34 us at L = 128)
             sm[(k1 * S + s) * T + c] = (k1 == 0) ? Y[k1] : cmul(Y[k1], w);
         }
         __syncthreads();
@@ -346,9 +353,9 @@ __device__ __forceinline__ void tile_coords(unsigned tile, const XformParams& P,
 // Forward phases on shared memory.  Phase 1: thread s parks Y_s[p1] w_L^(s p1) at slot [s][p1]; phase 2: thread q
 // owns p1 = q + S a, reads slots [sp][p1] (all sp) and overwrites THE SAME slots with X[p1 + R p2] at [p2][p1],
 // which is the natural mode order p = p1 + R p2: the exchange buffer becomes the [mode][T] output tile in place.
-template <int R, int S, int T>
+template <int R, int S, int T, bool TWREG = false>
 __device__ __forceinline__ void forward_phase1_smem(const double2 (&x)[R], int s, int c, const double2* __restrict__ tw,
-                                                    double2* exch) {
+                                                    double2* exch, const double2* twr = nullptr) {
     double2 Y[R];
     Dft<R, +1, true, false>::run(x, Y);
 #pragma unroll
@@ -356,7 +363,9 @@ __device__ __forceinline__ void forward_phase1_smem(const double2 (&x)[R], int s
         // w_L^(s p1), s p1 < L.  Measured: the constant table wins at L = 256 (155 -> 137 us at N = 225), the
         // global table (L1/L2) at L <= 128 (L = 32: 18.9 vs 20.6 us).
         double2 w;
-        if constexpr (R * S >= 256)
+        if constexpr (TWREG)
+            w = twr[p1];
+        else if constexpr (R * S >= 256)
             w = c_tw256[(s * p1) * (256 / (R * S))];
         else
             w = __ldg(&tw[s * p1]);
@@ -414,6 +423,9 @@ __global__ void __launch_bounds__(T* S) fft_forward_tma_kernel(const __grid_cons
     }
     __syncthreads();
 
+    double2 twr[R];   // this thread's forward twiddles w_L^(s p1), loaded once
+#pragma unroll
+    for (int p1 = 0; p1 < R; ++p1) twr[p1] = __ldg(&P.tw_fwd[s * p1]);
     unsigned it = 0;
     for (unsigned tile = blockIdx.x; tile < P.total_tiles; tile += gridDim.x, ++it) {
         const int stage = it % NS;
@@ -444,7 +456,7 @@ __global__ void __launch_bounds__(T* S) fft_forward_tma_kernel(const __grid_cons
             const unsigned next = tile + NS * gridDim.x;
             if (next < P.total_tiles) issue(next, stage);
         }
-        forward_phase1_smem<R, S, T>(x, s, c, P.tw_fwd, exch);
+        forward_phase1_smem<R, S, T, true>(x, s, c, P.tw_fwd, exch, twr);
         __syncthreads();
         forward_phase2_smem<R, S, T>(s, c, exch);
         fence_proxy_async_smem();
@@ -496,6 +508,16 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
     }
     __syncthreads();
 
+    double2 twr[R];   // this thread's inverse twiddles w_L^-(s k1), loaded once
+#pragma unroll
+    for (int k1 = 0; k1 < R; ++k1) twr[k1] = __ldg(&P.tw_inv[s * k1]);
+    // re-truncation: the forward twiddles too where the register budget allows (R <= 8)
+    constexpr bool FWD_TWREG = RETRUNC && (R <= 8);
+    double2 twf[FWD_TWREG ? R : 1];
+    if constexpr (FWD_TWREG) {
+#pragma unroll
+        for (int p1 = 0; p1 < R; ++p1) twf[p1] = __ldg(&P.tw_fwd[s * p1]);
+    }
     unsigned it = 0;
     for (unsigned tile = blockIdx.x; tile < P.total_tiles; tile += gridDim.x, ++it) {
         const int stage = it % NS;
@@ -513,12 +535,12 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
             if (next < P.total_tiles) issue(next, stage);
         }
         InvRegs<R, S, T> q;
-        inverse_from_regs<R, S, T>(x, s, c, P.tw_inv, exch, q);
+        inverse_from_regs<R, S, T, true>(x, s, c, P.tw_inv, exch, q, twr);
         if constexpr (RETRUNC) {
             double2 xf[R];
             retruncate_regs<R, S, T>(q, s, P.n, P.inv_L, xf);
             __syncthreads();  // phase-2 reads of the inverse are done
-            forward_phase1_smem<R, S, T>(xf, s, c, P.tw_fwd, exch);
+            forward_phase1_smem<R, S, T, FWD_TWREG>(xf, s, c, P.tw_fwd, exch, twf);
             __syncthreads();
             forward_phase2_smem<R, S, T>(s, c, exch);
             fence_proxy_async_smem();
