@@ -387,7 +387,7 @@ __device__ __forceinline__ void forward_phase2_smem(int s, int c, double2* exch)
 }
 
 template <int R, int S, int T>
-__global__ void __launch_bounds__(T* S) fft_forward_tma_kernel(const __grid_constant__ CUtensorMap in0,
+__global__ void __launch_bounds__(T* S, 1) fft_forward_tma_kernel(const __grid_constant__ CUtensorMap in0,
                                                               const __grid_constant__ CUtensorMap in1,
                                                               const __grid_constant__ CUtensorMap out0,
                                                               const __grid_constant__ CUtensorMap out1,
