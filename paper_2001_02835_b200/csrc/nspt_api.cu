@@ -32,7 +32,6 @@ struct Context {
     double order_scale = 1.0;
     int gemm_variant = 1;
     bool arch_checked = false;
-    bool tables_ready = false;
     // workspace
     void* user_ws = nullptr;
     size_t user_ws_bytes = 0;
@@ -95,22 +94,6 @@ int get_plan(int L, int n, double s, PlanTables* out) {
             *out = PlanTables{p.tw_fwd, p.tw_inv, p.scale_in, p.scale_out, 1.0 / L};
             return NSPT_OK;
         }
-    }
-    if (!g.tables_ready) {
-        std::vector<double> w(512);
-        const long double two_pi256 = 6.283185307179586476925286766559005768L / 256.0L;
-        for (int m = 0; m < 256; ++m) {
-            double c = (double)cosl(two_pi256 * m), sn = (double)sinl(two_pi256 * m);
-            if (m % 64 == 0) {  // multiples of pi/2 are exact
-                const int q = m / 64;
-                c = (q == 0) ? 1.0 : (q == 2 ? -1.0 : 0.0);
-                sn = (q == 1) ? 1.0 : (q == 3 ? -1.0 : 0.0);
-            }
-            w[2 * m] = c;
-            w[2 * m + 1] = sn;
-        }
-        NSPT_CUDA(fft_init_tables(w.data()));
-        g.tables_ready = true;
     }
     Plan p;
     p.L = L;

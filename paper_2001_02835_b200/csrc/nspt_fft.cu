@@ -61,10 +61,6 @@ __host__ __device__ constexpr double c16(int m) {
 }
 __host__ __device__ constexpr double s16(int m) { return c16((m + 12) & 15); }  // sin x = cos(x - pi/2)
 
-// w_256^m = exp(+2 pi i m / 256), m < 256, in constant memory (filled by fft_init_tables from the host's long
-// double values), used by the forward phase of the L = 256 kernels (see forward_phase1_smem).
-__constant__ double2 c_tw256[256];
-
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ double2 cmul(double2 a, double2 w) {
@@ -217,7 +213,7 @@ __device__ __forceinline__ void inverse_from_regs(double2 (&x)[R], int s, int c,
             if constexpr (TWREG)
                 w = twr[k1];
             else
-                w = __ldg(&tw[s * k1]);  // (the constant table measured slower here: 40 vs 34 us at L = 128)
+                w = __ldg(&tw[s * k1]);
             sm[(k1 * S + s) * T + c] = (k1 == 0) ? Y[k1] : cmul(Y[k1], w);
         }
         __syncthreads();
@@ -360,13 +356,10 @@ __device__ __forceinline__ void forward_phase1_smem(const double2 (&x)[R], int s
     Dft<R, +1, true, false>::run(x, Y);
 #pragma unroll
     for (int p1 = 0; p1 < R; ++p1) {
-        // w_L^(s p1), s p1 < L.  Measured: the constant table wins at L = 256 (155 -> 137 us at N = 225), the
-        // global table (L1/L2) at L <= 128 (L = 32: 18.9 vs 20.6 us).
+        // w_L^(s p1), s p1 < L: from the thread's register copy in the persistent kernels, else from the global table
         double2 w;
         if constexpr (TWREG)
             w = twr[p1];
-        else if constexpr (R * S >= 256)
-            w = c_tw256[(s * p1) * (256 / (R * S))];
         else
             w = __ldg(&tw[s * p1]);
         exch[(s * R + p1) * T + c] = (p1 == 0) ? Y[p1] : cmul(Y[p1], w);
@@ -744,10 +737,6 @@ XformParams base_params(const FreqLayout& f, const PlanTables& t, int batch) {
 }  // namespace
 
 bool fft_length_supported(int L) { return L >= 1 && L <= 256 && (L & (L - 1)) == 0; }
-
-cudaError_t fft_init_tables(const double* w256_re_im) {
-    return cudaMemcpyToSymbol(c_tw256, w256_re_im, sizeof(double2) * 256);
-}
 
 cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int batch, const nspt_c128* src0,
                                double* dst0, const nspt_c128* src1, double* dst1, cudaStream_t st, bool skip_order0) {

@@ -72,8 +72,6 @@ cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src
 cudaError_t launch_freq_scale_identity(const FreqLayout& f, int batch, const double* src, double* dst, double alpha,
                                        cudaStream_t st);
 bool fft_length_supported(int L);
-// Upload w_256^m = exp(2 pi i m/256), m < 256 (interleaved re, im) to the kernels' constant table; once per process.
-cudaError_t fft_init_tables(const double* w256_re_im);
 
 // ---- force projection (nspt_md.cu) -------------------------------------------------------------
 // F^(k) = i c [ S^(k) - S^(k)+ - Tr(S^(k) - S^(k)+)/N ] for k < n (eq. 2.3).  F must not alias S.
