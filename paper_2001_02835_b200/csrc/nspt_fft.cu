@@ -504,6 +504,17 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
     double2 twr[R];   // this thread's inverse twiddles w_L^-(s k1), loaded once
 #pragma unroll
     for (int k1 = 0; k1 < R; ++k1) twr[k1] = __ldg(&P.tw_inv[s * k1]);
+    // the output scales s^-k / L of the orders this thread stores (plain inverse), loaded once as well
+    double sco[InvRegs<R, S, T>::A][InvRegs<R, S, T>::K2];
+    if constexpr (!RETRUNC) {
+#pragma unroll
+        for (int a = 0; a < InvRegs<R, S, T>::A; ++a)
+#pragma unroll
+            for (int k2 = 0; k2 < InvRegs<R, S, T>::K2; ++k2) {
+                const int k = (s + S * a) + R * k2;
+                sco[a][k2] = (k < P.n) ? __ldg(&P.scale_out[k]) : 0.0;
+            }
+    }
     // re-truncation: the forward twiddles too where the register budget allows (R <= 8)
     constexpr bool FWD_TWREG = RETRUNC && (R <= 8);
     double2 twf[FWD_TWREG ? R : 1];
@@ -550,7 +561,7 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
                 for (int k2 = 0; k2 < InvRegs<R, S, T>::K2; ++k2) {
                     const int k = (s + S * a) + R * k2;
                     if (k < P.n) {
-                        const double sc = __ldg(&P.scale_out[k]);  // s^-k / L
+                        const double sc = sco[a][k2];  // s^-k / L
                         outb[k * T + c] = make_double2(q.v[a][k2].x * sc, q.v[a][k2].y * sc);
                     }
                 }
