@@ -588,7 +588,8 @@ def run_cuda(args):
         e2e_value, _ = aggregate_throughput(Ke * products_per_step, dt_ms, world, dev)
         e2e = {"value": e2e_value, "unit": f"{units_name}/s", "h2d_bytes_per_step": 2 * series_bytes,
                "d2h_bytes_per_step": series_bytes, "steps": Ke,
-               "how": "nspt_series_mul_host with pinned host buffers; wall clock around synchronous calls"}
+               "how": ("nspt_series_mul_batched_host" if kind == "batched" else "nspt_series_mul_host") +
+                      " with pinned host buffers; wall clock around synchronous calls"}
     elif kind == "staple":
         hU = [torch.from_numpy(u).pin_memory() for u in inp["U"]]
         hS = [torch.empty_like(u).pin_memory() for u in hU]
