@@ -106,6 +106,5 @@ struct GemmGroup {
 };
 cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup* groups, int ngroups, int variant,
                                 cudaStream_t st);
-cudaError_t zgemm_init();   // resolves the driver entry point for tensor maps
 
 }  // namespace nspt

@@ -385,8 +385,6 @@ cudaError_t tma_encode_f64(CUtensorMap* map, const void* base, int rank, const u
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-cudaError_t zgemm_init() { return cudaSuccess; }
-
 namespace {
 
 template <class TC>
