@@ -540,3 +540,39 @@ def test_force_matches_scalar_loops():
             for j in range(N):
                 d = complex(S[k, i, j]) - complex(S[k, j, i]).conjugate() - (tr / N if i == j else 0)
                 assert abs(F[k, i, j] - 1j * c * d) < 1e-15
+
+
+def test_staple_is_covariant_under_a_constant_gauge_rotation():
+    # eq. 2.3 is built from products U ... U^+ only, so U_mu -> W U_mu W^+ with one constant unitary W maps
+    # S_mu -> W S_mu W^+ order by order: a structural check of the staple (operand order, daggers) at once
+    rng = np.random.default_rng(76)
+    N, Ntrunc = 4, 3
+    U = [wl.unitary_series(N, Ntrunc, rng) for _ in range(4)]
+    z = wl.twist_tensor(2, 1)
+    H = wl.hermitian_traceless(N, rng)
+    evals, V = np.linalg.eigh(H)
+    W = (V * np.exp(1j * evals)) @ V.conj().T
+    assert np.abs(W @ W.conj().T - np.eye(N)).max() < 1e-14
+    rot = lambda X: np.einsum("ab,kbc,dc->kad", W, X, W.conj())
+    S = oracle.staple(U, z)
+    Sr = oracle.staple([rot(u) for u in U], z)
+    for mu in range(4):
+        assert np.abs(Sr[mu] - rot(S[mu])).max() < 1e-12
+
+
+def test_exp_of_a_sum_of_commuting_series_factorises():
+    # X and Y polynomials in one matrix commute, so exp(X + Y) = exp(X) * exp(Y) order by order
+    rng = np.random.default_rng(77)
+    N, n = 5, 8
+    M = 0.4 * (rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N)))
+    P = [np.eye(N, dtype=np.complex128)]
+    for _ in range(3):
+        P.append(P[-1] @ M)
+    X = np.zeros((n, N, N), dtype=np.complex128)
+    Y = np.zeros((n, N, N), dtype=np.complex128)
+    for k in range(1, n):
+        X[k] = rng.standard_normal() * P[1] + rng.standard_normal() * P[2]
+        Y[k] = rng.standard_normal() * P[0] + rng.standard_normal() * P[3]
+    lhs = oracle.series_exp(X + Y)
+    rhs = oracle.series_mul(oracle.series_exp(X), oracle.series_exp(Y))
+    assert oracle.per_order_error(lhs, rhs, oracle.exp_bound(X + Y)).max() < 1e-13
