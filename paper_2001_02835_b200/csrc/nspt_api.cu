@@ -152,14 +152,18 @@ void exp_split(int Ntrunc, int* s, int* r) {
     *r = (Ntrunc + 1 + q - 1) / q;           // <= 12
 }
 
+// The B-operand tensor map of the mode-wise product reads up to 112 bytes past the last row of the last spectrum (its
+// last 128-byte chunk of a row runs into what follows, nspt_zgemm.cu), so every workspace ends with a 256-byte pad.
+constexpr size_t WS_PAD = 256;
+
 size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
-    if (op == NSPT_OP_STAPLE) return 30 * spectrum_bytes(f, 1);
+    if (op == NSPT_OP_STAPLE) return 30 * spectrum_bytes(f, 1) + WS_PAD;
     if (op == NSPT_OP_SERIES_EXP) {
         int s, r;
         exp_split(f.n - 1, &s, &r);
-        return (size_t)(s ? s + r : 3) * spectrum_bytes(f, batch);
+        return (size_t)(s ? s + r : 3) * spectrum_bytes(f, batch) + WS_PAD;
     }
-    return 3 * spectrum_bytes(f, batch);
+    return 3 * spectrum_bytes(f, batch) + WS_PAD;
 }
 
 int get_workspace(size_t bytes, char** out) {

@@ -22,7 +22,8 @@
 //
 // Shared-memory layout: every operand row is 8 complex128 = 128 bytes, written by TMA with
 // SWIZZLE_128B (16-byte chunk index XOR row index mod 8).  A slice: [m 0..47][k 0..7]; B slice: six
-// boxes [k 0..7][n 0..7].  Lane (g = lane/4, t = lane%4) loads one complex element (re, im) per
+// blocks [k 0..7][n 0..7], fetched by ONE box of a 4-D view of the operand (encode_operand_b4; seven TMA
+// instructions per slice instead of two cost 2.4 % of the kernel).  Lane (g = lane/4, t = lane%4) loads one complex element (re, im) per
 // fragment with a 16-byte ld.shared; a slice is consumed as two k4 sub-steps whose k-slots are
 // {0,2,4,6} and {1,3,5,7} (any k permutation is legal as long as A and B agree), which makes the
 // eight lanes of every quarter-warp hit eight different 16-byte chunks: no bank conflicts.
@@ -98,9 +99,7 @@ __device__ __forceinline__ void issue_slice(const CUtensorMap* mapA, const CUten
                                             uint32_t full_bar, int k0, int m0, int n0, int modeA, int modeB) {
     mbar_expect_tx(full_bar, TC::STAGE_BYTES);
     tma_load_3d(stage_addr, mapA, full_bar, 2 * k0, m0, modeA);
-#pragma unroll
-    for (int c = 0; c < TC::BN / 8; ++c)
-        tma_load_3d(stage_addr + TC::A_STAGE_BYTES + c * B_BOX_BYTES, mapB, full_bar, 2 * (n0 + 8 * c), k0, modeB);
+    tma_load_4d(stage_addr + TC::A_STAGE_BYTES, mapB, full_bar, 0, k0, n0 / 8, modeB);
 }
 
 template <class TC, bool FULL>
@@ -352,6 +351,17 @@ zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict_
 
 // 3-D view of a spectrum as doubles: (2N doubles per row, N rows, modes); boxes are 16 doubles wide
 // (8 complex = 128 bytes, the swizzle span).
+// B operand as (16 doubles of one 128-byte chunk, N rows, ceil(2N/16) chunks per row, modes): one box (16, 8, BN/8, 1)
+// brings the BN/8 chunk columns of a K-slice with ONE instruction, laid out [chunk][k][8 complex] exactly like BN/8
+// separate boxes.  The last chunk of a row runs into the next row (columns >= N of the tile hold garbage that only
+// reaches output columns >= N, which are never stored); the caller's buffer must extend 128 bytes past the last row.
+cudaError_t encode_operand_b4(CUtensorMap* map, const double* basep, const FreqLayout& f, int modes, int chunks_box) {
+    const uint64_t dims[4] = {16, (uint64_t)f.N, (uint64_t)((2 * f.N + 15) / 16), (uint64_t)modes};
+    const uint64_t strides[3] = {(uint64_t)f.N * 16, 128, (uint64_t)f.NN * 16};
+    const uint32_t box[4] = {16, (uint32_t)BK, (uint32_t)chunks_box, 1};
+    return tma_encode_f64(map, basep, 4, dims, strides, box, true);
+}
+
 cudaError_t encode_operand(CUtensorMap* map, const double* basep, const FreqLayout& f, int modes, int box_rows) {
     const uint64_t dims[3] = {(uint64_t)(2 * f.N), (uint64_t)f.N, (uint64_t)modes};
     const uint64_t strides[2] = {(uint64_t)f.N * 16, (uint64_t)f.NN * 16};
@@ -371,8 +381,8 @@ cudaError_t tma_encode_f64(CUtensorMap* map, const void* base, int rank, const u
         if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
         g_encode = reinterpret_cast<EncodeTiledFn>(fn);
     }
-    cuuint64_t d[3] = {1, 1, 1}, st[2] = {16, 16};
-    cuuint32_t bx[3] = {1, 1, 1}, es[3] = {1, 1, 1};
+    cuuint64_t d[4] = {1, 1, 1, 1}, st[3] = {16, 16, 16};
+    cuuint32_t bx[4] = {1, 1, 1, 1}, es[4] = {1, 1, 1, 1};
     for (int i = 0; i < rank; ++i) {
         d[i] = dims[i];
         bx[i] = box[i];
@@ -401,7 +411,7 @@ cudaError_t launch_dmma(const FreqLayout& f, const double* baseA, int modesA, co
     P.tiles_n = (f.N + TC::BN - 1) / TC::BN;
     CUtensorMap mapA, mapB;
     if ((e = encode_operand(&mapA, baseA, f, modesA, TC::BM)) != cudaSuccess) return e;
-    if ((e = encode_operand(&mapB, baseB, f, modesB, BK)) != cudaSuccess) return e;
+    if ((e = encode_operand_b4(&mapB, baseB, f, modesB, TC::BN / 8)) != cudaSuccess) return e;
     const unsigned grid = (unsigned)(P.ngroups * P.nmodes * P.tiles_m * P.tiles_n);
     return launch_pdl(zgemm_modes_dmma_kernel<TC>, grid, TC::THREADS, TC::SMEM_BYTES, st, mapA, mapB, P);
 }

@@ -505,7 +505,7 @@ def test_caller_workspace_for_staple_and_exp(nspt):
     X = anti_hermitian_series(9, 7, seed=83)
     need_s = nspt.nspt_workspace_bytes(9, 7, 1, nspt.NSPT_OP_STAPLE)
     need_e = nspt.nspt_workspace_bytes(9, 7, 1, nspt.NSPT_OP_SERIES_EXP)
-    assert need_s == 30 * 16 * 81 * 16 and need_e == 6 * 16 * 81 * 16       # 30 and 3 + 3 spectra of L = 16 modes
+    assert need_s == 30 * 16 * 81 * 16 + 256 and need_e == 6 * 16 * 81 * 16 + 256   # 30 and 3 + 3 spectra of L = 16 modes, + pad
     ws = torch.empty(need_s, dtype=torch.uint8, device="cuda")
     try:
         nspt.nspt_set_workspace(ws.data_ptr(), need_s)
