@@ -96,6 +96,16 @@ def _dev_series(x, name):
     return x
 
 
+def _match(x, ref, name):
+    """Every operand and output of a call must have the shape of the first one (the C ABI takes N, Ntrunc and batch
+    once and cannot see a short buffer), and, for device tensors, live on the same device."""
+    if tuple(x.shape) != tuple(ref.shape):
+        raise ValueError(f"{name}: shape {tuple(x.shape)} does not match {tuple(ref.shape)}")
+    if getattr(ref, "is_cuda", False) and x.device != ref.device:
+        raise ValueError(f"{name}: on {x.device}, expected {ref.device}")
+    return x
+
+
 def _shape(x, batched):
     if batched:
         if x.ndim != 4 or x.shape[2] != x.shape[3]:
@@ -122,7 +132,8 @@ def nspt_series_mul(A, B, C=None):
     _, Ntrunc, N = _shape(A, False)
     if C is None:
         C = torch.empty_like(A)
-    _dev_series(C, "C")
+    _match(_dev_series(B, "B"), A, "B")
+    _match(_dev_series(C, "C"), A, "C")
     _check(_lib.nspt_series_mul(A.data_ptr(), B.data_ptr(), C.data_ptr(), N, Ntrunc), "nspt_series_mul")
     return C
 
@@ -135,7 +146,8 @@ def nspt_series_mul_batched(A, B, C=None):
     batch, Ntrunc, N = _shape(A, True)
     if C is None:
         C = torch.empty_like(A)
-    _dev_series(C, "C")
+    _match(_dev_series(B, "B"), A, "B")
+    _match(_dev_series(C, "C"), A, "C")
     _check(_lib.nspt_series_mul_batched(A.data_ptr(), B.data_ptr(), C.data_ptr(), N, Ntrunc, batch),
            "nspt_series_mul_batched")
     return C
@@ -156,6 +168,12 @@ def nspt_staple(U, z, S=None):
     if S is None:
         S = [torch.empty_like(u) for u in U]
     S = [_dev_series(s, "S") for s in S]
+    if len(S) != 4:
+        raise ValueError("four staple series expected")
+    for t in U[1:]:
+        _match(t, U[0], "U")
+    for t in S:
+        _match(t, U[0], "S")
     zz = _z_array(z)
     Up = (_vp * 4)(*[u.data_ptr() for u in U])
     Sp = (_vp * 4)(*[s.data_ptr() for s in S])
@@ -170,7 +188,7 @@ def nspt_series_exp(X, E=None):
     _, Ntrunc, N = _shape(X, False)
     if E is None:
         E = torch.empty_like(X)
-    _dev_series(E, "E")
+    _match(_dev_series(E, "E"), X, "E")
     _check(_lib.nspt_series_exp(X.data_ptr(), E.data_ptr(), N, Ntrunc), "nspt_series_exp")
     return E
 
@@ -182,7 +200,7 @@ def nspt_series_exp_batched(X, E=None):
     batch, Ntrunc, N = _shape(X, True)
     if E is None:
         E = torch.empty_like(X)
-    _dev_series(E, "E")
+    _match(_dev_series(E, "E"), X, "E")
     _check(_lib.nspt_series_exp_batched(X.data_ptr(), E.data_ptr(), N, Ntrunc, batch), "nspt_series_exp_batched")
     return E
 
@@ -194,7 +212,7 @@ def nspt_force(S, c: float, F=None):
     _, Ntrunc, N = _shape(S, False)
     if F is None:
         F = torch.empty_like(S)
-    _dev_series(F, "F")
+    _match(_dev_series(F, "F"), S, "F")
     _check(_lib.nspt_force(S.data_ptr(), F.data_ptr(), float(c), N, Ntrunc), "nspt_force")
     return F
 
@@ -217,6 +235,8 @@ def _host_ptr(x, name):
 
 def nspt_series_mul_host(A, B, C):
     _, Ntrunc, N = _shape(A, False)
+    _match(B, A, "B")
+    _match(C, A, "C")
     pa, _a = _host_ptr(A, "A")
     pb, _b = _host_ptr(B, "B")
     pc, _c = _host_ptr(C, "C")
@@ -226,6 +246,8 @@ def nspt_series_mul_host(A, B, C):
 
 def nspt_series_mul_batched_host(A, B, C):
     batch, Ntrunc, N = _shape(A, True)
+    _match(B, A, "B")
+    _match(C, A, "C")
     pa, _a = _host_ptr(A, "A")
     pb, _b = _host_ptr(B, "B")
     pc, _c = _host_ptr(C, "C")
@@ -234,7 +256,11 @@ def nspt_series_mul_batched_host(A, B, C):
 
 
 def nspt_staple_host(U, z, S):
+    if len(U) != 4 or len(S) != 4:
+        raise ValueError("four link series and four staple series expected")
     _, Ntrunc, N = _shape(U[0], False)
+    for t in list(U[1:]) + list(S):
+        _match(t, U[0], "U/S")
     up = [_host_ptr(u, "U") for u in U]
     sp = [_host_ptr(s, "S") for s in S]
     zz = _z_array(z)

@@ -82,3 +82,24 @@ def test_product_path_has_no_cpu_fallback():
         assert not imp2.search(f.read_text()), f"{f} imports the CUDA package"
     assert "include" not in (ROOT / "oracle" / "nspt_oracle.c").read_text().split("*/", 1)[1].replace(
         "#include <stdlib.h>", "").replace("#include <string.h>", "").replace("#include <omp.h>", "")
+
+
+def test_binding_rejects_mismatched_host_operands():
+    # the C ABI takes N, Ntrunc and batch once; a short second operand or output would be overrun silently, so the
+    # wrappers check every array before the call (no CUDA call is reached here)
+    import numpy as np
+    from paper_2001_02835_b200 import binding
+    A = np.zeros((4, 3, 3), dtype=np.complex128)
+    small = np.zeros((3, 3, 3), dtype=np.complex128)
+    with pytest.raises(ValueError):
+        binding.nspt_series_mul_host(A, A, small)
+    with pytest.raises(ValueError):
+        binding.nspt_series_mul_host(A, small, A)
+    with pytest.raises(ValueError):
+        binding.nspt_series_mul_batched_host(A[None], A[None], small[None])
+    with pytest.raises(ValueError):
+        binding.nspt_staple_host([A, A, A, small], np.ones((4, 4)), [A, A, A, A])
+    with pytest.raises(ValueError):
+        binding.nspt_staple_host([A, A, A, A], np.ones((4, 4)), [A, A, small, A])
+    with pytest.raises(ValueError):
+        binding.nspt_staple_host([A, A, A], np.ones((4, 4)), [A, A, A])

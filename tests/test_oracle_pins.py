@@ -576,3 +576,27 @@ def test_exp_of_a_sum_of_commuting_series_factorises():
     lhs = oracle.series_exp(X + Y)
     rhs = oracle.series_mul(oracle.series_exp(X), oracle.series_exp(Y))
     assert oracle.per_order_error(lhs, rhs, oracle.exp_bound(X + Y)).max() < 1e-13
+
+
+# ----------------------------------------------------------------------------- tolerance denominators, by hand
+
+def test_staple_bound_by_hand_two_orders():
+    # reading c12 with 1 x 1 "matrices" so that Frobenius norms are absolute values: a = (1, 2, 1, 3) at order 0,
+    # b = (2, 1, 1, 0) at order 1.  (u_nu * u_mu * u_nu)_0 = a_nu^2 a_mu, (..)_1 = 2 a_nu b_nu a_mu + a_nu^2 b_mu;
+    # acc = 2 * sum over nu != mu; bound = u_mu * acc.
+    #   mu = 0: acc = (2*14*1, 2*[(4+8)+(2+2)+(0+18)]) = (28, 68)  ->  bound = (28, 1*68 + 2*28) = (28, 124)
+    #   mu = 3: acc = (2*6*3, 2*(12+12+6)) = (36, 60)              ->  bound = (108, 3*60 + 0*36) = (108, 180)
+    U = [np.array([[[1.0]], [[-2.0j]]]), np.array([[[2.0j]], [[1.0]]]), np.array([[[-1.0]], [[1.0j]]]),
+         np.array([[[3.0]], [[0.0]]])]
+    b = oracle.staple_bound([u.astype(np.complex128) for u in U])
+    assert np.array_equal(b[0], [28.0, 124.0])
+    assert np.array_equal(b[3], [108.0, 180.0])
+
+
+def test_exp_bound_by_hand_three_orders():
+    # x = (0, 3, 4) -> exp(x) = 1 + 3 g + (4 + 9/2) g^2; the order-0 entry is sqrt(N) for the identity
+    X = np.zeros((3, 2, 2), dtype=np.complex128)
+    X[1, 0, 0] = 3.0
+    X[2, 0, 1] = 4.0j
+    e = oracle.exp_bound(X)
+    assert np.allclose(e, [np.sqrt(2.0), 3.0, 8.5], rtol=0, atol=1e-15)
