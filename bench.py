@@ -394,7 +394,7 @@ def run_cuda(args):
     stream = torch.cuda.Stream(device=dev)
     nspt.nspt_set_stream(stream.cuda_stream)
     nspt.nspt_set_order_scale(1.0)
-    nspt.nspt_set_gemm_variant(1)
+    nspt.nspt_set_gemm_variant(args.gemm_variant)
 
     series_bytes = n * N * N * 16 * batch
     with torch.cuda.stream(stream):
@@ -674,6 +674,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--gemm-variant", type=int, default=1, choices=[1, 2],
+                    help="mode-wise product kernel: 1 = FP64 tensor pipe (DMMA, default), 2 = INT8 tensor cores (tcgen05, Ozaki slicing)")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = args.steps if args.steps is not None else 5

@@ -157,6 +157,7 @@ void exp_split(int Ntrunc, int* s, int* r) {
 constexpr size_t WS_PAD = 256;
 
 size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
+    if (op == NSPT_OP_SERIES_MUL && g.gemm_variant == 2) return 3 * spectrum_bytes(f, batch) + WS_PAD + ozaki_workspace_bytes(f, batch);
     if (op == NSPT_OP_STAPLE) return 30 * spectrum_bytes(f, 1) + WS_PAD;
     if (op == NSPT_OP_SERIES_EXP) {
         int s, r;
@@ -282,13 +283,13 @@ int k_dagger(const FreqLayout& f, int batch, const double* src, double* dst) {
 int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_GEMM));
-    NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, out, g.gemm_variant, g.stream));
+    NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, out, g.gemm_variant == 2 ? 1 : g.gemm_variant, g.stream));
     return tm.end();
 }
 int k_gemm_groups(const FreqLayout& f, const GemmGroup* groups, int ngroups, int batch = 1) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_GEMM));
-    NSPT_CUDA(launch_zgemm_groups(f, batch, groups, ngroups, g.gemm_variant, g.stream));
+    NSPT_CUDA(launch_zgemm_groups(f, batch, groups, ngroups, g.gemm_variant == 2 ? 1 : g.gemm_variant, g.stream));
     return tm.end();
 }
 int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, double* C) {
@@ -315,7 +316,21 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
     // Steps 1-2 (eqs. 2.6-2.7): zero-padded forward transforms of A and B, one launch
     NSPT_TRY(k_forward(f, t, batch, A, At, B, Bt));
     // Step 3 (eq. 2.8): mode-wise matrix products
-    NSPT_TRY(k_gemm(f, batch, At, Bt, Ct));
+    if (g.gemm_variant == 2) {
+        void* oz = ws + 3 * sb + WS_PAD;
+        {
+            StageTimer tm;
+            NSPT_TRY(tm.begin(ST_OTHER));
+            NSPT_CUDA(launch_ozaki_slice(f, batch, At, Bt, oz, g.stream));
+            NSPT_TRY(tm.end());
+        }
+        StageTimer tm;
+        NSPT_TRY(tm.begin(ST_GEMM));
+        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream));
+        NSPT_TRY(tm.end());
+    } else {
+        NSPT_TRY(k_gemm(f, batch, At, Bt, Ct));
+    }
     // Steps 4-5 (eq. 2.9): inverse transform, 1/L, truncation
     NSPT_TRY(k_inverse(f, t, batch, Ct, C));
     return NSPT_OK;
@@ -682,7 +697,7 @@ int nspt_set_workspace(void* dptr, size_t bytes) {
 
 int nspt_set_gemm_variant(int variant) {
     std::lock_guard<std::mutex> lk(g.mu);
-    if (variant != 0 && variant != 1) return NSPT_EINVAL;
+    if (variant != 0 && variant != 1 && variant != 2) return NSPT_EINVAL;
     g.gemm_variant = variant;
     return NSPT_OK;
 }

@@ -107,4 +107,11 @@ struct GemmGroup {
 cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup* groups, int ngroups, int variant,
                                 cudaStream_t st);
 
+// ---- mode-wise matrix product on the INT8 tensor cores (nspt_ozaki.cu; gemm variant 2) -------------------------
+// Plain C~(p) = A~(p) B~(p) only (no alpha / accumulate / dagger epilogues): FP64 spectra are cut into int8 slices
+// (launch_ozaki_slice), multiplied exactly by tcgen05.mma.kind::i8 and recombined in FP64 (launch_ozaki_gemm).
+size_t ozaki_workspace_bytes(const FreqLayout& f, int batch);
+cudaError_t launch_ozaki_slice(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st);
+cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st);
+
 }  // namespace nspt

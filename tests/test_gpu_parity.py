@@ -116,6 +116,49 @@ def test_reference_variant_agrees_with_tensor_core_variant(nspt):
     assert e0 < 1e-13 and e1 < 1e-13
 
 
+# ----------------------------------------------------------------------------- gemm variant 2: INT8 tensor cores (Ozaki)
+
+@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (3, 2), (9, 7), (31, 4), (50, 12), (64, 15), (65, 3), (100, 31), (129, 3), (225, 7),
+                                      (33, 63)])
+def test_int8_sliced_product_matches_oracle(nspt, N, Ntrunc):
+    # the mode-wise product on tcgen05.mma.kind::i8 with exact INT32 accumulation of seven int8 slices
+    # per operand plane; same tolerance as the FP64 tensor-pipe kernel
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([3, N, Ntrunc])
+    A = wl.gaussian_series(N, Ntrunc, rng)
+    B = wl.gaussian_series(N, Ntrunc, rng)
+    nspt.nspt_set_gemm_variant(2)
+    try:
+        check_product(nspt, A, B)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+
+
+def test_int8_sliced_product_integer_bit_exact(nspt):
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([4, 70, 7])
+    A = wl.integer_series(70, 7, rng)
+    B = wl.integer_series(70, 7, rng)
+    ref = oracle.series_mul(A, B)
+    nspt.nspt_set_gemm_variant(2)
+    try:
+        got = gpu_mul(nspt, A, B)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+    assert np.array_equal(np.round(got.real), ref.real) and np.array_equal(np.round(got.imag), ref.imag)
+
+
+def test_int8_sliced_product_at_config2(nspt):
+    from paper_2001_02835_b200 import workloads as wl
+    A, B = wl.config_product(225, 31, seed=2)
+    nspt.nspt_set_gemm_variant(2)
+    try:
+        check_product(nspt, A, B)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+
+
 def test_unit_and_zero(nspt):
     from paper_2001_02835_b200 import workloads as wl
     rng = np.random.default_rng(3)
