@@ -36,8 +36,18 @@
  * Errors.  Every call returns 0 (NSPT_OK) or a negative code; nothing throws, aborts or
  * prints.  Kernel faults are asynchronous and surface at the caller's next synchronisation.
  *
- * Threads.  The library has one process-wide context guarded by a mutex; calls from several
- * host threads are serialised.
+ * Devices and threads.  The library keeps one context per CUDA device (plan tables, workspace, staging, stream,
+ * order scale), selected by the device that is current at the call (cudaGetDevice) and guarded by a mutex: calls for the
+ * same device are serialised, calls for different devices (e.g. one direction of the TEK model per GPU)
+ * run independently.  nspt_set_stream / nspt_set_order_scale / nspt_set_workspace apply to the current device only.
+ * All calls of one device share one workspace: when nspt_set_stream switches streams, work queued on the new stream
+ * is ordered after the work already queued on the old one (an event), so two streams never overlap inside the library.
+ *
+ * Allocation.  The library-owned workspace and staging buffers grow on demand: the FIRST call of a larger shape
+ * synchronises the library stream, frees and reallocates (cudaMalloc); every later call of that or a smaller shape is
+ * asynchronous and allocation-free.  Pass a workspace (nspt_set_workspace) to rule this out.
+ *
+ * Diagnostics (kernel selection, per-stage timing, FP64 peak probe, launch counter) live in nspt_debug.h.
  * ---------------------------------------------------------------------------------------
  */
 #ifndef NSPT_H
@@ -53,7 +63,7 @@ typedef struct { double re, im; } nspt_c128;
 
 enum {
     NSPT_OK = 0,
-    NSPT_EINVAL = -1,  /* null / misaligned pointer, N < 1, Ntrunc < 0, batch < 1, transform length > 256 */
+    NSPT_EINVAL = -1,  /* null / misaligned pointer, N < 1, Ntrunc < 0, batch < 1, Ntrunc > NSPT_MAX_NTRUNC */
     NSPT_ENOMEM = -2,  /* device or host allocation failed, or caller workspace too small */
     NSPT_ECUDA = -3,   /* CUDA runtime / launch error (text: nspt_strerror) */
     NSPT_EARCH = -4    /* current device is not compute capability 10.x */
@@ -148,27 +158,6 @@ int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out);
 /* Give the library a caller-owned device workspace (256-byte aligned).  Calls that need more
  * return NSPT_ENOMEM.  Pass (NULL, 0) to go back to the library-owned, grow-only workspace. */
 int nspt_set_workspace(void* dptr, size_t bytes);
-
-/* Select the mode-wise matrix product kernel: 0 = reference kernel (one thread per output
- * element, plain double FMAs; for debugging), 1 = tensor-core kernel (DMMA, TMA-fed,
- * 3-multiplication complex product; default). */
-int nspt_set_gemm_variant(int variant);
-
-/* Per-stage device timing.  After nspt_profile(1) every kernel the library launches is
- * bracketed by CUDA events on the library stream; nspt_profile_read synchronises the stream,
- * and for stage = 0 forward transforms, 1 mode-wise matrix products, 2 inverse transforms,
- * 3 re-truncation transforms, 4 other (dagger / copies) returns the summed milliseconds and
- * the number of launches since the last read, then resets the counters. */
-int nspt_profile(int enable);
-int nspt_profile_read(int stage, double* ms, long long* launches);
-
-/* Measure the FP64 tensor-pipe peak of the current device (TFLOP/s) with a DMMA.8x8x4 chain
- * microbenchmark on the legacy default stream (about 50 ms, synchronous).  This is the roofline
- * denominator for the mode-wise matrix product; it is not part of the hot path. */
-int nspt_probe_fp64_peak(double* tflops);
-
-/* Total kernels launched by the library since it was loaded. */
-long long nspt_launch_count(void);
 
 /* Free all library-owned device / host memory and cached plans. */
 int nspt_release(void);

@@ -1,0 +1,45 @@
+/*
+ * nspt_debug.h -- diagnostics of libnspt that are NOT part of the method's boundary (include/nspt.h): kernel selection
+ * for cross-checks and experiments, per-stage device timing, the FP64 tensor-pipe probe that supplies the roofline
+ * denominator, and the launch counter the benchmark reports.  Same conventions as nspt.h (int return codes, current
+ * device's context).
+ */
+#ifndef NSPT_DEBUG_H
+#define NSPT_DEBUG_H
+
+#include "nspt.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Select the kernel of the mode-wise matrix product (Step 3):
+ *   0 = reference kernel (one thread per output element, plain double FMAs; cross-check only),
+ *   1 = FP64 tensor-pipe kernel (DMMA, TMA-fed, 3-multiplication complex product; default),
+ *   2 = INT8 tensor-core kernel (tcgen05.mma.kind::i8, TMEM accumulators; FP64 emulated with seven int8 slices per
+ *       operand plane, exact INT32 sums).  Used by nspt_series_mul[_batched] only; products with
+ *       scaling / accumulating epilogues (staple, exponential) stay on kernel 1.  Needs extra workspace
+ *       (nspt_workspace_bytes reports it for the variant that is selected when it is called). */
+int nspt_set_gemm_variant(int variant);
+
+/* Per-stage device timing.  After nspt_profile(1) every kernel the library launches is
+ * bracketed by CUDA events on the library stream; nspt_profile_read synchronises the stream,
+ * and for stage = 0 forward transforms, 1 mode-wise matrix products, 2 inverse transforms,
+ * 3 re-truncation transforms, 4 other (dagger, force, scaling), 5 block polynomials of the series
+ * exponential, 6 int8 slicing passes of kernel 2 returns the summed milliseconds and the number of
+ * launches since the last read, then resets the counters. */
+int nspt_profile(int enable);
+int nspt_profile_read(int stage, double* ms, long long* launches);
+
+/* Measure the FP64 tensor-pipe peak of the current device (TFLOP/s) with a DMMA.8x8x4 chain
+ * microbenchmark on the legacy default stream (about 50 ms, synchronous).  This is the roofline
+ * denominator for the mode-wise matrix product; it is not part of the hot path. */
+int nspt_probe_fp64_peak(double* tflops);
+
+/* Total kernels launched by the library since it was loaded. */
+long long nspt_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NSPT_DEBUG_H */

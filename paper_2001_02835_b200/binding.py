@@ -20,7 +20,8 @@ _LIB_PATH = _PKG / "libnspt.so"
 
 NSPT_OK, NSPT_EINVAL, NSPT_ENOMEM, NSPT_ECUDA, NSPT_EARCH = 0, -1, -2, -3, -4
 NSPT_OP_SERIES_MUL, NSPT_OP_STAPLE, NSPT_OP_SERIES_EXP = 0, 1, 2
-STAGES = {"fft_forward": 0, "zgemm_modes": 1, "fft_inverse": 2, "fft_retruncate": 3, "other": 4}
+STAGES = {"fft_forward": 0, "zgemm_modes": 1, "fft_inverse": 2, "fft_retruncate": 3, "other": 4, "freq_block_polys": 5,
+          "int8_slicing": 6}
 
 EXPORTS = [
     "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_series_exp", "nspt_series_exp_batched", "nspt_force",

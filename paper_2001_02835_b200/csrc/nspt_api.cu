@@ -29,6 +29,8 @@ struct ProfEvent {
 struct Context {
     std::mutex mu;
     cudaStream_t stream = nullptr;
+    cudaEvent_t order_event = nullptr;   // orders a newly set stream after the work of the previous one
+    bool used = false;                   // a kernel has been enqueued since the library was loaded / released
     double order_scale = 1.0;
     int gemm_variant = 1;
     bool arch_checked = false;
@@ -47,13 +49,42 @@ struct Context {
     bool profiling = false;
     std::vector<ProfEvent> prof_used;
     std::vector<ProfEvent> prof_free;
-    double prof_ms[ST_COUNT] = {0, 0, 0, 0, 0};
-    long long prof_n[ST_COUNT] = {0, 0, 0, 0, 0};
+    double prof_ms[ST_COUNT] = {};
+    long long prof_n[ST_COUNT] = {};
     long long launches = 0;
     char cuda_msg[256] = "no CUDA error recorded";
 };
 
-Context g;
+// One context per CUDA device, selected by the device current at the call (cudaGetDevice): plans, workspace, staging,
+// stream and profiling state never cross devices, so one process can drive several GPUs (one direction of the TEK model per
+// GPU) from one or several host threads.
+constexpr int MAX_DEVICES = 64;
+Context g_contexts[MAX_DEVICES];
+thread_local Context* g_current = &g_contexts[0];
+#define g (*g_current)
+
+struct ContextLock {
+    bool ok = false;
+    Context* c = nullptr;
+    ContextLock() {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) {   // no device at all: argument checks still work (context 0)
+            cudaGetLastError();
+            dev = 0;
+        }
+        if (dev < 0 || dev >= MAX_DEVICES) return;
+        c = &g_contexts[dev];
+        c->mu.lock();
+        g_current = c;
+        ok = true;
+    }
+    ~ContextLock() {
+        if (ok) c->mu.unlock();
+    }
+};
+#define NSPT_LOCK()     \
+    ContextLock lk__;   \
+    if (!lk__.ok) return NSPT_ECUDA
 
 int cuda_fail(cudaError_t e) {
     snprintf(g.cuda_msg, sizeof(g.cuda_msg), "CUDA error: %s", cudaGetErrorString(e));
@@ -222,6 +253,7 @@ struct StageTimer {
     ProfEvent ev{};
     int begin(int stage) {
         g.launches += 1;
+        g.used = true;
         if (!g.profiling) return NSPT_OK;
         if (g.prof_used.size() >= 4096) {
             int rc = prof_flush();
@@ -320,7 +352,7 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
         void* oz = ws + 3 * sb + WS_PAD;
         {
             StageTimer tm;
-            NSPT_TRY(tm.begin(ST_OTHER));
+            NSPT_TRY(tm.begin(ST_SLICE));
             NSPT_CUDA(launch_ozaki_slice(f, batch, At, Bt, oz, g.stream));
             NSPT_TRY(tm.end());
         }
@@ -394,7 +426,7 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
                     coef[j * ps + i] = (m <= Ntrunc) ? (double)(1.0L / fct) : 0.0;
                 }
             StageTimer tm;
-            NSPT_TRY(tm.begin(ST_OTHER));
+            NSPT_TRY(tm.begin(ST_POLY));
             NSPT_CUDA(launch_freq_block_polys(f, batch, pw(1), bj(0), ps, pr, coef, g.stream));
             NSPT_TRY(tm.end());
         }
@@ -557,37 +589,37 @@ using namespace nspt;
 extern "C" {
 
 int nspt_series_mul(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     return series_mul_device(A, B, C, N, Ntrunc, 1);
 }
 
 int nspt_series_mul_batched(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc, int batch) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     return series_mul_device(A, B, C, N, Ntrunc, batch);
 }
 
 int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4], int N, int Ntrunc) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     return staple_device(U, z, S, N, Ntrunc);
 }
 
 int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     return series_exp_device(X, E, N, Ntrunc, 1);
 }
 
 int nspt_series_exp_batched(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int batch) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     return series_exp_device(X, E, N, Ntrunc, batch);
 }
 
 int nspt_force(const nspt_c128* S, nspt_c128* F, double c, int N, int Ntrunc) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     return force_device(S, F, c, N, Ntrunc);
 }
 
 int nspt_series_mul_batched_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc, int batch) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     NSPT_TRY(check_dims(N, Ntrunc, batch));
     if (!A || !B || !C) return NSPT_EINVAL;
     const size_t bytes = (size_t)batch * (Ntrunc + 1) * N * N * sizeof(nspt_c128);
@@ -639,7 +671,7 @@ int nspt_series_mul_host(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, i
 }
 
 int nspt_staple_host(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4], int N, int Ntrunc) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     NSPT_TRY(check_dims(N, Ntrunc, 1));
     if (!U || !z || !S) return NSPT_EINVAL;
     for (int mu = 0; mu < 4; ++mu)
@@ -662,14 +694,29 @@ int nspt_staple_host(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c1
 }
 
 int nspt_set_stream(void* cuda_stream) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     if (g.profiling) NSPT_TRY(prof_flush());
-    g.stream = static_cast<cudaStream_t>(cuda_stream);
+    cudaStream_t next = static_cast<cudaStream_t>(cuda_stream);
+    if (next != g.stream && g.used) {
+        // all calls share one workspace: work queued on the new stream must not overtake what the old one still runs.
+        // (Skipped while either stream is capturing: a captured stream cannot wait on work outside its graph.)
+        cudaStreamCaptureStatus a = cudaStreamCaptureStatusNone, b = cudaStreamCaptureStatusNone;
+        cudaStreamIsCapturing(g.stream, &a);
+        cudaStreamIsCapturing(next, &b);
+        if (a == cudaStreamCaptureStatusNone && b == cudaStreamCaptureStatusNone) {
+            if (!g.order_event) NSPT_CUDA(cudaEventCreateWithFlags(&g.order_event, cudaEventDisableTiming));
+            NSPT_CUDA(cudaEventRecord(g.order_event, g.stream));
+            NSPT_CUDA(cudaStreamWaitEvent(next, g.order_event, 0));
+        } else {
+            cudaGetLastError();
+        }
+    }
+    g.stream = next;
     return NSPT_OK;
 }
 
 int nspt_set_order_scale(double s) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     if (!(s > 0.0) || !std::isfinite(s)) return NSPT_EINVAL;
     g.order_scale = s;
     return NSPT_OK;
@@ -677,6 +724,7 @@ int nspt_set_order_scale(double s) {
 
 int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out) {
     if (!out) return NSPT_EINVAL;
+    NSPT_LOCK();
     if (op != NSPT_OP_SERIES_MUL && op != NSPT_OP_STAPLE && op != NSPT_OP_SERIES_EXP) return NSPT_EINVAL;
     if (op == NSPT_OP_STAPLE) batch = 1;
     NSPT_TRY(check_dims(N, Ntrunc, batch));
@@ -687,7 +735,7 @@ int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out) {
 }
 
 int nspt_set_workspace(void* dptr, size_t bytes) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     if (dptr && (reinterpret_cast<uintptr_t>(dptr) & 255)) return NSPT_EINVAL;
     if (!dptr && bytes) return NSPT_EINVAL;
     g.user_ws = dptr;
@@ -696,21 +744,21 @@ int nspt_set_workspace(void* dptr, size_t bytes) {
 }
 
 int nspt_set_gemm_variant(int variant) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     if (variant != 0 && variant != 1 && variant != 2) return NSPT_EINVAL;
     g.gemm_variant = variant;
     return NSPT_OK;
 }
 
 int nspt_profile(int enable) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     if (!enable && g.profiling) NSPT_TRY(prof_flush());
     g.profiling = enable != 0;
     return NSPT_OK;
 }
 
 int nspt_profile_read(int stage, double* ms, long long* launches) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     if (stage < 0 || stage >= ST_COUNT || !ms || !launches) return NSPT_EINVAL;
     NSPT_TRY(prof_flush());
     *ms = g.prof_ms[stage];
@@ -721,12 +769,12 @@ int nspt_profile_read(int stage, double* ms, long long* launches) {
 }
 
 long long nspt_launch_count(void) {
-    std::lock_guard<std::mutex> lk(g.mu);
-    return g.launches;
+    ContextLock lk;
+    return lk.ok ? g.launches : 0;
 }
 
 int nspt_release(void) {
-    std::lock_guard<std::mutex> lk(g.mu);
+    NSPT_LOCK();
     cudaStreamSynchronize(g.stream);
     for (Plan& p : g.plans) {
         cudaFree(p.tw_fwd);
@@ -756,6 +804,9 @@ int nspt_release(void) {
     }
     g.prof_used.clear();
     g.prof_free.clear();
+    if (g.order_event) cudaEventDestroy(g.order_event);
+    g.order_event = nullptr;
+    g.used = false;
     return NSPT_OK;
 }
 
@@ -770,6 +821,6 @@ const char* nspt_strerror(int code) {
     }
 }
 
-int nspt_version(void) { return 200; }
+int nspt_version(void) { return 300; }
 
 }  // extern "C"

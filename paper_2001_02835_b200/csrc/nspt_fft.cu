@@ -579,26 +579,28 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
 // Spectrum of the daggered series (g is real): FFT[X^+](p) = (X~((L-p) mod L))^H.
 // dst(b,p)[i][j] = conj(src(b,(L-p)%L)[j][i]); 32x32 tiles through shared memory.
 __global__ void __launch_bounds__(256) freq_dagger_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
-                                                         int N, size_t NN, int L) {
+                                                         int N, size_t NN, int L, int modes) {
     __shared__ double2 tile[32][33];
-    const int bp = blockIdx.z;  // b*L + p
-    const int b = bp / L, p = bp % L;
-    const double2* s = src + (size_t)(b * L + (L - p) % L) * NN;
-    double2* d = dst + (size_t)bp * NN;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;  // 32 x 8
     const int i0 = blockIdx.y * 32, j0 = blockIdx.x * 32;
+    for (int bp = blockIdx.z; bp < modes; bp += gridDim.z) {  // b*L + p (the grid's z extent is capped at 65535)
+        const int b = bp / L, p = bp % L;
+        const double2* s = src + (size_t)(b * L + (L - p) % L) * NN;
+        double2* d = dst + (size_t)bp * NN;
+        __syncthreads();
 #pragma unroll
-    for (int r = ty; r < 32; r += 8) {
-        const int j = j0 + r, i = i0 + tx;
-        tile[r][tx] = (j < N && i < N) ? s[(size_t)j * N + i] : make_double2(0.0, 0.0);
-    }
-    __syncthreads();
+        for (int r = ty; r < 32; r += 8) {
+            const int j = j0 + r, i = i0 + tx;
+            tile[r][tx] = (j < N && i < N) ? s[(size_t)j * N + i] : make_double2(0.0, 0.0);
+        }
+        __syncthreads();
 #pragma unroll
-    for (int r = ty; r < 32; r += 8) {
-        const int i = i0 + r, j = j0 + tx;
-        if (i < N && j < N) {
-            const double2 v = tile[tx][r];
-            d[(size_t)i * N + j] = make_double2(v.x, -v.y);
+        for (int r = ty; r < 32; r += 8) {
+            const int i = i0 + r, j = j0 + tx;
+            if (i < N && j < N) {
+                const double2 v = tile[tx][r];
+                d[(size_t)i * N + j] = make_double2(v.x, -v.y);
+            }
         }
     }
 }
@@ -606,39 +608,40 @@ __global__ void __launch_bounds__(256) freq_dagger_kernel(const double2* __restr
 // dst(p) = alpha * src(p) + 1 for every mode p: alpha X + (identity series), whose spectrum is the unit matrix
 // at every mode.  First Horner step of the series exponential.
 __global__ void __launch_bounds__(256) freq_scale_identity_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
-                                                                 int N, size_t NN, double alpha) {
+                                                                 int N, size_t NN, double alpha, int modes) {
     const size_t e = (size_t)blockIdx.x * 256 + threadIdx.x;
     if (e >= NN) return;
-    const size_t o = (size_t)blockIdx.y * NN + e;
-    double2 v = src[o];
-    v.x *= alpha;
-    v.y *= alpha;
-    if (e / N == e % N) v.x += 1.0;
-    dst[o] = v;
+    for (int m = blockIdx.y; m < modes; m += gridDim.y) {   // the grid's y extent is capped at 65535
+        const size_t o = (size_t)m * NN + e;
+        double2 v = src[o];
+        v.x *= alpha;
+        v.y *= alpha;
+        if (e / N == e % N) v.x += 1.0;
+        dst[o] = v;
+    }
 }
 
 // ------------------------------------------------------------------------------------ host side
 enum Which { W_FWD, W_INV, W_RET };
 
 int num_sms() {
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (sms <= 0) sms = 148;
+    static int sms[NSPT_MAX_DEVICES] = {};
+    const int dev = current_device();
+    if (!sms[dev]) {
+        cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev);
+        if (sms[dev] <= 0) sms[dev] = 148;
     }
-    return sms;
+    return sms[dev];
 }
 
 // Resident CTAs per SM of a kernel, looked up once per kernel (the attribute and occupancy calls cost more host
 // time than a small transform takes on the device).
 template <typename K>
 cudaError_t persistent_grid(K kernel, int threads, int smem, unsigned total_tiles, unsigned* grid) {
-    static std::map<const void*, int> cache;
+    static std::map<std::pair<int, const void*>, int> cache;   // (device, kernel): function attributes are per device
     static std::mutex mu;
     std::lock_guard<std::mutex> lk(mu);
-    const void* key = reinterpret_cast<const void*>(kernel);
+    const std::pair<int, const void*> key(current_device(), reinterpret_cast<const void*>(kernel));
     auto it = cache.find(key);
     int occ;
     if (it == cache.end()) {
@@ -778,17 +781,19 @@ cudaError_t launch_fft_retruncate(const FreqLayout& f, const PlanTables& t, int 
 }
 
 cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src, double* dst, cudaStream_t st) {
-    dim3 grid((f.N + 31) / 32, (f.N + 31) / 32, (unsigned)(batch * f.L));
+    const int modes = batch * f.L;
+    dim3 grid((f.N + 31) / 32, (f.N + 31) / 32, (unsigned)(modes < 65535 ? modes : 65535));
     freq_dagger_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst), f.N,
-                                             f.NN, f.L);
+                                             f.NN, f.L, modes);
     return cudaGetLastError();
 }
 
 cudaError_t launch_freq_scale_identity(const FreqLayout& f, int batch, const double* src, double* dst, double alpha,
                                        cudaStream_t st) {
-    dim3 grid((unsigned)((f.NN + 255) / 256), (unsigned)(batch * f.L));
+    const int modes = batch * f.L;
+    dim3 grid((unsigned)((f.NN + 255) / 256), (unsigned)(modes < 65535 ? modes : 65535));
     freq_scale_identity_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst),
-                                                     f.N, f.NN, alpha);
+                                                     f.N, f.NN, alpha, modes);
     return cudaGetLastError();
 }
 

@@ -4,6 +4,7 @@
 #include <cstddef>
 #include <cstdint>
 #include "../../include/nspt.h"
+#include "../../include/nspt_debug.h"
 
 namespace nspt {
 
@@ -48,7 +49,18 @@ struct PlanTables {
     double inv_L;
 };
 
-enum Stage { ST_FWD = 0, ST_GEMM = 1, ST_INV = 2, ST_RETRUNC = 3, ST_OTHER = 4, ST_COUNT = 5 };
+// Launcher-side caches (function attributes, occupancy, SM counts) are per device.
+constexpr int NSPT_MAX_DEVICES = 64;
+inline int current_device() {
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess) {
+        cudaGetLastError();
+        d = 0;
+    }
+    return (d < 0 || d >= NSPT_MAX_DEVICES) ? 0 : d;
+}
+
+enum Stage { ST_FWD = 0, ST_GEMM = 1, ST_INV = 2, ST_RETRUNC = 3, ST_OTHER = 4, ST_POLY = 5, ST_SLICE = 6, ST_COUNT = 7 };
 
 // Complex scalar for epilogues.
 struct Cplx { double re, im; };

@@ -55,8 +55,9 @@ static_assert(OZ_STAGE % 1024 == 0 && OZ_M_STAGE % 1024 == 0, "stage alignment")
 // ---- slicing ------------------------------------------------------------------------------------------------
 // max over a mode of max(|re|, |im|) as the bit pattern of a non-negative double (ordered like an unsigned integer)
 __global__ void __launch_bounds__(256) oz_absmax_kernel(const double2* __restrict__ X, unsigned long long* __restrict__ maxbits,
-                                                      size_t NN) {
-    const int mode = blockIdx.y;
+                                                      size_t NN, int modes) {
+    __shared__ double red[8];
+    for (int mode = blockIdx.y; mode < modes; mode += gridDim.y) {   // the grid's y extent is capped at 65535
     const double2* x = X + (size_t)mode * NN;
     double m = 0.0;
     for (size_t e = (size_t)blockIdx.x * 256 + threadIdx.x; e < NN; e += (size_t)gridDim.x * 256) {
@@ -65,13 +66,14 @@ __global__ void __launch_bounds__(256) oz_absmax_kernel(const double2* __restric
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-    __shared__ double red[8];
+    __syncthreads();
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
     __syncthreads();
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int w = 1; w < 8; ++w) m = fmax(m, red[w]);
         atomicMax(maxbits + mode, (unsigned long long)__double_as_longlong(m));
+    }
     }
 }
 
@@ -104,13 +106,13 @@ __device__ __forceinline__ unsigned long long oz_digits(double x, double scale) 
 template <bool QUAD>
 __global__ void __launch_bounds__(256) oz_slice_kernel(const double2* __restrict__ X, int8_t* __restrict__ out,
                                                       const unsigned long long* __restrict__ maxbits, int* __restrict__ exps,
-                                                      int N, int pitch) {
-    const int mode = blockIdx.y;
+                                                      int N, int pitch, int modes) {
+    for (int mode = blockIdx.y; mode < modes; mode += gridDim.y) {   // the grid's y extent is capped at 65535
     const int qpr = QUAD ? (pitch >> 5) : ((N + 3) >> 2);   // 4-column groups per row (QUAD: 256 bytes of pitch per 32 columns, k padded)
     const int t = blockIdx.x * 256 + threadIdx.x;
     const int e = oz_exponent(maxbits[mode]);
     if (t == 0) exps[mode] = e;
-    if (t >= N * qpr) return;
+    if (t >= N * qpr) continue;
     const int row = t / qpr, j0 = (t % qpr) * 4;
     const double sc = oz_pow2(OZ_FRAC_BITS - e), sc_sum = oz_pow2(OZ_FRAC_BITS - e - 1);
     const double2* x = X + ((size_t)mode * N + row) * N + j0;
@@ -137,6 +139,7 @@ __global__ void __launch_bounds__(256) oz_slice_kernel(const double2* __restrict
             // ROWS: pitch is a multiple of 64 and j0 of 4; pad columns N..pitch-1 receive zeros (never read: TMA clips at N)
             *reinterpret_cast<unsigned int*>(base + (size_t)q * plane_stride + (QUAD ? (size_t)s * 32 : (size_t)s * N * pitch)) = word;
         }
+    }
     }
 }
 
@@ -416,13 +419,14 @@ cudaError_t launch_ozaki_slice(const FreqLayout& f, int batch, const double* A, 
     cudaError_t e;
     if ((e = cudaMemsetAsync(w.maxbits, 0, sizeof(unsigned long long) * 2 * modes, st)) != cudaSuccess) return e;
     const unsigned chunks = (unsigned)((f.NN + 256 * 8 - 1) / (256 * 8));
-    oz_absmax_kernel<<<dim3(chunks, modes), 256, 0, st>>>(reinterpret_cast<const double2*>(A), w.maxbits, f.NN);
-    oz_absmax_kernel<<<dim3(chunks, modes), 256, 0, st>>>(reinterpret_cast<const double2*>(B), w.maxbits + modes, f.NN);
+    const unsigned gy = (unsigned)(modes < 65535 ? modes : 65535);
+    oz_absmax_kernel<<<dim3(chunks, gy), 256, 0, st>>>(reinterpret_cast<const double2*>(A), w.maxbits, f.NN, modes);
+    oz_absmax_kernel<<<dim3(chunks, gy), 256, 0, st>>>(reinterpret_cast<const double2*>(B), w.maxbits + modes, f.NN, modes);
     const int pq = oz_pitch_quad(N), pr = oz_pitch_rows(N);
-    oz_slice_kernel<true><<<dim3((unsigned)((N * (pq / 256 * 8) + 255) / 256), modes), 256, 0, st>>>(
-        reinterpret_cast<const double2*>(A), w.sA, w.maxbits, w.exps, N, pq);
-    oz_slice_kernel<false><<<dim3((unsigned)((N * ((N + 3) / 4) + 255) / 256), modes), 256, 0, st>>>(
-        reinterpret_cast<const double2*>(B), w.sB, w.maxbits + modes, w.exps + modes, N, pr);
+    oz_slice_kernel<true><<<dim3((unsigned)((N * (pq / 256 * 8) + 255) / 256), gy), 256, 0, st>>>(
+        reinterpret_cast<const double2*>(A), w.sA, w.maxbits, w.exps, N, pq, modes);
+    oz_slice_kernel<false><<<dim3((unsigned)((N * ((N + 3) / 4) + 255) / 256), gy), 256, 0, st>>>(
+        reinterpret_cast<const double2*>(B), w.sB, w.maxbits + modes, w.exps + modes, N, pr, modes);
     return cudaGetLastError();
 }
 
@@ -432,11 +436,12 @@ cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, do
     const int N = f.N;
     const OzWs w = oz_carve(f, batch, const_cast<void*>(ws));
     cudaError_t e;
-    static bool attr_done = false;
-    if (!attr_done) {
+    static bool attr_done[NSPT_MAX_DEVICES] = {};
+    const int dev = current_device();
+    if (!attr_done[dev]) {
         e = cudaFuncSetAttribute(zgemm_modes_ozaki_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, OZ_SMEM);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done[dev] = true;
     }
     const int pq = oz_pitch_quad(N), pr = oz_pitch_rows(N), nkc = (N + OZ_KC - 1) / OZ_KC;
     CUtensorMap mapM, mapN;

@@ -313,11 +313,11 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
 // complex product with plain FMAs.  For debugging the tensor-core kernel; never the default.
 __global__ void __launch_bounds__(256)
 zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict__ B, const GemmGroupDev G, int N, size_t NN,
-                       int L) {
-    const int mode = blockIdx.z;
+                       int L, int modes) {
     const int j = blockIdx.x * 16 + (threadIdx.x & 15);
     const int i = blockIdx.y * 16 + (threadIdx.x >> 4);
     if (i >= N || j >= N) return;
+    for (int mode = blockIdx.z; mode < modes; mode += gridDim.z) {   // the grid's z extent is capped at 65535
     const double2* Am = A + (size_t)mode * NN;
     const double2* Bm = B + (size_t)mode * NN;
     double cr = 0.0, ci = 0.0;
@@ -347,6 +347,7 @@ zgemm_modes_ref_kernel(const double2* __restrict__ A, const double2* __restrict_
         }
         *d = out;
     }
+    }
 }
 
 // 3-D view of a spectrum as doubles: (2N doubles per row, N rows, modes); boxes are 16 doubles wide
@@ -371,6 +372,35 @@ cudaError_t encode_operand(CUtensorMap* map, const double* basep, const FreqLayo
 
 }  // namespace
 
+// A tensor map depends only on (pointer, shape, strides, box, swizzle); encoding one costs 1-2 us of host time and a product
+// needs eight, which is most of the host cost of a small product.  Repeated calls on the same buffers (the normal case in an
+// NSPT run) therefore reuse the last encodings: a small per-thread cache, most recently used first.
+namespace {
+struct MapKey {
+    const void* base;
+    int rank;
+    int swizzle;
+    uint64_t dims[4];
+    uint64_t strides[3];
+    uint32_t box[4];
+    bool operator==(const MapKey& o) const {
+        if (base != o.base || rank != o.rank || swizzle != o.swizzle) return false;
+        for (int i = 0; i < 4; ++i)
+            if (dims[i] != o.dims[i] || box[i] != o.box[i]) return false;
+        for (int i = 0; i < 3; ++i)
+            if (strides[i] != o.strides[i]) return false;
+        return true;
+    }
+};
+struct MapEntry {
+    MapKey key;
+    CUtensorMap map;
+};
+constexpr int MAP_CACHE = 48;
+thread_local MapEntry t_maps[MAP_CACHE];
+thread_local int t_nmaps = 0;
+}  // namespace
+
 cudaError_t tma_encode_f64(CUtensorMap* map, const void* base, int rank, const uint64_t* dims,
                            const uint64_t* strides_bytes, const uint32_t* box, bool swizzle128) {
     if (!g_encode) {
@@ -381,6 +411,10 @@ cudaError_t tma_encode_f64(CUtensorMap* map, const void* base, int rank, const u
         if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
         g_encode = reinterpret_cast<EncodeTiledFn>(fn);
     }
+    MapKey key{};
+    key.base = base;
+    key.rank = rank;
+    key.swizzle = swizzle128 ? 1 : 0;
     cuuint64_t d[4] = {1, 1, 1, 1}, st[3] = {16, 16, 16};
     cuuint32_t bx[4] = {1, 1, 1, 1}, es[4] = {1, 1, 1, 1};
     for (int i = 0; i < rank; ++i) {
@@ -388,11 +422,32 @@ cudaError_t tma_encode_f64(CUtensorMap* map, const void* base, int rank, const u
         bx[i] = box[i];
     }
     for (int i = 0; i + 1 < rank; ++i) st[i] = strides_bytes[i];
+    for (int i = 0; i < 4; ++i) {
+        key.dims[i] = d[i];
+        key.box[i] = bx[i];
+    }
+    for (int i = 0; i < 3; ++i) key.strides[i] = st[i];
+    for (int i = 0; i < t_nmaps; ++i) {
+        if (t_maps[i].key == key) {
+            *map = t_maps[i].map;
+            if (i > 0) {   // move to the front
+                const MapEntry hit = t_maps[i];
+                for (int j = i; j > 0; --j) t_maps[j] = t_maps[j - 1];
+                t_maps[0] = hit;
+            }
+            return cudaSuccess;
+        }
+    }
     const CUresult r = g_encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, const_cast<void*>(base), d, st, bx, es,
                                 CU_TENSOR_MAP_INTERLEAVE_NONE,
                                 swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
                                 CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    if (t_nmaps < MAP_CACHE) ++t_nmaps;
+    for (int j = t_nmaps - 1; j > 0; --j) t_maps[j] = t_maps[j - 1];
+    t_maps[0].key = key;
+    t_maps[0].map = *map;
+    return cudaSuccess;
 }
 
 namespace {
@@ -400,12 +455,13 @@ namespace {
 template <class TC>
 cudaError_t launch_dmma(const FreqLayout& f, const double* baseA, int modesA, const double* baseB, int modesB, GemmParams P,
                         cudaStream_t st) {
-    static bool attr_done = false;
+    static bool attr_done[NSPT_MAX_DEVICES] = {};   // the function attribute is per device
     cudaError_t e;
-    if (!attr_done) {
+    const int dev = current_device();
+    if (!attr_done[dev]) {
         e = cudaFuncSetAttribute(zgemm_modes_dmma_kernel<TC>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC::SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done[dev] = true;
     }
     P.tiles_m = (f.N + TC::BM - 1) / TC::BM;
     P.tiles_n = (f.N + TC::BN - 1) / TC::BN;
@@ -440,10 +496,10 @@ cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup*
         if (!groups[i].A || !groups[i].B || (!groups[i].out.C && !groups[i].out.D)) return cudaErrorInvalidValue;
     if (variant == 0) {
         for (int i = 0; i < ngroups; ++i) {
-            dim3 grid((f.N + 15) / 16, (f.N + 15) / 16, modes);
+            dim3 grid((f.N + 15) / 16, (f.N + 15) / 16, modes < 65535 ? modes : 65535);
             zgemm_modes_ref_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(groups[i].A),
                                                          reinterpret_cast<const double2*>(groups[i].B), to_dev(groups[i].out),
-                                                         f.N, f.NN, f.L);
+                                                         f.N, f.NN, f.L, modes);
             cudaError_t e = cudaGetLastError();
             if (e != cudaSuccess) return e;
         }

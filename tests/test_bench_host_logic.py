@@ -67,3 +67,28 @@ def test_reference_arm_nonzero_rank_exits_quietly():
     out = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--impl", "reference", "--workload", "small",
                           "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=120, env=env)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_reference_arm_uses_the_cuda_arm_workload_string():
+    sys.path.insert(0, str(ROOT))
+    import bench
+    out = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--impl", "reference", "--workload", "small",
+                          "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=120)
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["config"]["workload"] == bench.WORKLOAD_DESC["small"]
+    assert "1 full star-product" in line["cpu_baseline"]["sample"]
+
+
+def test_replica_environment_and_cpu_fftconv():
+    sys.path.insert(0, str(ROOT))
+    import numpy as np
+    import bench
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    env = bench.replica_env(3, 4, 12345)
+    assert (env["RANK"], env["LOCAL_RANK"], env["WORLD_SIZE"], env["MASTER_ADDR"], env["MASTER_PORT"]) == \
+        ("3", "3", "4", "127.0.0.1", "12345")
+    # the second CPU baseline (the paper's FFT-CONV with library FFT + GEMM) computes the same product as the oracle
+    A, B = wl.config_product(12, 9, seed=[7, 12, 9])
+    err = oracle.per_order_error(bench.cpu_fftconv(A, B), oracle.series_mul(A, B), oracle.product_bound(A, B)).max()
+    assert err < 1e-13

@@ -17,16 +17,22 @@ def lib():
     return ctypes.CDLL(str(path))
 
 
-def declared_functions():
-    text = (ROOT / "include" / "nspt.h").read_text()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(nspt_[a-z0-9_]+)\s*\(", text)))
+def declared_functions(headers=("nspt.h", "nspt_debug.h")):
+    names = set()
+    for h in headers:
+        text = (ROOT / "include" / h).read_text()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names |= set(re.findall(r"\b(nspt_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_header_declares_the_north_star_calls():
-    names = declared_functions()
+    names = declared_functions(("nspt.h",))
     for must in ("nspt_series_mul", "nspt_series_mul_batched", "nspt_staple"):
         assert must in names
+    # diagnostics are kept out of the method's boundary
+    for dbg in ("nspt_set_gemm_variant", "nspt_profile", "nspt_profile_read", "nspt_probe_fp64_peak", "nspt_launch_count"):
+        assert dbg not in names and dbg in declared_functions(("nspt_debug.h",))
 
 
 def test_library_exports_every_declared_symbol(lib):
@@ -62,7 +68,7 @@ def test_argument_validation_without_a_gpu(lib):
     assert lib.nspt_force(None, None, 1.0, 4, 3) == -1
     assert lib.nspt_workspace_bytes(225, 31, 5, 2, ctypes.byref(out)) == 0 and out.value == 5 * 12 * 64 * 225 * 225 * 16 + 256   # Paterson-Stockmeyer: 6 powers + 6 block polynomials, + pad
     assert lib.nspt_set_order_scale(ctypes.c_double(-1.0)) == -1
-    assert lib.nspt_set_gemm_variant(9) == -1
+    assert lib.nspt_set_gemm_variant(9) == -1 and lib.nspt_set_gemm_variant(1) == 0
     assert b"invalid" in lib.nspt_strerror(-1)
     assert lib.nspt_version() >= 100
 
