@@ -744,7 +744,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--gemm-variant", type=int, default=1, choices=[1, 2],
+    ap.add_argument("--gemm-variant", type=int, default=1, choices=[1, 2, 3],
                     help="mode-wise product kernel: 1 = FP64 tensor pipe (DMMA, default), 2 = INT8 tensor cores (tcgen05, Ozaki slicing)")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":

@@ -22,6 +22,12 @@ extern "C" {
  *       (nspt_workspace_bytes reports it for the variant that is selected when it is called). */
 int nspt_set_gemm_variant(int variant);
 
+/* Select the convolution algorithm of nspt_series_mul[_batched]: 0 = automatic (default), 1 = FFT-CONV,
+ * 2 = Naive-CONV (eq. 2.5 evaluated directly, one launch of the tensor-pipe kernel with the K dimension
+ * concatenated over the order index; no transforms, no workspace).  Naive-CONV reads its inputs while it writes its
+ * output, so a call whose output aliases an input uses FFT-CONV whatever is selected here. */
+int nspt_set_conv_algorithm(int algorithm);
+
 /* Per-stage device timing.  After nspt_profile(1) every kernel the library launches is
  * bracketed by CUDA events on the library stream; nspt_profile_read synchronises the stream,
  * and for stage = 0 forward transforms, 1 mode-wise matrix products, 2 inverse transforms,

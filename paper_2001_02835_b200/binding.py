@@ -27,7 +27,7 @@ EXPORTS = [
     "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_series_exp", "nspt_series_exp_batched", "nspt_force",
     "nspt_series_mul_host", "nspt_series_mul_batched_host", "nspt_staple_host",
     "nspt_set_stream", "nspt_set_order_scale", "nspt_workspace_bytes", "nspt_set_workspace",
-    "nspt_set_gemm_variant", "nspt_probe_fp64_peak", "nspt_profile", "nspt_profile_read", "nspt_launch_count",
+    "nspt_set_gemm_variant", "nspt_set_conv_algorithm", "nspt_probe_fp64_peak", "nspt_profile", "nspt_profile_read", "nspt_launch_count",
     "nspt_release", "nspt_strerror", "nspt_version",
 ]
 
@@ -59,6 +59,7 @@ _lib.nspt_set_order_scale.argtypes = [_dbl]
 _lib.nspt_workspace_bytes.argtypes = [_int, _int, _int, _int, ctypes.POINTER(ctypes.c_size_t)]
 _lib.nspt_set_workspace.argtypes = [_vp, ctypes.c_size_t]
 _lib.nspt_set_gemm_variant.argtypes = [_int]
+_lib.nspt_set_conv_algorithm.argtypes = [_int]
 _lib.nspt_probe_fp64_peak.argtypes = [ctypes.POINTER(_dbl)]
 _lib.nspt_profile.argtypes = [_int]
 _lib.nspt_profile_read.argtypes = [_int, ctypes.POINTER(_dbl), ctypes.POINTER(ctypes.c_longlong)]
@@ -293,6 +294,11 @@ def nspt_set_workspace(dptr, nbytes: int):
 
 def nspt_set_gemm_variant(variant: int):
     _check(_lib.nspt_set_gemm_variant(int(variant)), "nspt_set_gemm_variant")
+
+
+def nspt_set_conv_algorithm(algorithm: int):
+    """0 = automatic, 1 = FFT-CONV, 2 = Naive-CONV (include/nspt_debug.h)."""
+    _check(_lib.nspt_set_conv_algorithm(int(algorithm)), "nspt_set_conv_algorithm")
 
 
 def nspt_profile(enable: bool):

@@ -33,6 +33,7 @@ struct Context {
     bool used = false;                   // a kernel has been enqueued since the library was loaded / released
     double order_scale = 1.0;
     int gemm_variant = 1;
+    int conv_algorithm = 0;              // 0 = automatic, 1 = FFT-CONV, 2 = Naive-CONV (nspt_debug.h)
     bool arch_checked = false;
     // workspace
     void* user_ws = nullptr;
@@ -331,12 +332,36 @@ int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, dou
 }
 
 // ---- the products --------------------------------------------------------------------------
+// Naive-CONV or FFT-CONV (PAPER.md:66 vs :68-102).  The direct evaluation needs N^3 n(n+1)/2 matrix multiplications against
+// N^3 L plus three transform passes, but it is a single launch without workspace traffic: it wins where the product is
+// launch- or transform-bound (see DESIGN.md 5.5 for the measured crossover).  It reads A and B while it writes C, so an
+// output that aliases an input always takes FFT-CONV.
+bool use_naive_conv(const FreqLayout& f, const nspt_c128* A, const nspt_c128* B, const nspt_c128* C) {
+    if (C == A || C == B || (g.gemm_variant != 1 && g.gemm_variant != 3)) return false;
+    if (g.conv_algorithm == 1) return false;
+    if (g.conv_algorithm == 2) return true;
+    // measured crossover (one B200, time per product through the binding): the direct form is one launch
+    // (7.5 us) against three (13 us) and wins while its n(n+1)/2 products stay a fraction of a wave
+    if (f.n == 1) return true;                 // a single matrix product: nothing to transform
+    if (f.N <= 16) return f.n <= 8;
+    if (f.N <= 32) return f.n <= 4;
+    if (f.N <= 64) return f.n <= 2;
+    return false;
+}
+
 int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc, int batch) {
     NSPT_TRY(check_dims(N, Ntrunc, batch));
     if (!A || !B || !C || !aligned16(A) || !aligned16(B) || !aligned16(C)) return NSPT_EINVAL;
     NSPT_TRY(check_arch());
     const FreqLayout f = make_layout(N, Ntrunc);
     if (!fft_length_supported(f.L)) return NSPT_EINVAL;
+    if (use_naive_conv(f, A, B, C)) {
+        // eq. 2.5 directly: one launch, no transforms, no workspace
+        StageTimer tm;
+        NSPT_TRY(tm.begin(ST_GEMM));
+        NSPT_CUDA(launch_naive_conv(f, batch, A, B, C, g.stream));
+        return tm.end();
+    }
     PlanTables t;
     NSPT_TRY(get_plan(f.L, f.n, g.order_scale, &t));
     char* ws = nullptr;
@@ -745,8 +770,15 @@ int nspt_set_workspace(void* dptr, size_t bytes) {
 
 int nspt_set_gemm_variant(int variant) {
     NSPT_LOCK();
-    if (variant != 0 && variant != 1 && variant != 2) return NSPT_EINVAL;
+    if (variant < 0 || variant > 3) return NSPT_EINVAL;
     g.gemm_variant = variant;
+    return NSPT_OK;
+}
+
+int nspt_set_conv_algorithm(int algorithm) {
+    NSPT_LOCK();
+    if (algorithm < 0 || algorithm > 2) return NSPT_EINVAL;
+    g.conv_algorithm = algorithm;
     return NSPT_OK;
 }
 

@@ -119,6 +119,10 @@ struct GemmGroup {
 cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup* groups, int ngroups, int variant,
                                 cudaStream_t st);
 
+// Naive-CONV: eq. 2.5 evaluated directly on the series (no transforms, no workspace), one launch.  C must not alias A, B.
+cudaError_t launch_naive_conv(const FreqLayout& f, int batch, const nspt_c128* A, const nspt_c128* B, nspt_c128* C,
+                              cudaStream_t st);
+
 // ---- mode-wise matrix product on the INT8 tensor cores (nspt_ozaki.cu; gemm variant 2) -------------------------
 // Plain C~(p) = A~(p) B~(p) only (no alpha / accumulate / dagger epilogues): FP64 spectra are cut into int8 slices
 // (launch_ozaki_slice), multiplied exactly by tcgen05.mma.kind::i8 and recombined in FP64 (launch_ozaki_gemm).

@@ -91,7 +91,28 @@ struct GemmParams {
     int tiles_m, tiles_n;
     int nmodes;    // modes per group (batch * L)
     int ngroups;
+    // Naive-CONV: the operands are the series themselves ("mode" = order index, n per batch element) and the
+    // product of order k is ONE matrix product with the K dimension concatenated over l = 0..k, A^(l) against B^(k-l).
+    int conv;      // 0 = mode-wise product, 1 = convolution over the order index
+    int n;         // coefficients per series (conv only)
     GemmGroupDev g[MAX_GROUPS];
+};
+
+// Which slice of which matrices K-slice j of a CTA reads.
+struct SliceMap {
+    int conv, nk_seg, modeA, modeB;   // conv: modeA = first coefficient of A, modeB = coefficient k of B (l = 0)
+    __device__ __forceinline__ void coords(int j, int& k0, int& ma, int& mb) const {
+        if (!conv) {
+            k0 = j * 8;
+            ma = modeA;
+            mb = modeB;
+        } else {
+            const int l = j / nk_seg;
+            k0 = (j - l * nk_seg) * 8;
+            ma = modeA + l;
+            mb = modeB - l;
+        }
+    }
 };
 
 template <class TC>
@@ -101,11 +122,32 @@ __device__ __forceinline__ void issue_slice(const CUtensorMap* mapA, const CUten
     tma_load_3d(stage_addr, mapA, full_bar, 2 * k0, m0, modeA);
     tma_load_4d(stage_addr + TC::A_STAGE_BYTES, mapB, full_bar, 0, k0, n0 / 8, modeB);
 }
+// The same slice with the B operand fetched as BN/8 boxes of a plain 3-D map (columns beyond N are zero-filled, nothing
+// beyond the operand is touched): used when B is a caller's array (Naive-CONV), which has no pad behind its last row.
+template <class TC>
+__device__ __forceinline__ void issue_slice_b3(const CUtensorMap* mapA, const CUtensorMap* mapB, uint32_t stage_addr,
+                                               uint32_t full_bar, int k0, int m0, int n0, int modeA, int modeB) {
+    mbar_expect_tx(full_bar, TC::STAGE_BYTES);
+    tma_load_3d(stage_addr, mapA, full_bar, 2 * k0, m0, modeA);
+#pragma unroll
+    for (int c = 0; c < TC::BN / 8; ++c)
+        tma_load_3d(stage_addr + TC::A_STAGE_BYTES + c * B_BOX_BYTES, mapB, full_bar, 2 * (n0 + 8 * c), k0, modeB);
+}
+template <class TC>
+__device__ __forceinline__ void issue_mapped(const CUtensorMap* mapA, const CUtensorMap* mapB, uint32_t stage_addr, uint32_t full_bar,
+                                             const SliceMap& sm, int j, int m0, int n0) {
+    int k0, ma, mb;
+    sm.coords(j, k0, ma, mb);
+    if (sm.conv)
+        issue_slice_b3<TC>(mapA, mapB, stage_addr, full_bar, k0, m0, n0, ma, mb);
+    else
+        issue_slice<TC>(mapA, mapB, stage_addr, full_bar, k0, m0, n0, ma, mb);
+}
 
 template <class TC, bool FULL>
 __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUtensorMap& mapB, const GemmParams& P,
                                               uint32_t base, const uint8_t* sgen, uint32_t bar_full, uint32_t bar_empty,
-                                              int warp, int lane, int nk, int m0, int n0, int modeA, int modeB, int nbm,
+                                              int warp, int lane, int nk, int m0, int n0, const SliceMap smap, int nbm,
                                               int nbn,
                                               uint32_t offA0, uint32_t offA1, uint32_t offB0, uint32_t offB1,
                                               double (&p1)[TC::MB][TC::NB][2], double (&p2)[TC::MB][TC::NB][2],
@@ -113,6 +155,7 @@ __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUt
     constexpr int MB = TC::MB, NB = TC::NB, STAGES = TC::STAGES, STAGE_BYTES = TC::STAGE_BYTES;
     const int N = P.N;
     const bool active = FULL || ((nbm > 0) && (nbn > 0));
+    int seg_it = 0;   // slice index inside the current K segment (one segment unless conv)
     for (int it = 0; it < nk; ++it) {
         // keep the four fragment offsets in registers (ptxas otherwise rematerialises them from the lane and
         // CTA indices inside every sub-step, ~20 dependent integer instructions in front of the loads)
@@ -121,7 +164,7 @@ __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUt
         mbar_wait(bar_full + 8 * slot, (it / STAGES) & 1);
         if (active) {
             const uint8_t* st = sgen + slot * STAGE_BYTES;
-            const int nsub = (it * BK + 1 < N) ? 2 : 1;  // odd k-slots of the last slice may all be padding
+            const int nsub = (seg_it * BK + 1 < N) ? 2 : 1;  // odd k-slots of the last slice may all be padding
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
                 if (s < nsub) {
@@ -153,6 +196,7 @@ __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUt
                 }
             }
         }
+        if (++seg_it == smap.nk_seg) seg_it = 0;
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
         if (it + 1 >= TC::LAG && warp == ((it + 1) & (TC::WARPS - 1))) {
@@ -162,99 +206,22 @@ __device__ __forceinline__ void gemm_mainloop(const CUtensorMap& mapA, const CUt
             if (j + STAGES < nk && lane == 0) {
                 const int sl = j % STAGES;
                 mbar_wait(bar_empty + 8 * sl, (j / STAGES) & 1);
-                issue_slice<TC>(&mapA, &mapB, base + sl * STAGE_BYTES, bar_full + 8 * sl, (j + STAGES) * BK, m0, n0, modeA,
-                                modeB);
+                issue_mapped<TC>(&mapA, &mapB, base + sl * STAGE_BYTES, bar_full + 8 * sl, smap, j + STAGES, m0, n0);
             }
             __syncwarp();
         }
     }
 }
 
+// Epilogue of one warp: C = alpha AB (+ diag 1), C += alpha AB, and / or the conjugate-transposed (accumulating) store into
+// the mirrored mode (the spectrum of the daggered product series, FFT[X^+](p') = (X~(p))^H with p' = (L - p) mod L).
 template <class TC>
-__global__ void __launch_bounds__(TC::THREADS, TC::MINB)
-zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
-                        const GemmParams P) {
-    constexpr int MB = TC::MB, NB = TC::NB, STAGES = TC::STAGES, STAGE_BYTES = TC::STAGE_BYTES;
-    constexpr int BM = TC::BM, BN = TC::BN;
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));  // same address, generic-shared pointer for loads
-    const uint32_t bar_full = base + STAGES * STAGE_BYTES;
-    const uint32_t bar_empty = bar_full + STAGES * 8;
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int tiles = P.tiles_m * P.tiles_n;
-    const int grp = blockIdx.x / (tiles * P.nmodes);
-    const int rest = blockIdx.x % (tiles * P.nmodes);
-    const int mode = rest / tiles;    // mode inside the group
-    const int tile = rest % tiles;
-    const int m0 = (tile / P.tiles_n) * BM, n0 = (tile % P.tiles_n) * BN;
+__device__ __forceinline__ void gemm_epilogue(const GemmParams& P, const GemmGroupDev& G, int mode, int m0, int n0, int mw, int nw,
+                                              int nbm, int nbn, int g, int t, double (&p1)[TC::MB][TC::NB][2],
+                                              double (&p2)[TC::MB][TC::NB][2], double (&p3)[TC::MB][TC::NB][2]) {
+    constexpr int MB = TC::MB, NB = TC::NB;
     const int N = P.N;
-    const int nk = (N + BK - 1) / BK;
-    const GemmGroupDev& G = P.g[grp];
-    const int modeA = G.aoff + mode, modeB = G.boff + mode;
-
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(bar_full + 8 * s, 1);
-            mbar_init(bar_empty + 8 * s, TC::WARPS);
-        }
-        mbar_fence_init();
-    }
-    pdl_wait();      // the set-up above overlaps the tail of the previous kernel of the stream
-    pdl_trigger();
-    if (threadIdx.x == 0) {
-        const int pre = nk < STAGES ? nk : STAGES;
-        for (int it = 0; it < pre; ++it)
-            issue_slice<TC>(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, it * BK, m0, n0, modeA, modeB);
-    }
-    __syncthreads();
-
-    const int g = lane >> 2, t = lane & 3;
-    // Part of the CTA tile this warp owns.  Edge tiles give the warps unequal work (out-of-range 8-blocks are
-    // skipped) and warp w always runs on scheduler w % 4 of its SM, each with its own DMMA pipe: rotating the
-    // assignment with the CTA index spreads the light parts over the four schedulers.
-    const int quad = (warp + blockIdx.x) & (TC::WARPS - 1);
-    const int wm = quad / TC::WN, wn = quad % TC::WN;
-    const int mw = 8 * MB * wm, nw = 8 * NB * wn;  // warp offsets inside the CTA tile
-    // number of 8-row / 8-column blocks of this warp that intersect the matrix
-    int nbm = (N - (m0 + mw) + 7) >> 3;
-    nbm = nbm < 0 ? 0 : (nbm > MB ? MB : nbm);
-    int nbn = (N - (n0 + nw) + 7) >> 3;
-    nbn = nbn < 0 ? 0 : (nbn > NB ? NB : nbn);
-    const bool active = (nbm > 0) && (nbn > 0);
-
-    double p1[MB][NB][2], p2[MB][NB][2], p3[MB][NB][2];
-#pragma unroll
-    for (int i = 0; i < MB; ++i)
-#pragma unroll
-        for (int j = 0; j < NB; ++j) {
-            p1[i][j][0] = p1[i][j][1] = 0.0;
-            p2[i][j][0] = p2[i][j][1] = 0.0;
-            p3[i][j][0] = p3[i][j][1] = 0.0;
-        }
-
-    // per-lane byte offsets of the fragment loads inside a stage (sub-step 0; sub-step 1 is derived)
-    const uint32_t offA0 = (uint32_t)((mw + g) * 128 + (((2 * t) ^ g) << 4));           // + bm*1024
-    const uint32_t offA1 = offA0 ^ 16u;                                                   // k-slot 2t+1
-    const uint32_t offB0 =
-        (uint32_t)(TC::A_STAGE_BYTES + (NB * wn) * B_BOX_BYTES + (2 * t) * 128 + ((g ^ (2 * t)) << 4));  // + bn*1024
-    const uint32_t offB1 = (offB0 + 128u) ^ 16u;                                          // row 2t+1
-
-    // Warps whose MB x NB blocks all intersect the matrix (all but those on the last tile row / column) run
-    // an unpredicated copy of the loop: predicated mma.sync costs a WARPSYNC and issue bubbles per group.
-    if (nbm == MB && nbn == NB)
-        gemm_mainloop<TC, true>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, modeA, modeB, MB, NB,
-                                offA0, offA1, offB0, offB1, p1, p2, p3);
-    else
-        gemm_mainloop<TC, false>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, modeA, modeB, nbm,
-                                 nbn, offA0, offA1, offB0, offB1, p1, p2, p3);
-
-    if (!active) return;
-    // ---------------------------------------------------------------- epilogue
     double2* Cm = G.C ? G.C + (size_t)mode * P.NN : nullptr;
-    // spectrum of the daggered series: FFT[X^+](p') = (X~(p))^H with p' = (L - p) mod L, same batch element
     const int pm = mode % P.L;
     double2* Dm = G.D ? G.D + (size_t)(mode - pm + ((P.L - pm) % P.L)) * P.NN : nullptr;
     const double alpha_re = G.alpha_re, alpha_im = G.alpha_im, beta_re = G.beta_re, beta_im = G.beta_im;
@@ -306,6 +273,275 @@ zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
                 }
             }
         }
+    }
+}
+
+template <class TC>
+__global__ void __launch_bounds__(TC::THREADS, TC::MINB)
+zgemm_modes_dmma_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
+                        const GemmParams P) {
+    constexpr int MB = TC::MB, NB = TC::NB, STAGES = TC::STAGES, STAGE_BYTES = TC::STAGE_BYTES;
+    constexpr int BM = TC::BM, BN = TC::BN;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));  // same address, generic-shared pointer for loads
+    const uint32_t bar_full = base + STAGES * STAGE_BYTES;
+    const uint32_t bar_empty = bar_full + STAGES * 8;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tiles = P.tiles_m * P.tiles_n;
+    const int grp = blockIdx.x / (tiles * P.nmodes);
+    const int rest = blockIdx.x % (tiles * P.nmodes);
+    int mode = rest / tiles;          // mode inside the group
+    const int tile = rest % tiles;
+    const int m0 = (tile / P.tiles_n) * BM, n0 = (tile % P.tiles_n) * BN;
+    const int N = P.N;
+    const GemmGroupDev& G = P.g[grp];
+    SliceMap smap;
+    smap.conv = P.conv;
+    smap.nk_seg = (N + BK - 1) / BK;
+    int nk = smap.nk_seg;
+    if (P.conv) {
+        // order k of batch element b; the heavy high orders come first in the grid, the light ones fill its tail
+        const int b = mode / P.n, k = P.n - 1 - mode % P.n;
+        mode = b * P.n + k;            // where the result goes
+        nk = (k + 1) * smap.nk_seg;    // K runs over A^(0..k) against B^(k..0)
+        smap.modeA = G.aoff + b * P.n;
+        smap.modeB = G.boff + b * P.n + k;
+    } else {
+        smap.modeA = G.aoff + mode;
+        smap.modeB = G.boff + mode;
+    }
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_empty + 8 * s, TC::WARPS);
+        }
+        mbar_fence_init();
+    }
+    pdl_wait();      // the set-up above overlaps the tail of the previous kernel of the stream
+    pdl_trigger();
+    if (threadIdx.x == 0) {
+        const int pre = nk < STAGES ? nk : STAGES;
+        for (int it = 0; it < pre; ++it)
+            issue_mapped<TC>(&mapA, &mapB, base + it * STAGE_BYTES, bar_full + 8 * it, smap, it, m0, n0);
+    }
+    __syncthreads();
+
+    const int g = lane >> 2, t = lane & 3;
+    // Part of the CTA tile this warp owns.  Edge tiles give the warps unequal work (out-of-range 8-blocks are
+    // skipped) and warp w always runs on scheduler w % 4 of its SM, each with its own DMMA pipe: rotating the
+    // assignment with the CTA index spreads the light parts over the four schedulers.
+    const int quad = (warp + blockIdx.x) & (TC::WARPS - 1);
+    const int wm = quad / TC::WN, wn = quad % TC::WN;
+    const int mw = 8 * MB * wm, nw = 8 * NB * wn;  // warp offsets inside the CTA tile
+    // number of 8-row / 8-column blocks of this warp that intersect the matrix
+    int nbm = (N - (m0 + mw) + 7) >> 3;
+    nbm = nbm < 0 ? 0 : (nbm > MB ? MB : nbm);
+    int nbn = (N - (n0 + nw) + 7) >> 3;
+    nbn = nbn < 0 ? 0 : (nbn > NB ? NB : nbn);
+    const bool active = (nbm > 0) && (nbn > 0);
+
+    double p1[MB][NB][2], p2[MB][NB][2], p3[MB][NB][2];
+#pragma unroll
+    for (int i = 0; i < MB; ++i)
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+            p1[i][j][0] = p1[i][j][1] = 0.0;
+            p2[i][j][0] = p2[i][j][1] = 0.0;
+            p3[i][j][0] = p3[i][j][1] = 0.0;
+        }
+
+    // per-lane byte offsets of the fragment loads inside a stage (sub-step 0; sub-step 1 is derived)
+    const uint32_t offA0 = (uint32_t)((mw + g) * 128 + (((2 * t) ^ g) << 4));           // + bm*1024
+    const uint32_t offA1 = offA0 ^ 16u;                                                   // k-slot 2t+1
+    const uint32_t offB0 =
+        (uint32_t)(TC::A_STAGE_BYTES + (NB * wn) * B_BOX_BYTES + (2 * t) * 128 + ((g ^ (2 * t)) << 4));  // + bn*1024
+    const uint32_t offB1 = (offB0 + 128u) ^ 16u;                                          // row 2t+1
+
+    // Warps whose MB x NB blocks all intersect the matrix (all but those on the last tile row / column) run
+    // an unpredicated copy of the loop: predicated mma.sync costs a WARPSYNC and issue bubbles per group.
+    if (nbm == MB && nbn == NB)
+        gemm_mainloop<TC, true>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, smap, MB, NB,
+                                offA0, offA1, offB0, offB1, p1, p2, p3);
+    else
+        gemm_mainloop<TC, false>(mapA, mapB, P, base, sgen, bar_full, bar_empty, warp, lane, nk, m0, n0, smap, nbm,
+                                 nbn, offA0, offA1, offB0, offB1, p1, p2, p3);
+
+    if (!active) return;
+    gemm_epilogue<TC>(P, G, mode, m0, n0, mw, nw, nbm, nbn, g, t, p1, p2, p3);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Persistent, warp-specialised form of the same product (one CTA per SM).  Warp group 0 holds the producers: warp q feeds
+// consumer group q -- four warps that own one CTA tile at a time, exactly the warp tile and inner loop of the kernel
+// above -- through a ring of its own.  What changes: (1) a producer runs up to STAGES slices ahead across tile boundaries,
+// so a consumer group never waits for the first slices of its next tile, and no warp spends registers or issue slots on
+// refill bookkeeping; (2) consumer group q of SM b walks the tiles q * SMs + b, + GROUPS * SMs, ... : all groups of all SMs
+// stay within a window of GROUPS * SMs consecutive tiles (the same L2 locality as block-order scheduling), every SM gets
+// the same number of tiles up to one, and the surplus tiles of the last round land on group 0 of different SMs, where
+// each has an SM's FP64 pipe to itself; (3) the register file is split with setmaxnreg (producers 32, consumers 160).
+template <class TC, bool FULL>
+__device__ __forceinline__ void ws_consume_tile(const GemmParams& P, const uint8_t* ring, uint32_t bar_full, uint32_t bar_empty,
+                                                int lane, int nk, int nbm, int nbn, uint32_t offA0, uint32_t offA1,
+                                                uint32_t offB0, uint32_t offB1, uint32_t& slot, uint32_t& phase,
+                                                double (&p1)[TC::MB][TC::NB][2], double (&p2)[TC::MB][TC::NB][2],
+                                                double (&p3)[TC::MB][TC::NB][2]) {
+    constexpr int MB = TC::MB, NB = TC::NB, STAGES = TC::STAGES, STAGE_BYTES = TC::STAGE_BYTES;
+    const int N = P.N;
+    const bool active = FULL || ((nbm > 0) && (nbn > 0));
+    for (int it = 0; it < nk; ++it) {
+        asm volatile("" : "+r"(offA0), "+r"(offA1), "+r"(offB0), "+r"(offB1));
+        mbar_wait(bar_full + 8 * slot, phase);
+        if (active) {
+            const uint8_t* st = ring + slot * STAGE_BYTES;
+            const int nsub = (it * BK + 1 < N) ? 2 : 1;  // odd k-slots of the last slice may all be padding
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                if (s < nsub) {
+                    double2 a[MB], b[NB];
+                    double as[MB], bs[NB];
+#pragma unroll
+                    for (int bm = 0; bm < MB; ++bm) {
+                        a[bm] = *reinterpret_cast<const double2*>(st + (s ? offA1 : offA0) + bm * 1024);
+                        as[bm] = a[bm].x + a[bm].y;
+                    }
+#pragma unroll
+                    for (int bn = 0; bn < NB; ++bn) {
+                        b[bn] = *reinterpret_cast<const double2*>(st + (s ? offB1 : offB0) + bn * B_BOX_BYTES);
+                        bs[bn] = b[bn].x + b[bn].y;
+                    }
+                    if constexpr (FULL) {
+#pragma unroll
+                        for (int bm = 0; bm < MB; ++bm)
+#pragma unroll
+                            for (int bn = 0; bn < NB; ++bn) {
+                                dmma(p1[bm][bn][0], p1[bm][bn][1], a[bm].x, b[bn].x);
+                                dmma(p2[bm][bn][0], p2[bm][bn][1], a[bm].y, b[bn].y);
+                                dmma(p3[bm][bn][0], p3[bm][bn][1], as[bm], bs[bn]);
+                            }
+                    } else {
+#pragma unroll
+                        for (int bm = 0; bm < MB; ++bm)
+                            if (bm < nbm) {
+#pragma unroll
+                                for (int bn = 0; bn < NB; ++bn)
+                                    if (bn < nbn) {
+                                        dmma(p1[bm][bn][0], p1[bm][bn][1], a[bm].x, b[bn].x);
+                                        dmma(p2[bm][bn][0], p2[bm][bn][1], a[bm].y, b[bn].y);
+                                        dmma(p3[bm][bn][0], p3[bm][bn][1], as[bm], bs[bn]);
+                                    }
+                            }
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
+        if (++slot == STAGES) {
+            slot = 0;
+            phase ^= 1u;
+        }
+    }
+}
+
+template <class TC, int GROUPS, int PRODUCER_REGS, int CONSUMER_REGS>
+__global__ void __launch_bounds__(128 * (GROUPS + 1), 1)
+zgemm_modes_dmma_ws_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
+                           const GemmParams P) {
+    constexpr int MB = TC::MB, NB = TC::NB, STAGES = TC::STAGES, STAGE_BYTES = TC::STAGE_BYTES;
+    constexpr int BM = TC::BM, BN = TC::BN;
+    constexpr int RING_BYTES = STAGES * STAGE_BYTES;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));
+    const uint32_t bars = base + GROUPS * RING_BYTES;   // per group: STAGES full barriers, then STAGES empty barriers
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wg = warp >> 2;
+    const int tiles = P.tiles_m * P.tiles_n;
+    const int per_product = tiles * P.nmodes;
+    const int total = P.ngroups * per_product;
+    const int stride = GROUPS * (int)gridDim.x;
+    const int N = P.N;
+    const int nk = (N + BK - 1) / BK;
+
+    if (threadIdx.x == 0) {
+        for (int q = 0; q < GROUPS; ++q)
+            for (int s = 0; s < STAGES; ++s) {
+                mbar_init(bars + (q * 2 * STAGES + s) * 8, 1);
+                mbar_init(bars + (q * 2 * STAGES + STAGES + s) * 8, TC::WARPS);
+            }
+        mbar_fence_init();
+    }
+    pdl_wait();
+    pdl_trigger();
+    __syncthreads();
+
+    if (wg == 0) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PRODUCER_REGS));
+        if (warp < GROUPS && lane == 0) {
+            const uint32_t ring = base + warp * RING_BYTES;
+            const uint32_t bar_full = bars + warp * 2 * STAGES * 8, bar_empty = bar_full + STAGES * 8;
+            uint32_t slot = 0, phase = 0;
+            for (int tl = warp * (int)gridDim.x + (int)blockIdx.x; tl < total; tl += stride) {
+                const int grp = tl / per_product, rest = tl - grp * per_product;
+                const int mode = rest / tiles, tile = rest - mode * tiles;
+                const int m0 = (tile / P.tiles_n) * BM, n0 = (tile % P.tiles_n) * BN;
+                const int modeA = P.g[grp].aoff + mode, modeB = P.g[grp].boff + mode;
+                for (int it = 0; it < nk; ++it) {
+                    mbar_wait(bar_empty + 8 * slot, phase ^ 1u);
+                    issue_slice<TC>(&mapA, &mapB, ring + slot * STAGE_BYTES, bar_full + 8 * slot, it * BK, m0, n0, modeA, modeB);
+                    if (++slot == STAGES) {
+                        slot = 0;
+                        phase ^= 1u;
+                    }
+                }
+            }
+        }
+        return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(CONSUMER_REGS));
+    const int q = wg - 1, w4 = warp & 3;
+    const uint8_t* ring = sgen + q * RING_BYTES;
+    const uint32_t bar_full = bars + q * 2 * STAGES * 8, bar_empty = bar_full + STAGES * 8;
+    const int g = lane >> 2, t = lane & 3;
+    uint32_t slot = 0, phase = 0;
+    for (int tl = q * (int)gridDim.x + (int)blockIdx.x; tl < total; tl += stride) {
+        const int grp = tl / per_product, rest = tl - grp * per_product;
+        const int mode = rest / tiles, tile = rest - mode * tiles;
+        const int m0 = (tile / P.tiles_n) * BM, n0 = (tile % P.tiles_n) * BN;
+        // rotate the warp -> quarter-tile assignment with the tile: edge tiles give the warps unequal work
+        const int quad = (w4 + tl) & (TC::WARPS - 1);
+        const int wm = quad / TC::WN, wn = quad % TC::WN;
+        const int mw = 8 * MB * wm, nw = 8 * NB * wn;
+        int nbm = (N - (m0 + mw) + 7) >> 3;
+        nbm = nbm < 0 ? 0 : (nbm > MB ? MB : nbm);
+        int nbn = (N - (n0 + nw) + 7) >> 3;
+        nbn = nbn < 0 ? 0 : (nbn > NB ? NB : nbn);
+        double p1[MB][NB][2], p2[MB][NB][2], p3[MB][NB][2];
+#pragma unroll
+        for (int i = 0; i < MB; ++i)
+#pragma unroll
+            for (int j = 0; j < NB; ++j) {
+                p1[i][j][0] = p1[i][j][1] = 0.0;
+                p2[i][j][0] = p2[i][j][1] = 0.0;
+                p3[i][j][0] = p3[i][j][1] = 0.0;
+            }
+        const uint32_t offA0 = (uint32_t)((mw + g) * 128 + (((2 * t) ^ g) << 4));
+        const uint32_t offA1 = offA0 ^ 16u;
+        const uint32_t offB0 =
+            (uint32_t)(TC::A_STAGE_BYTES + (NB * wn) * B_BOX_BYTES + (2 * t) * 128 + ((g ^ (2 * t)) << 4));
+        const uint32_t offB1 = (offB0 + 128u) ^ 16u;
+        if (nbm == MB && nbn == NB)
+            ws_consume_tile<TC, true>(P, ring, bar_full, bar_empty, lane, nk, nbm, nbn, offA0, offA1, offB0, offB1, slot, phase, p1,
+                                      p2, p3);
+        else
+            ws_consume_tile<TC, false>(P, ring, bar_full, bar_empty, lane, nk, nbm, nbn, offA0, offA1, offB0, offB1, slot, phase, p1,
+                                       p2, p3);
+        if (nbm > 0 && nbn > 0) gemm_epilogue<TC>(P, P.g[grp], mode, m0, n0, mw, nw, nbm, nbn, g, t, p1, p2, p3);
     }
 }
 
@@ -467,9 +703,37 @@ cudaError_t launch_dmma(const FreqLayout& f, const double* baseA, int modesA, co
     P.tiles_n = (f.N + TC::BN - 1) / TC::BN;
     CUtensorMap mapA, mapB;
     if ((e = encode_operand(&mapA, baseA, f, modesA, TC::BM)) != cudaSuccess) return e;
-    if ((e = encode_operand_b4(&mapB, baseB, f, modesB, TC::BN / 8)) != cudaSuccess) return e;
+    if (P.conv)   // a caller's array: plain 3-D map, one box per eight columns
+        e = encode_operand(&mapB, baseB, f, modesB, BK);
+    else
+        e = encode_operand_b4(&mapB, baseB, f, modesB, TC::BN / 8);
+    if (e != cudaSuccess) return e;
     const unsigned grid = (unsigned)(P.ngroups * P.nmodes * P.tiles_m * P.tiles_n);
     return launch_pdl(zgemm_modes_dmma_kernel<TC>, grid, TC::THREADS, TC::SMEM_BYTES, st, mapA, mapB, P);
+}
+
+template <class TC, int GROUPS, int PREGS, int CREGS>
+cudaError_t launch_dmma_ws(const FreqLayout& f, const double* baseA, int modesA, const double* baseB, int modesB, GemmParams P,
+                           cudaStream_t st) {
+    constexpr int SMEM = GROUPS * TC::STAGES * TC::STAGE_BYTES + GROUPS * 2 * TC::STAGES * 8 + 1024;
+    static bool attr_done[NSPT_MAX_DEVICES] = {};
+    static int sms[NSPT_MAX_DEVICES] = {};
+    cudaError_t e;
+    const int dev = current_device();
+    auto kern = zgemm_modes_dmma_ws_kernel<TC, GROUPS, PREGS, CREGS>;
+    if (!attr_done[dev]) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+        if (e != cudaSuccess) return e;
+        cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev);
+        if (sms[dev] <= 0) sms[dev] = 148;
+        attr_done[dev] = true;
+    }
+    P.tiles_m = (f.N + TC::BM - 1) / TC::BM;
+    P.tiles_n = (f.N + TC::BN - 1) / TC::BN;
+    CUtensorMap mapA, mapB;
+    if ((e = encode_operand(&mapA, baseA, f, modesA, TC::BM)) != cudaSuccess) return e;
+    if ((e = encode_operand_b4(&mapB, baseB, f, modesB, TC::BN / 8)) != cudaSuccess) return e;
+    return launch_pdl(kern, (unsigned)sms[dev], 128 * (GROUPS + 1), SMEM, st, mapA, mapB, P);
 }
 
 GemmGroupDev to_dev(const GemmOut& out) {
@@ -505,7 +769,7 @@ cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup*
         }
         return cudaSuccess;
     }
-    if (variant != 1) return cudaErrorInvalidValue;
+    if (variant != 1 && variant != 3) return cudaErrorInvalidValue;
     // one tensor map per operand side spans every group's spectrum: the groups address it by mode offset, so
     // their operands must sit a whole number of N x N matrices apart (spectra of one workspace always do)
     const double* baseA = groups[0].A;
@@ -540,9 +804,33 @@ cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup*
     // N = 121: 67 / 48, 169: 119 / 111, 200: 172 / 156, 256: 306 / 268, 289: 449 / 430, 400: 988 / 979 (B wins);
     // N = 144: 72 / 74, 192: 122 / 126, 225: 213 / 226, 240: 220 / 244 (A wins); N = 184 (nb = 23): 126 / 121, hence nb >= 29 for the 'nearly' case.
     const int nb = (f.N + 7) / 8;
+    if (variant == 3) return launch_dmma_ws<Tile<3, 3, 2, 2, 3, 5>, 3, 32, 160>(f, baseA, (int)maxA + modes, baseB, (int)maxB + modes, P, st);
     if (nb % 6 == 0 || (nb % 6 == 5 && nb >= 29))
         return launch_dmma<Tile<3, 3, 2, 2, 3, 5>>(f, baseA, (int)maxA + modes, baseB, (int)maxB + modes, P, st);
     return launch_dmma<Tile<2, 2, 2, 2, 5, 5>>(f, baseA, (int)maxA + modes, baseB, (int)maxB + modes, P, st);
+}
+
+// Naive-CONV (eq. 2.5 evaluated directly): C^(k) = sum_{l<=k} A^(l) B^(k-l) as ONE launch of the tensor-pipe
+// kernel, each order a matrix product whose K dimension is concatenated over l.  No transforms, no workspace; N^3 n(n+1)/2
+// multiplications instead of N^3 L, so it wins only for very low orders or launch-bound sizes.  C must not alias A or B.
+cudaError_t launch_naive_conv(const FreqLayout& f, int batch, const nspt_c128* A, const nspt_c128* B, nspt_c128* C,
+                              cudaStream_t st) {
+    GemmParams P{};
+    P.NN = f.NN;
+    P.N = f.N;
+    P.L = f.n;
+    P.nmodes = batch * f.n;
+    P.ngroups = 1;
+    P.conv = 1;
+    P.n = f.n;
+    P.g[0].C = reinterpret_cast<double2*>(C);
+    P.g[0].alpha_re = 1.0;
+    const double* a = reinterpret_cast<const double*>(A);
+    const double* b = reinterpret_cast<const double*>(B);
+    const int nb = (f.N + 7) / 8;
+    if (nb % 6 == 0 || (nb % 6 == 5 && nb >= 29))
+        return launch_dmma<Tile<3, 3, 2, 2, 3, 5>>(f, a, P.nmodes, b, P.nmodes, P, st);
+    return launch_dmma<Tile<2, 2, 2, 2, 5, 5>>(f, a, P.nmodes, b, P.nmodes, P, st);
 }
 
 cudaError_t launch_zgemm_modes(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out,

@@ -23,9 +23,11 @@ def nspt():
     binding.use_current_stream()
     binding.nspt_set_order_scale(1.0)
     binding.nspt_set_gemm_variant(1)
+    binding.nspt_set_conv_algorithm(0)
     yield binding
     binding.nspt_set_order_scale(1.0)
     binding.nspt_set_gemm_variant(1)
+    binding.nspt_set_conv_algorithm(0)
 
 
 def to_dev(x):
@@ -157,6 +159,80 @@ def test_int8_sliced_product_at_config2(nspt):
         check_product(nspt, A, B)
     finally:
         nspt.nspt_set_gemm_variant(1)
+
+
+# ----------------------------------------------------------------------------- gemm variant 3: persistent warp-specialised DMMA
+
+@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (9, 7), (47, 15), (49, 15), (100, 31), (145, 3), (225, 15), (240, 7)])
+def test_persistent_gemm_matches_oracle(nspt, N, Ntrunc):
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([6, N, Ntrunc])
+    A = wl.gaussian_series(N, Ntrunc, rng)
+    B = wl.gaussian_series(N, Ntrunc, rng)
+    nspt.nspt_set_gemm_variant(3)
+    try:
+        check_product(nspt, A, B)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+
+
+def test_persistent_gemm_staple_and_exp(nspt):
+    # grouped launches, accumulating and conjugate-transposed epilogues through the persistent kernel
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(48)
+    U = [wl.unitary_series(50, 7, rng) for _ in range(4)]
+    z = wl.twist_tensor(7, 1)
+    X = anti_hermitian_series(33, 15, seed=49)
+    nspt.nspt_set_gemm_variant(3)
+    try:
+        check_staple(nspt, U, z)
+        err = oracle.per_order_error(gpu_exp(nspt, X), oracle.series_exp(X), oracle.exp_bound(X))
+        assert err.max() <= TOL
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+
+
+# ----------------------------------------------------------------------------- Naive-CONV on the GPU
+
+@pytest.mark.parametrize("alg", [1, 2])
+@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (1, 5), (3, 2), (9, 7), (17, 1), (47, 3), (48, 15), (50, 12), (97, 5), (100, 31),
+                                      (225, 3)])
+def test_both_convolution_algorithms_match_oracle(nspt, N, Ntrunc, alg):
+    # eq. 2.5 evaluated directly on the tensor pipe (K concatenated over the order index) and by FFT-CONV (Steps 1-5)
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([7, N, Ntrunc])
+    A = wl.gaussian_series(N, Ntrunc, rng)
+    B = wl.gaussian_series(N, Ntrunc, rng)
+    nspt.nspt_set_conv_algorithm(alg)
+    try:
+        check_product(nspt, A, B)
+    finally:
+        nspt.nspt_set_conv_algorithm(0)
+
+
+def test_naive_conv_integer_bit_exact_batched_and_aliased(nspt):
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([8, 57, 9])
+    A = np.stack([wl.integer_series(57, 9, rng) for _ in range(3)])
+    B = np.stack([wl.integer_series(57, 9, rng) for _ in range(3)])
+    nspt.nspt_set_conv_algorithm(2)
+    try:
+        C = nspt.nspt_series_mul_batched(to_dev(A), to_dev(B))
+        torch.cuda.synchronize()
+        C = C.cpu().numpy()
+        for b in range(3):
+            assert np.array_equal(C[b], oracle.series_mul(A[b], B[b]))     # no transform: exact, not just after rounding
+        # an output that aliases an input cannot use the direct form (it would read what it has overwritten)
+        dA, dB = to_dev(A[0]), to_dev(B[0])
+        nspt.nspt_series_mul(dA, dB, dA)
+        torch.cuda.synchronize()
+        ref = oracle.series_mul(A[0], B[0])
+        assert np.array_equal(np.round(dA.cpu().numpy().real), ref.real)
+    finally:
+        nspt.nspt_set_conv_algorithm(0)
 
 
 def test_unit_and_zero(nspt):
