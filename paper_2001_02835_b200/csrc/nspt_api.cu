@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "nspt_internal.cuh"
+#include "nspt_ozaki.cuh"
 
 namespace nspt {
 namespace {
@@ -189,7 +190,7 @@ void exp_split(int Ntrunc, int* s, int* r) {
 constexpr size_t WS_PAD = 256;
 
 size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
-    if (op == NSPT_OP_SERIES_MUL && g.gemm_variant == 2) return 3 * spectrum_bytes(f, batch) + WS_PAD + ozaki_workspace_bytes(f, batch);
+    if (op == NSPT_OP_SERIES_MUL && (g.gemm_variant == 2 || g.gemm_variant >= 4)) return 3 * spectrum_bytes(f, batch) + WS_PAD + ozaki_workspace_bytes(f, batch);
     if (op == NSPT_OP_STAPLE) return 30 * spectrum_bytes(f, 1) + WS_PAD;
     if (op == NSPT_OP_SERIES_EXP) {
         int s, r;
@@ -316,13 +317,13 @@ int k_dagger(const FreqLayout& f, int batch, const double* src, double* dst) {
 int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_GEMM));
-    NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, out, g.gemm_variant == 2 ? 1 : g.gemm_variant, g.stream));
+    NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, out, (g.gemm_variant == 2 || g.gemm_variant >= 4) ? 1 : g.gemm_variant, g.stream));
     return tm.end();
 }
 int k_gemm_groups(const FreqLayout& f, const GemmGroup* groups, int ngroups, int batch = 1) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_GEMM));
-    NSPT_CUDA(launch_zgemm_groups(f, batch, groups, ngroups, g.gemm_variant == 2 ? 1 : g.gemm_variant, g.stream));
+    NSPT_CUDA(launch_zgemm_groups(f, batch, groups, ngroups, (g.gemm_variant == 2 || g.gemm_variant >= 4) ? 1 : g.gemm_variant, g.stream));
     return tm.end();
 }
 int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, double* C) {
@@ -370,10 +371,53 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
     double* At = reinterpret_cast<double*>(ws);
     double* Bt = reinterpret_cast<double*>(ws + sb);
     double* Ct = reinterpret_cast<double*>(ws + 2 * sb);
+    // gemm variants: 1 = FP64 tensor pipe; 2 = INT8 tensor cores (forward transform tracks the per-mode maxima, slicing pass,
+    // persistent tcgen05 kernel); diagnostics: 4 = first-generation INT8 path, 5 = forward transform writes the slices itself,
+    // 6 = variant 2 with CTA pairs (cta_group::2)
+    const int gv = g.gemm_variant;
+    const bool int8 = gv == 2 || gv >= 4;
+    if (gv == 5 && fft_slices_supported(f.L)) {
+        void* oz = ws + 3 * sb + WS_PAD;
+        OzSliceDst da, db;
+        ozaki_slice_targets(f, batch, oz, &da, &db);
+        {
+            StageTimer tm;
+            NSPT_TRY(tm.begin(ST_FWD));
+            NSPT_CUDA(launch_fft_forward_slices(f, t, batch, A, da, B, db, g.stream));
+            NSPT_TRY(tm.end());
+        }
+        StageTimer tm;
+        NSPT_TRY(tm.begin(ST_GEMM));
+        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream, 1));
+        NSPT_TRY(tm.end());
+    } else if (int8 && gv != 4 && f.L >= 16) {
+        void* oz = ws + 3 * sb + WS_PAD;
+        OzSliceDst da, db;
+        ozaki_slice_targets(f, batch, oz, &da, &db);
+        {
+            // Steps 1-2 (eqs. 2.6-2.7); the transform also records max(|re|, |im|) of every mode of both spectra
+            StageTimer tm;
+            NSPT_TRY(tm.begin(ST_FWD));
+            NSPT_CUDA(cudaMemsetAsync(da.maxbits, 0, sizeof(unsigned long long) * 2 * batch * f.L, g.stream));
+            NSPT_CUDA(launch_fft_forward(f, t, batch, A, At, B, Bt, g.stream, false, da.maxbits, db.maxbits));
+            NSPT_TRY(tm.end());
+        }
+        {
+            StageTimer tm;
+            NSPT_TRY(tm.begin(ST_SLICE));
+            NSPT_CUDA(launch_ozaki_slice2(f, batch, At, Bt, oz, g.stream));
+            NSPT_TRY(tm.end());
+        }
+        // Step 3 (eq. 2.8) on the INT8 tensor cores
+        StageTimer tm;
+        NSPT_TRY(tm.begin(ST_GEMM));
+        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream, gv == 6 ? 2 : 1));
+        NSPT_TRY(tm.end());
+    } else {
     // Steps 1-2 (eqs. 2.6-2.7): zero-padded forward transforms of A and B, one launch
     NSPT_TRY(k_forward(f, t, batch, A, At, B, Bt));
     // Step 3 (eq. 2.8): mode-wise matrix products
-    if (g.gemm_variant == 2) {
+    if (int8) {
         void* oz = ws + 3 * sb + WS_PAD;
         {
             StageTimer tm;
@@ -383,10 +427,11 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
         }
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_GEMM));
-        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream));
+        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream, 0));
         NSPT_TRY(tm.end());
     } else {
         NSPT_TRY(k_gemm(f, batch, At, Bt, Ct));
+    }
     }
     // Steps 4-5 (eq. 2.9): inverse transform, 1/L, truncation
     NSPT_TRY(k_inverse(f, t, batch, Ct, C));
@@ -770,7 +815,7 @@ int nspt_set_workspace(void* dptr, size_t bytes) {
 
 int nspt_set_gemm_variant(int variant) {
     NSPT_LOCK();
-    if (variant < 0 || variant > 3) return NSPT_EINVAL;
+    if (variant < 0 || variant > 6) return NSPT_EINVAL;
     g.gemm_variant = variant;
     return NSPT_OK;
 }

@@ -70,7 +70,8 @@ struct Cplx { double re, im; };
 cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int batch,
                                const nspt_c128* src0, double* dst0,
                                const nspt_c128* src1, double* dst1, cudaStream_t st,
-                               bool skip_order0 = false);
+                               bool skip_order0 = false, unsigned long long* maxbits0 = nullptr,
+                               unsigned long long* maxbits1 = nullptr);
 // Inverse + 1/L + truncation (+ unscale): spectrum -> series.
 cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int batch,
                                const double* src, nspt_c128* dst, cudaStream_t st);
@@ -128,6 +129,7 @@ cudaError_t launch_naive_conv(const FreqLayout& f, int batch, const nspt_c128* A
 // (launch_ozaki_slice), multiplied exactly by tcgen05.mma.kind::i8 and recombined in FP64 (launch_ozaki_gemm).
 size_t ozaki_workspace_bytes(const FreqLayout& f, int batch);
 cudaError_t launch_ozaki_slice(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st);
-cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st);
+cudaError_t launch_ozaki_slice2(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st);
+cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st, int kernel = -1);
 
 }  // namespace nspt

@@ -20,15 +20,16 @@
 // after the other through the same accumulators; eight epilogue warps drain them with tcgen05.ld, recombine the seven
 // INT32 sums in FP64 (Horner in 2^-8) and keep the running real / imaginary parts of the 3M product in registers.
 #include <cuda.h>
+#include <cstdio>
+#include <cstdlib>
 
 #include "nspt_internal.cuh"
+#include "nspt_ozaki.cuh"
 #include "nspt_tma.cuh"
 
 namespace nspt {
 namespace {
 
-constexpr int OZ_S = 7;                              // slices per plane
-constexpr int OZ_PLANES = 3;                         // re, im, re + im
 // Operand staging, measured on B200 with probes of the TMA unit and of tcgen05.mma.kind::i8: the TMA unit is row-rate bound
 // (1.9 cycles per row of <= 128 bytes with all SMs loading), so every shared-memory row is 128 bytes; a 128 x 64 x 32 MMA
 // takes 46-58 cycles depending on the operand layouts (32 would be the tensor rate, reached only from N = 128 up, which the
@@ -48,7 +49,6 @@ constexpr int OZ_STAGE = OZ_M_STAGE + OZ_N_STAGE;    // 45056
 constexpr int OZ_SMEM = OZ_STAGES * OZ_STAGE + 1024 + 128;
 constexpr int OZ_THREADS = 384;                      // warp 0 TMA, warp 1 MMA, warp 2 TMEM allocator, warps 4-11 epilogue
 constexpr int OZ_TMEM_COLS = 512;
-constexpr int OZ_FRAC_BITS = 54;                     // v = rint(x 2^(54-e)), |v| <= 2^54
 
 static_assert(OZ_STAGE % 1024 == 0 && OZ_M_STAGE % 1024 == 0, "stage alignment");
 
@@ -75,25 +75,6 @@ __global__ void __launch_bounds__(256) oz_absmax_kernel(const double2* __restric
         atomicMax(maxbits + mode, (unsigned long long)__double_as_longlong(m));
     }
     }
-}
-
-// exponent e with max < 2^e from the bit pattern of the mode's maximum (0 for an all-zero mode)
-__device__ __forceinline__ int oz_exponent(unsigned long long bits) {
-    const int field = (int)((bits >> 52) & 0x7ff);
-    if (bits == 0ull) return 0;
-    if (field == 0x7ff) return 1 << 20;   // Inf / NaN in the spectrum: the product kernel answers NaN
-    return field - 1022;   // max = m 2^(field-1023) with m in [1,2)  ->  max < 2^(field-1022)
-}
-__device__ __forceinline__ double oz_pow2(int k) {   // 2^k, k in [-1022, 1023]
-    k = k < -1022 ? -1022 : (k > 1023 ? 1023 : k);
-    return __longlong_as_double((long long)(k + 1023) << 52);
-}
-// the seven digits of v = rint(x * scale), |v| <= 2^54, packed in bytes 0..6 of the result: byte j holds the balanced digit
-// of weight 256^j (two's-complement int8), byte 6 the leading digit in [-64, 64]
-__device__ __forceinline__ unsigned long long oz_digits(double x, double scale) {
-    const long long v = __double2ll_rn(x * scale);
-    const unsigned long long u = (unsigned long long)v + 0x0000808080808080ull;   // + 128 at digits 0..5
-    return u ^ 0x0000808080808080ull;                                              // digit - 128 as int8
 }
 
 // Slice layouts in global memory (both from row-major FP64 spectra X[mode][row][col]):
@@ -143,6 +124,115 @@ __global__ void __launch_bounds__(256) oz_slice_kernel(const double2* __restrict
     }
 }
 
+// Second-generation slicing pass: both operands in one launch (blockIdx.z), the per-mode maxima come from the forward
+// transform (maxbits), digits without 64-bit conversions (oz_digits2), 4 x 4 byte transposes for the packing.
+// thread = 4 consecutive columns of a row of one mode; a warp writes 128 contiguous bytes per (plane, slice).
+struct Slice2Params {
+    const double2* X[2];
+    int8_t* out[2];
+    const unsigned long long* maxbits[2];
+    int* exps[2];
+    int pitch[2];
+    int N, modes;
+};
+constexpr int OZ_SLICE_MODES = 8;   // consecutive modes per thread: the loads of the next mode are in flight while one is cut
+// the 21 slice words of four columns of one mode: re and im planes from the fixed-point integers V1, V2, the re + im plane from
+// floor((V1 + V2) / 2) (same accuracy as rounding (re + im) / 2, without a third conversion)
+__device__ __forceinline__ void oz_slice_store4(const double2 (&v)[4], double sc, int8_t* base, size_t plane_stride, size_t slice_stride) {
+    unsigned int lo[OZ_PLANES][4], hi[OZ_PLANES][4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const long long v1 = oz_fixed(v[c].x, sc), v2 = oz_fixed(v[c].y, sc);
+        oz_digits_of(v1, lo[0][c], hi[0][c]);
+        oz_digits_of(v2, lo[1][c], hi[1][c]);
+        oz_digits_of((v1 + v2) >> 1, lo[2][c], hi[2][c]);
+    }
+#pragma unroll
+    for (int q = 0; q < OZ_PLANES; ++q) {
+        unsigned int w[8];
+        transpose4x4(lo[q], w);
+        transpose4x4(hi[q], w + 4);
+        int8_t* p = base + (size_t)q * plane_stride + (size_t)(OZ_S - 1) * slice_stride;
+#pragma unroll
+        for (int d = 0; d < OZ_S; ++d) {   // word d = digit of weight 256^d of the four columns = slice 6 - d
+            *reinterpret_cast<unsigned int*>(p) = w[d];
+            p -= slice_stride;
+        }
+    }
+}
+// The spectrum of a mode is one contiguous array of N^2 elements and the 256 threads of a CTA (row-aligned groups of four
+// columns, row-major) cover one contiguous range of it: the CTA copies that range to shared memory with 16-byte cp.async
+// (coalesced, no registers, two modes in flight) and every thread then picks up its four columns from there.
+constexpr int OZ_SLICE_BUF = 1024 + 8;   // elements per stage (256 groups of 4, plus slack for the row ends)
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int PENDING>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(PENDING) : "memory"); }
+// position of element p of the staged range: XOR of the low two bits with bits 3-4, so that the 16-byte reads of a quarter
+// warp (stride four elements) cover all banks
+__device__ __forceinline__ int oz_swz(int p) { return p ^ ((p >> 3) & 3); }
+
+__global__ void __launch_bounds__(256) oz_slice2_kernel(const Slice2Params P) {
+    __shared__ double2 stage[2][OZ_SLICE_BUF];
+    __shared__ double ssc[OZ_SLICE_MODES];
+    const int z = blockIdx.z;
+    const bool quad = (z == 0);
+    const double2* X = z ? P.X[1] : P.X[0];
+    int8_t* O = z ? P.out[1] : P.out[0];
+    const unsigned long long* MB = z ? P.maxbits[1] : P.maxbits[0];
+    int* EX = z ? P.exps[1] : P.exps[0];
+    const int N = P.N, pitch = z ? P.pitch[1] : P.pitch[0];
+    const int qpr = quad ? (pitch >> 5) : ((N + 3) >> 2);   // 4-column groups per row (QUAD: the k padding is written too)
+    const int total = N * qpr;
+    const int t0 = blockIdx.x * 256, t = t0 + threadIdx.x;
+    const int m_begin = blockIdx.y * OZ_SLICE_MODES;
+    const int nm = P.modes - m_begin < OZ_SLICE_MODES ? P.modes - m_begin : OZ_SLICE_MODES;
+    // contiguous element range of this CTA: from the first column of its first group to the end of its last group
+    const int tl = (t0 + 255 < total ? t0 + 255 : total - 1);
+    const int c0 = 4 * (t0 % qpr), c1 = 4 * (tl % qpr) + 4;
+    const int e0 = (t0 / qpr) * N + (c0 < N ? c0 : N), e1 = (tl / qpr) * N + (c1 < N ? c1 : N);
+    const int count = e1 - e0;   // <= OZ_SLICE_BUF
+    pdl_wait();
+    pdl_trigger();
+    if (threadIdx.x < nm) {
+        const int e = oz_exponent(MB[m_begin + threadIdx.x]);
+        ssc[threadIdx.x] = oz_pow2(OZ_FRAC_BITS - e);
+        if (blockIdx.x == 0) EX[m_begin + threadIdx.x] = e;
+    }
+    auto fetch = [&](int i) {   // mode m_begin + i -> stage i & 1
+        if (i < nm) {
+            const double2* src = X + (size_t)(m_begin + i) * N * N + e0;
+            const uint32_t dst = smem_u32(&stage[i & 1][0]);
+            for (int p = threadIdx.x; p < count; p += 256) cp_async16(dst + 16u * (uint32_t)oz_swz(p), src + p);
+        }
+        cp_async_commit();
+    };
+    fetch(0);
+    const bool active = t < total;
+    const int row = active ? t / qpr : 0, j0 = active ? (t % qpr) * 4 : 0;
+    const int nvalid = active ? N - j0 : 0;   // columns of this group inside the matrix (<= 0: k padding of the QUAD layout)
+    const int p0 = row * N + j0 - e0;
+    const size_t plane_stride = quad ? (size_t)N * pitch : (size_t)OZ_S * N * pitch;
+    const size_t slice_stride = quad ? (size_t)32 : (size_t)N * pitch;
+    const size_t mode_stride = (size_t)OZ_PLANES * plane_stride;
+    int8_t* out = O + (size_t)m_begin * mode_stride + (size_t)row * pitch + (quad ? (size_t)(j0 >> 5) * 256 + (j0 & 31) : (size_t)j0);
+#pragma unroll 1
+    for (int i = 0; i < nm; ++i) {
+        fetch(i + 1);
+        cp_async_wait<1>();
+        __syncthreads();   // mode i has landed (and the scales, first time round)
+        if (active) {
+            double2 v[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) v[c] = c < nvalid ? stage[i & 1][oz_swz(p0 + c)] : make_double2(0.0, 0.0);
+            oz_slice_store4(v, ssc[i], out + (size_t)i * mode_stride, plane_stride, slice_stride);
+        }
+        __syncthreads();   // stage i & 1 may be refilled
+    }
+}
+
 // ---- tcgen05 wrappers ---------------------------------------------------------------------------------------
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -184,6 +274,12 @@ __device__ __forceinline__ void tc_commit(uint32_t bar) {
 __device__ __forceinline__ void tc_ld8(uint32_t taddr, int (&r)[8]) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr)
+                 : "memory");
+}
+__device__ __forceinline__ void tc_ld4(uint32_t taddr, int (&r)[4]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
                  : "r"(taddr)
                  : "memory");
 }
@@ -362,6 +458,402 @@ zgemm_modes_ozaki_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_
     if (warp == 2) tc_dealloc(tmem, OZ_TMEM_COLS);
 }
 
+
+// =====================================================================================================================
+// Second-generation kernel: persistent, one tile per CTA PAIR (tcgen05.mma.cta_group::2, M = 256) or per CTA (CG = 1).
+// The pair computes a 256 (j) x 64 (i) tile: each CTA keeps the seven 128 x 64 INT32 accumulators of its own 128 output
+// columns j in its own TMEM and stages its own half of both operands -- the M-side slices of its 128 columns and 32 of the 64
+// rows of the N-side slices -- so a stage is 36 KB per SM instead of 44 KB and every byte of the N-side operand is read from
+// shared memory by one SM only (the single-CTA kernel above is bound by shared-memory and L2 bandwidth, not by the tensor
+// core).  The leader CTA issues the MMAs for both; TMA loads of both CTAs report to the leader's "full" barrier, MMA
+// completion is multicast to both CTAs' "empty" / "accumulator full" barriers, and the epilogue warps of both CTAs report to
+// the leader's "accumulator empty" barrier.  CTAs are persistent (static round-robin schedule over tiles): barrier set-up and
+// the TMEM allocation happen once, the producer runs ahead into the next tile while the accumulators drain, and the final
+// scaling and stores of a tile overlap the next tile's MMAs.
+// =====================================================================================================================
+constexpr int OZ2_BN = 64;
+constexpr int OZ2_THREADS = 384;
+template <int CG>
+struct Oz2 {
+    static constexpr int N_ROWS = OZ2_BN / CG;               // rows of the N-side operand staged by one CTA
+    static constexpr int N_HALF = N_ROWS * 128;              // slices 4h..4h+3 of a stage
+    static constexpr int N_STAGE = 2 * N_HALF;
+    static constexpr int STAGE = OZ_M_STAGE + N_STAGE;       // 45056 (CG = 1) / 36864 (CG = 2)
+    static constexpr int STAGES = CG == 2 ? 5 : 4;
+    static constexpr int SMEM = STAGES * STAGE + 1024 + 256;
+    static constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (0u << 16) | ((OZ2_BN >> 3) << 17) |
+                                      (((128 * CG) >> 4) << 24);
+    static_assert(STAGE % 1024 == 0, "stage alignment");
+};
+
+__device__ __forceinline__ uint32_t cluster_rank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of the same shared-memory location in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa_rank(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// mbarrier wait with a watchdog: a protocol error traps instead of hanging the GPU
+__device__ __forceinline__ void mbar_wait_wd(uint32_t bar, uint32_t parity) {
+    uint32_t done = 0;
+    for (unsigned long long spins = 0; !done; ++spins) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+        if (spins > (1ull << 22)) __trap();
+    }
+}
+template <int CG, int COLLECT>
+__device__ __forceinline__ void tc_mma_i8_cg(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+#define NSPT_OZ_MMA2(G, Q)                                                                         \
+    asm volatile(                                                                                  \
+        "{\n"                                                                                      \
+        ".reg .pred p;\n"                                                                          \
+        "setp.ne.b32 p, %4, 0;\n"                                                                  \
+        "tcgen05.mma.cta_group::" G ".kind::i8" Q " [%0], %1, %2, %3, p;\n"                        \
+        "}\n" ::"r"(d_tmem),                                                                       \
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)                                      \
+        : "memory")
+    if constexpr (CG == 2) {
+        if constexpr (COLLECT == 1) NSPT_OZ_MMA2("2", ".collector::a::fill");
+        else if constexpr (COLLECT == 2) NSPT_OZ_MMA2("2", ".collector::a::use");
+        else if constexpr (COLLECT == 3) NSPT_OZ_MMA2("2", ".collector::a::lastuse");
+        else NSPT_OZ_MMA2("2", "");
+    } else {
+        if constexpr (COLLECT == 1) NSPT_OZ_MMA2("1", ".collector::a::fill");
+        else if constexpr (COLLECT == 2) NSPT_OZ_MMA2("1", ".collector::a::use");
+        else if constexpr (COLLECT == 3) NSPT_OZ_MMA2("1", ".collector::a::lastuse");
+        else NSPT_OZ_MMA2("1", "");
+    }
+#undef NSPT_OZ_MMA2
+}
+// completion of all MMAs issued so far -> arrive on the barrier at the same offset in every CTA of the pair
+template <int CG>
+__device__ __forceinline__ void tc_commit_cg(uint32_t bar) {
+    if constexpr (CG == 2) {
+        asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+                     "h"((uint16_t)3)
+                     : "memory");
+    } else {
+        tc_commit(bar);
+    }
+}
+// TMA loads whose completion is reported to a barrier that may live in the peer CTA (the leader's)
+template <int CG>
+__device__ __forceinline__ void tma_load_4d_cg(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3) {
+    if constexpr (CG == 2) {
+        asm volatile(
+            "cp.async.bulk.tensor.4d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], "
+            "[%2];" ::"r"(dst),
+            "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+            : "memory");
+    } else {
+        tma_load_4d(dst, map, bar, c0, c1, c2, c3);
+    }
+}
+template <int CG>
+__device__ __forceinline__ void tma_load_5d_cg(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3,
+                                               int c4) {
+    if constexpr (CG == 2) {
+        asm volatile(
+            "cp.async.bulk.tensor.5d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, "
+            "%7}], [%2];" ::"r"(dst),
+            "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+            : "memory");
+    } else {
+        tma_load_5d(dst, map, bar, c0, c1, c2, c3, c4);
+    }
+}
+template <int CG>
+__device__ __forceinline__ void tc_alloc_cg(uint32_t smem_dst, uint32_t cols) {
+    if constexpr (CG == 2) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+        tc_alloc(smem_dst, cols);
+    }
+}
+template <int CG>
+__device__ __forceinline__ void tc_dealloc_cg(uint32_t taddr, uint32_t cols) {
+    if constexpr (CG == 2)
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+    else
+        tc_dealloc(taddr, cols);
+}
+
+// One lane of the MMA warp issues; everything the instruction consumes (descriptors, TMEM address) is computed by the WHOLE
+// warp from warp-uniform values so that the compiler keeps it in uniform registers -- inside a lane-0-only branch it falls
+// back to a R2UR "waterfall" loop of ~17 instructions per MMA, which costs more than the 32 cycles an MMA takes.
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "elect.sync _|p, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(pred));
+    return pred != 0;
+}
+template <int CG, int T0, int S0, bool FIRSTK>
+__device__ __forceinline__ void oz2_issue_pairs(uint32_t tmem, uint64_t dm0, uint64_t dn0, bool elected) {
+    constexpr int LAST = OZ_S - 1 - T0;
+    constexpr int COLLECT = (LAST == 0) ? 0 : (S0 == 0 ? 1 : (S0 == LAST ? 3 : 2));
+    // descriptors differ from the stage's first ones by a constant in the 14-bit start-address field (no carry: < 256 KB)
+    const uint64_t dm = dm0 + (uint64_t)((T0 * OZ_M_SLICE) >> 4);
+    const uint64_t dn = dn0 + (uint64_t)(((S0 >> 2) * Oz2<CG>::N_HALF + (S0 & 3) * 32) >> 4);
+    const uint32_t d = tmem + (uint32_t)((S0 + T0) * OZ2_BN);
+    if (elected) tc_mma_i8_cg<CG, COLLECT>(d, dm, dn, Oz2<CG>::IDESC, (!FIRSTK || T0 != 0) ? 1u : 0u);
+    if constexpr (S0 < LAST)
+        oz2_issue_pairs<CG, T0, S0 + 1, FIRSTK>(tmem, dm0, dn0, elected);
+    else if constexpr (T0 + 1 < OZ_S)
+        oz2_issue_pairs<CG, T0 + 1, 0, FIRSTK>(tmem, dm0, dn0, elected);
+}
+
+// exact conversion of the weighted sum of the seven accumulators of one output element:
+//   h = sum_d a_d 2^(-8 d) = hi 2^-24 + lo 2^-48,  hi = a0 2^24 + a1 2^16 + a2 2^8 + a3,  lo = a4 2^16 + a5 2^8 + a6
+// (|a_d| < 2^26, so |hi| < 2^51 and |lo| < 2^43: both convert exactly with the 2^52 + 2^51 trick); returns h * 2^24
+__device__ __forceinline__ long long mad_wide(int a, int b, long long c) {
+    long long r;
+    asm("mad.wide.s32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(c));
+    return r;
+}
+// multipliers 2^24, 2^16, 2^8, 1 in registers the optimizer cannot see through: with literal powers of two ptxas rewrites every
+// 64-bit multiply-add as shifts and carry chains (about 20 instructions per output element instead of 7 IMAD.WIDE)
+struct OzMul {
+    int m24, m16, m8, m1;
+};
+__device__ __forceinline__ OzMul oz_multipliers() {
+    OzMul m;
+    asm volatile("mov.b32 %0, 0x1000000;" : "=r"(m.m24));
+    asm volatile("mov.b32 %0, 0x10000;" : "=r"(m.m16));
+    asm volatile("mov.b32 %0, 0x100;" : "=r"(m.m8));
+    asm volatile("mov.b32 %0, 0x1;" : "=r"(m.m1));
+    return m;
+}
+__device__ __forceinline__ double oz2_combine(const OzMul& k, int a0, int a1, int a2, int a3, int a4, int a5, int a6) {
+    // the 2^52 + 2^51 bias rides along as the addend of the first multiply-add: the chains produce the bit patterns of
+    // 2^52 + 2^51 + hi and 2^52 + 2^51 + lo directly (one IMAD.WIDE per accumulator)
+    constexpr long long BIAS = 0x4338000000000000ll;
+    const long long hi = mad_wide(a0, k.m24, mad_wide(a1, k.m16, mad_wide(a2, k.m8, mad_wide(a3, k.m1, BIAS))));
+    const long long lo = mad_wide(a4, k.m16, mad_wide(a5, k.m8, mad_wide(a6, k.m1, BIAS)));
+    const double dhi = __longlong_as_double(hi) - 6755399441055744.0;
+    const double dlo = __longlong_as_double(lo) - 6755399441055744.0;
+    return fma(dlo, 5.9604644775390625e-08, dhi);   // 2^-24
+}
+
+struct Oz2Params {
+    double2* C;
+    const int* expA;
+    const int* expB;
+    unsigned long long* dbg;   // optional per-CTA clock samples (diagnostics), may be null
+    size_t NN;
+    int N;
+    int tiles_i, tiles_j;      // tiles per mode: rows in steps of 64, columns in steps of 128 * CG
+    int total_tiles;
+    int nkc;
+    int flags;                 // diagnostics: 1 = no MMAs, 2 = no accumulator drain / stores, 4 = no TMA loads
+};
+
+template <int CG>
+__global__ void __launch_bounds__(OZ2_THREADS, 1)
+zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_constant__ CUtensorMap mapN, const Oz2Params P) {
+    using K = Oz2<CG>;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_full = base + K::STAGES * K::STAGE;
+    const uint32_t bar_empty = bar_full + 8 * K::STAGES;
+    const uint32_t bar_acc_full = bar_empty + 8 * K::STAGES;
+    const uint32_t bar_acc_empty = bar_acc_full + 8;
+    const uint32_t tmem_slot = bar_acc_empty + 8;
+    volatile uint32_t* tmem_slot_gen = reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = CG == 2 ? cluster_rank() : 0u;
+    const int cluster_id = blockIdx.x / CG, nclusters = gridDim.x / CG;
+    const int nkc = P.nkc;
+    const int tiles_per_mode = P.tiles_i * P.tiles_j;
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < K::STAGES; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_empty + 8 * s, 1);
+        }
+        mbar_init(bar_acc_full, 1);
+        mbar_init(bar_acc_empty, 8 * CG);
+        mbar_fence_init();
+    }
+    if (warp == 2) tc_alloc_cg<CG>(tmem_slot, OZ_TMEM_COLS);
+    tc_fence_before();
+    if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot_gen;
+    pdl_wait();
+    pdl_trigger();
+    if (P.dbg && blockIdx.x == 0 && threadIdx.x == 0) {
+        unsigned long long gt;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+        P.dbg[200] = gt;
+        P.dbg[201] = clock64();
+    }
+    // barriers of the leader CTA, as shared::cluster addresses (identity for CG = 1)
+    const uint32_t lead_full = CG == 2 ? mapa_rank(bar_full, 0) : bar_full;
+    const uint32_t lead_acc_empty = CG == 2 ? mapa_rank(bar_acc_empty, 0) : bar_acc_empty;
+
+    if (warp < 4) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        if (warp == 0) {
+            // ------------------------------------------------------------ TMA producer (one thread per CTA)
+            if (lane == 0) {
+                int it = 0;
+                for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
+                    const int mode = tile / tiles_per_mode, rem = tile % tiles_per_mode;
+                    const int i0 = (rem / P.tiles_j) * OZ2_BN + (int)rank * K::N_ROWS;
+                    const int j0 = (rem % P.tiles_j) * (OZ_BM * CG) + (int)rank * OZ_BM;
+                    for (int plane = 0; plane < OZ_PLANES; ++plane) {
+                        const int pidx = mode * OZ_PLANES + plane;
+                        for (int kc = 0; kc < nkc; ++kc, ++it) {
+                            const int slot = it % K::STAGES;
+                            if (P.flags & 8) continue;
+                            mbar_wait_wd(bar_empty + 8 * slot, ((it / K::STAGES) & 1) ^ 1);
+                            if (P.flags & 4) {
+                                if (rank == 0) mbar_arrive(bar_full + 8 * slot);
+                                continue;
+                            }
+                            if (rank == 0) mbar_expect_tx(bar_full + 8 * slot, K::STAGE * CG);
+                            const uint32_t st = base + slot * K::STAGE;
+                            tma_load_4d_cg<CG>(st, &mapM, lead_full + 8 * slot, j0, kc * OZ_KC, 0, pidx);
+                            tma_load_5d_cg<CG>(st + OZ_M_STAGE, &mapN, lead_full + 8 * slot, 0, i0, 0, kc, pidx);
+                        }
+                    }
+                }
+            }
+        } else if (warp == 1) {
+            // ------------------------------------------------------------ MMA issuer (warp 1 of the leader CTA, one lane issues)
+            if (rank == 0) {
+                const bool elected = elect_one();
+                int it = 0, acc_it = 0;
+                for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
+                    for (int plane = 0; plane < OZ_PLANES; ++plane, ++acc_it) {
+                        if (P.dbg && blockIdx.x == 0 && acc_it < 8 && elected) P.dbg[acc_it * 16 + 0] = clock64();
+                        if (acc_it > 0) mbar_wait_wd(bar_acc_empty, (acc_it - 1) & 1);
+                        tc_fence_after();
+                        if (P.dbg && blockIdx.x == 0 && acc_it < 8 && elected) P.dbg[acc_it * 16 + 1] = clock64();
+                        for (int kc = 0; kc < nkc; ++kc, ++it) {
+                            const int slot = it % K::STAGES;
+                            if (!(P.flags & 8)) mbar_wait_wd(bar_full + 8 * slot, (it / K::STAGES) & 1);
+                            tc_fence_after();
+                            if (P.dbg && blockIdx.x == 0 && acc_it < 8 && elected && kc < 8) P.dbg[acc_it * 16 + 4 + kc] = clock64();
+                            const uint32_t sm = base + slot * K::STAGE;
+                            const uint64_t dm0 = oz_desc(sm, 4096, 1024), dn0 = oz_desc(sm + OZ_M_STAGE, 16, 1024);
+                            if (P.flags & 1) {
+                            } else if (kc == 0)
+                                oz2_issue_pairs<CG, 0, 0, true>(tmem, dm0, dn0, elected);
+                            else
+                                oz2_issue_pairs<CG, 0, 0, false>(tmem, dm0, dn0, elected);
+                            if (elected && !(P.flags & 8)) tc_commit_cg<CG>(bar_empty + 8 * slot);
+                            if (!(P.flags & 16)) __syncwarp();
+                        }
+                        if (elected) tc_commit_cg<CG>(bar_acc_full);
+                        __syncwarp();
+                        if (P.dbg && blockIdx.x == 0 && acc_it < 8 && elected) P.dbg[acc_it * 16 + 2] = clock64();
+                    }
+                }
+            }
+        }
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+        // ------------------------------------------------------------ epilogue: 8 warps; warp w reads TMEM lanes 32 (w % 4) ..
+        const int we = warp - 4, quarter = we & 3, half = we >> 2;
+        const OzMul mul = oz_multipliers();
+        int acc_it = 0;
+        for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
+            const int mode = tile / tiles_per_mode, rem = tile % tiles_per_mode;
+            const int row0 = (rem / P.tiles_j) * OZ2_BN + 32 * half;
+            const int col = (rem % P.tiles_j) * (OZ_BM * CG) + (int)rank * OZ_BM + 32 * quarter + lane;
+            double re[32], im[32];
+#pragma unroll
+            for (int plane = 0; plane < OZ_PLANES; ++plane, ++acc_it) {
+                mbar_wait_wd(bar_acc_full, acc_it & 1);
+                tc_fence_after();
+                if (P.dbg && blockIdx.x == 0 && acc_it < 8 && threadIdx.x == 128) P.dbg[acc_it * 16 + 12] = clock64();
+                if (!(P.flags & 2)) {
+                    // eight chunks of four columns; the loads of the next chunk are in flight while one is combined
+                    const uint32_t tbase = tmem + ((uint32_t)(32 * quarter) << 16) + (uint32_t)(32 * half);
+                    int a[2][OZ_S][4];
+#pragma unroll
+                    for (int d = 0; d < OZ_S; ++d) tc_ld4(tbase + (uint32_t)(d * OZ2_BN), a[0][d]);
+#pragma unroll
+                    for (int cc = 0; cc < 8; ++cc) {
+                        tc_wait_ld();
+                        if (cc + 1 < 8) {
+#pragma unroll
+                            for (int d = 0; d < OZ_S; ++d) tc_ld4(tbase + (uint32_t)(d * OZ2_BN + 4 * (cc + 1)), a[(cc + 1) & 1][d]);
+                        }
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const int (&b)[OZ_S][4] = a[cc & 1];
+                            const double h = oz2_combine(mul, b[0][j], b[1][j], b[2][j], b[3][j], b[4][j], b[5][j], b[6][j]);
+                            // 3M: Cr = P1 - P2, Ci = 4 P3 - P1 - P2 (the sum planes carry one more exponent bit each)
+                            if (plane == 0) {
+                                re[4 * cc + j] = h;
+                                im[4 * cc + j] = -h;
+                            } else if (plane == 1) {
+                                re[4 * cc + j] -= h;
+                                im[4 * cc + j] -= h;
+                            } else {
+                                im[4 * cc + j] = fma(4.0, h, im[4 * cc + j]);
+                            }
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    if (CG == 2) mbar_arrive_cluster(lead_acc_empty); else mbar_arrive(bar_acc_empty);
+                }
+                if (P.dbg && blockIdx.x == 0 && acc_it < 8 && threadIdx.x == 128) P.dbg[acc_it * 16 + 13] = clock64();
+            }
+            const int esum = P.expA[mode] + P.expB[mode];
+            const double sc = esum >= (1 << 20) ? __longlong_as_double(0x7ff8000000000000ll) : oz_pow2(esum - 12 - 24);
+            if (col < P.N && !(P.flags & 2)) {
+                double2* c = P.C + (size_t)mode * P.NN + col;
+#pragma unroll
+                for (int j = 0; j < 32; ++j)   // the 32 lanes of a warp write 512 contiguous bytes of row row0 + j
+                    if (row0 + j < P.N) c[(size_t)(row0 + j) * P.N] = make_double2(sc * re[j], sc * im[j]);
+            }
+        }
+    }
+    __syncwarp();
+    tc_fence_before();
+    if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+    if (P.dbg && blockIdx.x == 0 && threadIdx.x == 0) {
+        unsigned long long gt;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+        P.dbg[202] = gt;
+        P.dbg[203] = clock64();
+    }
+    if (warp == 2) tc_dealloc_cg<CG>(tmem, OZ_TMEM_COLS);
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -390,10 +882,6 @@ struct OzWs {
     unsigned long long* maxbits;   // [2][modes]
     int* exps;                     // [2][modes]
 };
-int oz_pitch_rows(int N) { return (N + 127) / 128 * 128; }   // rows start on 128-byte boundaries: a 128-byte box row is one line
-int oz_pitch_quad(int N) { return (N + 31) / 32 * 256; }     // 8 slots x 32 bytes per chunk of 32 columns
-size_t oz_bytes_quad(int N, size_t modes) { return (modes * OZ_PLANES * (size_t)N * oz_pitch_quad(N) + 255) / 256 * 256; }
-size_t oz_bytes_rows(int N, size_t modes) { return (modes * OZ_PLANES * OZ_S * (size_t)N * oz_pitch_rows(N) + 255) / 256 * 256; }
 OzWs oz_carve(const FreqLayout& f, int batch, void* ws) {
     const size_t modes = (size_t)batch * f.L;
     OzWs w;
@@ -405,6 +893,19 @@ OzWs oz_carve(const FreqLayout& f, int batch, void* ws) {
 }
 
 }  // namespace
+
+void ozaki_slice_targets(const FreqLayout& f, int batch, void* ws, OzSliceDst* a, OzSliceDst* b) {
+    const int modes = batch * f.L;
+    const OzWs w = oz_carve(f, batch, ws);
+    a->slices = w.sA;
+    a->layout = OZ_QUAD;
+    a->maxbits = w.maxbits;
+    a->exps = w.exps;
+    b->slices = w.sB;
+    b->layout = OZ_ROWS;
+    b->maxbits = w.maxbits + modes;
+    b->exps = w.exps + modes;
+}
 
 size_t ozaki_workspace_bytes(const FreqLayout& f, int batch) {
     const size_t modes = (size_t)batch * f.L;
@@ -430,11 +931,145 @@ cudaError_t launch_ozaki_slice(const FreqLayout& f, int batch, const double* A, 
     return cudaGetLastError();
 }
 
-// C~(p) = A~(p) B~(p) for all batch * L modes from the slices in `ws`
-cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st) {
+// FP64 spectra A~, B~ -> int8 slices, with the per-mode maxima already in the workspace (written by the forward transform)
+cudaError_t launch_ozaki_slice2(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st) {
+    const int modes = batch * f.L;
+    const int N = f.N;
+    const OzWs w = oz_carve(f, batch, ws);
+    Slice2Params P;
+    P.X[0] = reinterpret_cast<const double2*>(A);
+    P.X[1] = reinterpret_cast<const double2*>(B);
+    P.out[0] = w.sA;
+    P.out[1] = w.sB;
+    P.maxbits[0] = w.maxbits;
+    P.maxbits[1] = w.maxbits + modes;
+    P.exps[0] = w.exps;
+    P.exps[1] = w.exps + modes;
+    P.pitch[0] = oz_pitch_quad(N);
+    P.pitch[1] = oz_pitch_rows(N);
+    P.N = N;
+    P.modes = modes;
+    const int groups = N * (P.pitch[0] >> 5);   // the QUAD operand has the most 4-column groups per mode
+    cudaLaunchConfig_t cfg = {};
+    const int my = (modes + OZ_SLICE_MODES - 1) / OZ_SLICE_MODES;
+    cfg.gridDim = dim3((unsigned)((groups + 255) / 256), (unsigned)(my < 65535 ? my : 65535), 2);
+    cfg.blockDim = dim3(256, 1, 1);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, oz_slice2_kernel, P);
+}
+
+// launch with programmatic stream serialization and (CG = 2) clusters of two CTAs
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl_cluster(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, unsigned cluster,
+                               cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[2];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = cluster;
+    attr[1].val.clusterDim.y = 1;
+    attr[1].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = cluster > 1 ? 2 : 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
+void oz_maps(const FreqLayout& f, int modes, const OzWs& w, int n_rows, CUtensorMap* mapM, CUtensorMap* mapN, cudaError_t* err) {
+    const int N = f.N;
+    const int pq = oz_pitch_quad(N), pr = oz_pitch_rows(N), nkc = (N + OZ_KC - 1) / OZ_KC;
+    {   // B~ slices, ROWS layout: (col j, row k, slice, mode * plane); box = [7 slices][32 k][128 bytes of j]
+        const cuuint64_t dims[4] = {(cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)OZ_S, (cuuint64_t)modes * OZ_PLANES};
+        const cuuint64_t strides[3] = {(cuuint64_t)pr, (cuuint64_t)N * pr, (cuuint64_t)OZ_S * N * pr};
+        const cuuint32_t box[4] = {(cuuint32_t)OZ_BM, (cuuint32_t)OZ_KC, (cuuint32_t)OZ_S, 1};
+        if ((*err = encode_u8(mapM, w.sB, 4, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) != cudaSuccess) return;
+    }
+    {   // A~ slices, QUAD layout: (128 bytes = 4 slots, row i, half, k-chunk, mode * plane); box = [2 halves][rows][128 bytes]
+        const cuuint64_t dims[5] = {128, (cuuint64_t)N, 2, (cuuint64_t)nkc, (cuuint64_t)modes * OZ_PLANES};
+        const cuuint64_t strides[4] = {(cuuint64_t)pq, 128, 256, (cuuint64_t)N * pq};
+        const cuuint32_t box[5] = {128, (cuuint32_t)n_rows, 2, 1, 1};
+        *err = encode_u8(mapN, w.sA, 5, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+    }
+}
+
+template <int CG>
+cudaError_t launch_oz2(const FreqLayout& f, int modes, const OzWs& w, double* C, unsigned long long* dbg, cudaStream_t st) {
+    using K = Oz2<CG>;
+    const int N = f.N;
+    cudaError_t e;
+    static bool attr_done[NSPT_MAX_DEVICES] = {};
+    const int dev = current_device();
+    if (!attr_done[dev]) {
+        e = cudaFuncSetAttribute(zgemm_modes_i8_kernel<CG>, cudaFuncAttributeMaxDynamicSharedMemorySize, K::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_done[dev] = true;
+    }
+    CUtensorMap mapM, mapN;
+    oz_maps(f, modes, w, K::N_ROWS, &mapM, &mapN, &e);
+    if (e != cudaSuccess) return e;
+    Oz2Params P;
+    P.C = reinterpret_cast<double2*>(C);
+    P.expA = w.exps;
+    P.expB = w.exps + modes;
+    P.dbg = dbg;
+    P.NN = f.NN;
+    P.N = N;
+    P.tiles_i = (N + OZ2_BN - 1) / OZ2_BN;
+    P.tiles_j = (N + OZ_BM * CG - 1) / (OZ_BM * CG);
+    P.total_tiles = modes * P.tiles_i * P.tiles_j;
+    P.nkc = (N + OZ_KC - 1) / OZ_KC;
+    {
+        const char* fl = getenv("NSPT_OZ_DBG");
+        P.flags = fl ? atoi(fl) : 0;
+    }
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    int clusters = sms / CG;
+    if (clusters > P.total_tiles) clusters = P.total_tiles;
+    return launch_pdl_cluster(zgemm_modes_i8_kernel<CG>, (unsigned)(clusters * CG), OZ2_THREADS, K::SMEM, CG, st, mapM, mapN, P);
+}
+
+// C~(p) = A~(p) B~(p) for all batch * L modes from the slices in `ws`.  kernel: 0 = first-generation kernel (one tile per CTA),
+// 1 = persistent single-CTA tiles, 2 = persistent CTA pairs (cta_group::2), -1 = automatic (pairs when N > 128).
+cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st, int kernel) {
     const int modes = batch * f.L;
     const int N = f.N;
     const OzWs w = oz_carve(f, batch, const_cast<void*>(ws));
+    if (kernel < 0) kernel = N > 128 ? 2 : 1;
+    if (kernel == 1 || kernel == 2) {
+        static unsigned long long* dbg = nullptr;
+        const bool trace = getenv("NSPT_OZ_TRACE") != nullptr;
+        if (trace && !dbg) {
+            cudaMalloc(&dbg, 256 * 8);
+        }
+        if (trace) cudaMemsetAsync(dbg, 0, 256 * 8, st);
+        cudaError_t e = kernel == 2 ? launch_oz2<2>(f, modes, w, C, trace ? dbg : nullptr, st)
+                                    : launch_oz2<1>(f, modes, w, C, trace ? dbg : nullptr, st);
+        if (trace && e == cudaSuccess) {
+            unsigned long long h[256];
+            cudaStreamSynchronize(st);
+            cudaMemcpy(h, dbg, sizeof(h), cudaMemcpyDeviceToHost);
+            const unsigned long long t0 = h[0];
+            printf("CTA 0: %lld cycles in %lld ns = %.0f MHz\n", (long long)(h[203] - h[201]), (long long)(h[202] - h[200]),
+                   1e3 * (double)(h[203] - h[201]) / (double)(h[202] - h[200]));
+            for (int a = 0; a < 7; ++a) {
+                printf("acc_it %d: mma[wait_begin %lld wait_end %lld issued %lld] stages:", a, (long long)(h[a * 16] - t0),
+                       (long long)(h[a * 16 + 1] - t0), (long long)(h[a * 16 + 2] - t0));
+                for (int k = 0; k < 8; ++k) printf(" %lld", (long long)(h[a * 16 + 4 + k] - t0));
+                printf(" | epi[full_seen %lld drained %lld]\n", (long long)(h[a * 16 + 12] - t0), (long long)(h[a * 16 + 13] - t0));
+            }
+        }
+        return e;
+    }
     cudaError_t e;
     static bool attr_done[NSPT_MAX_DEVICES] = {};
     const int dev = current_device();
@@ -443,20 +1078,9 @@ cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, do
         if (e != cudaSuccess) return e;
         attr_done[dev] = true;
     }
-    const int pq = oz_pitch_quad(N), pr = oz_pitch_rows(N), nkc = (N + OZ_KC - 1) / OZ_KC;
     CUtensorMap mapM, mapN;
-    {   // B~ slices, ROWS layout: (col j, row k, slice, mode * plane); box = [7 slices][32 k][128 bytes of j]
-        const cuuint64_t dims[4] = {(cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)OZ_S, (cuuint64_t)modes * OZ_PLANES};
-        const cuuint64_t strides[3] = {(cuuint64_t)pr, (cuuint64_t)N * pr, (cuuint64_t)OZ_S * N * pr};
-        const cuuint32_t box[4] = {(cuuint32_t)OZ_BM, (cuuint32_t)OZ_KC, (cuuint32_t)OZ_S, 1};
-        if ((e = encode_u8(&mapM, w.sB, 4, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) != cudaSuccess) return e;
-    }
-    {   // A~ slices, QUAD layout: (128 bytes = 4 slots, row i, half, k-chunk, mode * plane); box = [2 halves][64 i][128 bytes]
-        const cuuint64_t dims[5] = {128, (cuuint64_t)N, 2, (cuuint64_t)nkc, (cuuint64_t)modes * OZ_PLANES};
-        const cuuint64_t strides[4] = {(cuuint64_t)pq, 128, 256, (cuuint64_t)N * pq};
-        const cuuint32_t box[5] = {128, (cuuint32_t)OZ_BN, 2, 1, 1};
-        if ((e = encode_u8(&mapN, w.sA, 5, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) != cudaSuccess) return e;
-    }
+    oz_maps(f, modes, w, OZ_BN, &mapM, &mapN, &e);
+    if (e != cudaSuccess) return e;
     OzParams P;
     P.C = reinterpret_cast<double2*>(C);
     P.expA = w.exps;
@@ -465,7 +1089,7 @@ cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, do
     P.N = N;
     P.tiles_i = (N + OZ_BN - 1) / OZ_BN;
     P.tiles_j = (N + OZ_BM - 1) / OZ_BM;
-    P.nkc = nkc;
+    P.nkc = (N + OZ_KC - 1) / OZ_KC;
     const unsigned grid = (unsigned)(modes * P.tiles_i * P.tiles_j);
     return launch_pdl(zgemm_modes_ozaki_kernel, grid, OZ_THREADS, OZ_SMEM, st, mapM, mapN, P);
 }
