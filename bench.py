@@ -300,7 +300,7 @@ def run_sweep(args):
     stream = torch.cuda.Stream(device=dev)
     nspt.nspt_set_stream(stream.cuda_stream)
     nspt.nspt_set_order_scale(1.0)
-    nspt.nspt_set_gemm_variant(1)
+    nspt.nspt_set_gemm_variant(args.gemm_variant)
     fp64_peak = nspt.nspt_probe_fp64_peak()
     peaks = {}
     pfile = ROOT / "MEASURED_PEAKS.json"
@@ -342,13 +342,15 @@ def run_sweep(args):
                 nspt.nspt_profile_read(name)
             for i in range(K):
                 nspt.nspt_series_mul(*sets[i % R])
-            st = {name: nspt.nspt_profile_read(name) for name in ("fft_forward", "zgemm_modes", "fft_inverse")}
+            st = {name: nspt.nspt_profile_read(name) for name in ("fft_forward", "zgemm_modes", "fft_inverse", "int8_slicing")}
             nspt.nspt_profile(False)
         t_gemm = 8.0 * N ** 3 * L / (fp64_peak * 1e12)
         t_fft = 9.0 * n * N * N * 16 / (hbm * 1e9)
         row = {"N": N, "N_trunc": Ntrunc, "L": L, "us_per_product": us, "products_per_s": 1e6 / us,
                "fft_forward_us": st["fft_forward"][0] / K * 1e3, "zgemm_modes_us": st["zgemm_modes"][0] / K * 1e3,
                "fft_inverse_us": st["fft_inverse"][0] / K * 1e3,
+               "int8_slicing_us": st["int8_slicing"][0] / K * 1e3,
+               "mode_wise_product": "int8 tensor cores" if st["int8_slicing"][1] else "fp64 tensor pipe",
                "fftconv_roofline_us": max(t_gemm, t_fft) * 1e6, "bound": "fp64" if t_gemm >= t_fft else "hbm",
                "fftconv_roofline_frac": max(t_gemm, t_fft) * 1e6 / us, "buffer_sets": R}
         if not args.no_cpu_baseline:
@@ -574,7 +576,32 @@ def run_cuda(args):
         t_gemm_roof = flops_per_launch / (fp64_peak * 1e12)
         t_fft_roof = 9.0 * n * N * N * 16 * batch / (hbm * 1e9)
         roof_time = max(t_gemm_roof, t_fft_roof)
-        line_extra["roofline"] = {
+        int8_path = "int8_slicing" in stage_ms      # the library chose (or was told to use) the INT8 tensor-core product
+        if int8_path and gemm:
+            # the dominant kernel is a contraction in INT8: 28 slice pairs x 3 planes of N^3 multiply-adds per mode, against
+            # the INT8 peak = measured dense bf16 peak x the nominal ratio 2 (B200_PROFILING.md); beside it the FP64 work it stands for
+            int8_ops = 84 * 2.0 * N ** 3 * L * batch
+            bf16 = peaks.get("bf16_tflops", 1630.0)
+            int8_peak = 2.0 * bf16
+            ach_i8 = int8_ops * K / (gemm["ms_total"] * 1e-3) * 1e-12
+            traffic = read_traffic(args.workload, "zgemm_modes_i8")
+            line_extra["roofline"] = {
+                "bound": "tensor", "kernel": "zgemm_modes_i8_kernel (tcgen05.mma.kind::i8, TMEM accumulators; FP64 product emulated with 7 int8 slices per plane)",
+                "achieved": ach_i8, "peak": int8_peak, "unit": "TOP/s", "frac": ach_i8 / int8_peak, "traffic": traffic,
+                "flops_basis": "84 INT8 matrix products (28 slice pairs x 3 planes of the 3M complex product) of 2*N^3 ops per mode; tiles are padded to 128 x 64 x 32, the executed count is higher",
+                "peak_source": ("MEASURED_PEAKS.json bf16_tflops (burst) x 2 (nominal INT8 : bf16 ratio, B200_PROFILING.md)" if "bf16_tflops" in peaks
+                                else "fallback 1630 TFLOP/s bf16 x 2"),
+                "fp64_equivalent": {"achieved": achieved, "unit": "TFLOP/s", "basis": "conventional 8*N^3*L", "fp64_tensor_peak": fp64_peak,
+                                    "ratio_to_fp64_tensor_peak": (achieved / fp64_peak) if achieved else None},
+                "hbm_peak_GB_s": hbm, "hbm_peak_source": hbm_src,
+            }
+            fft_step_bytes["int8_slicing"] = 2 * (16 + 21) * L * N * N * batch   # per operand: read L*e, write 21 bytes per element
+            if "int8_slicing" in stages_out and stage_ms["int8_slicing"]["ms_total"] > 0:
+                gbs = fft_step_bytes["int8_slicing"] * K / (stage_ms["int8_slicing"]["ms_total"] * 1e-3) * 1e-9
+                stages_out["int8_slicing"].update({"algorithmic_bytes_per_step": fft_step_bytes["int8_slicing"], "algorithmic_GB_s": gbs,
+                                                   "frac_of_hbm_peak": gbs / hbm})
+        else:
+          line_extra["roofline"] = {
             "bound": "tensor", "kernel": "zgemm_modes_dmma_kernel (FP64 tensor pipe, DMMA.8x8x4)",
             "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
             "frac": (achieved / fp64_peak) if achieved else None, "traffic": traffic,
@@ -583,7 +610,7 @@ def run_cuda(args):
             "frac_executed": (achieved * 0.75 / fp64_peak) if achieved else None,
             "peak_source": "nspt_probe_fp64_peak: DMMA m8n8k4 chain, measured in this run (MEASURED_PEAKS.json has no FP64 entry)",
             "hbm_peak_GB_s": hbm, "hbm_peak_source": hbm_src,
-        }
+          }
         if kind == "exp":
             step_s = ms_local / K * 1e-3
             line_extra["exp_roofline"] = {
@@ -598,6 +625,8 @@ def run_cuda(args):
                 "definition": "slower of 8*N^3*L flops at FP64 peak and 9*n*16*N^2 bytes at HBM peak (SURVEY.md 8d)",
                 "roofline_products_per_s": batch / roof_time, "t_gemm_us": t_gemm_roof * 1e6, "t_fft_us": t_fft_roof * 1e6,
                 "frac": roof_time / step_s if step_s else None,
+                "mode_wise_product": ("INT8 tensor cores (FP64 emulated by exact integer slices): the FP64-peak bound above does not bind this path"
+                                      if int8_path else "FP64 tensor pipe"),
                 # the kernel executes the 3-multiplication product (6*N^3*L), for which 8*N^3*L / peak is NOT a lower bound:
                 # the same fraction against the bound of the arithmetic actually executed, transforms not overlapped
                 "frac_vs_3m_bound": (0.75 * t_gemm_roof + t_fft_roof) / step_s if step_s else None,
@@ -744,8 +773,9 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--gemm-variant", type=int, default=1, choices=[1, 2, 3],
-                    help="mode-wise product kernel: 1 = FP64 tensor pipe (DMMA, default), 2 = INT8 tensor cores (tcgen05, Ozaki slicing)")
+    ap.add_argument("--gemm-variant", type=int, default=-1, choices=[-1, 1, 2, 3, 4],
+                    help="mode-wise product kernel (include/nspt_debug.h): -1 = the library's automatic choice (default), 1 = FP64 tensor pipe "
+                         "(DMMA), 2 = INT8 tensor cores (tcgen05, Ozaki slicing), 3 = persistent DMMA, 4 = INT8 on CTA pairs")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
         return spawn_replicas(args.gpus, sys.argv[1:])

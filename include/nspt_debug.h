@@ -14,12 +14,18 @@ extern "C" {
 #endif
 
 /* Select the kernel of the mode-wise matrix product (Step 3):
+ *  -1 = automatic (default): nspt_series_mul[_batched] uses the INT8 tensor-core path where it is measured faster and its error
+ *       stays far below the tolerance (N >= 192, 32 <= L <= 128), the FP64 tensor-pipe kernel elsewhere,
  *   0 = reference kernel (one thread per output element, plain double FMAs; cross-check only),
- *   1 = FP64 tensor-pipe kernel (DMMA, TMA-fed, 3-multiplication complex product; default),
- *   2 = INT8 tensor-core kernel (tcgen05.mma.kind::i8, TMEM accumulators; FP64 emulated with seven int8 slices per
- *       operand plane, exact INT32 sums).  Used by nspt_series_mul[_batched] only; products with
- *       scaling / accumulating epilogues (staple, exponential) stay on kernel 1.  Needs extra workspace
- *       (nspt_workspace_bytes reports it for the variant that is selected when it is called). */
+ *   1 = FP64 tensor-pipe kernel (DMMA, TMA-fed, 3-multiplication complex product) everywhere,
+ *   2 = INT8 tensor-core path wherever it exists (L >= 16): the forward transform records the largest element of every
+ *       mode, one pass cuts both spectra into seven int8 slices per plane (fixed point relative to that maximum), a
+ *       persistent tcgen05.mma.kind::i8 kernel forms the exact INT32 sums in TMEM and recombines them in FP64
+ *       (SURVEY.md 8f NEXT-3).  nspt_series_mul[_batched] only; products with scaling / accumulating epilogues (staple,
+ *       exponential) stay on kernel 1.  Needs extra workspace (nspt_workspace_bytes reports it for the variant that is
+ *       selected when it is called),
+ *   3 = persistent warp-specialised FP64 tensor-pipe kernel (measured slower than 1; kept as a cross-check),
+ *   4 = as 2 with every tile on a CTA pair (tcgen05.mma.cta_group::2, M = 256). */
 int nspt_set_gemm_variant(int variant);
 
 /* Select the convolution algorithm of nspt_series_mul[_batched]: 0 = automatic (default), 1 = FFT-CONV,
@@ -32,7 +38,7 @@ int nspt_set_conv_algorithm(int algorithm);
  * bracketed by CUDA events on the library stream; nspt_profile_read synchronises the stream,
  * and for stage = 0 forward transforms, 1 mode-wise matrix products, 2 inverse transforms,
  * 3 re-truncation transforms, 4 other (dagger, force, scaling), 5 block polynomials of the series
- * exponential, 6 int8 slicing passes of kernel 2 returns the summed milliseconds and the number of
+ * exponential, 6 int8 slicing passes of the INT8 path returns the summed milliseconds and the number of
  * launches since the last read, then resets the counters. */
 int nspt_profile(int enable);
 int nspt_profile_read(int stage, double* ms, long long* launches);

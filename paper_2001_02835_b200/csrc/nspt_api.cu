@@ -8,7 +8,6 @@
 #include <vector>
 
 #include "nspt_internal.cuh"
-#include "nspt_ozaki.cuh"
 
 namespace nspt {
 namespace {
@@ -33,7 +32,7 @@ struct Context {
     cudaEvent_t order_event = nullptr;   // orders a newly set stream after the work of the previous one
     bool used = false;                   // a kernel has been enqueued since the library was loaded / released
     double order_scale = 1.0;
-    int gemm_variant = 1;
+    int gemm_variant = -1;               // nspt_debug.h: -1 = automatic
     int conv_algorithm = 0;              // 0 = automatic, 1 = FFT-CONV, 2 = Naive-CONV (nspt_debug.h)
     bool arch_checked = false;
     // workspace
@@ -189,8 +188,20 @@ void exp_split(int Ntrunc, int* s, int* r) {
 // last 128-byte chunk of a row runs into what follows, nspt_zgemm.cu), so every workspace ends with a 256-byte pad.
 constexpr size_t WS_PAD = 256;
 
+// Mode-wise product of nspt_series_mul[_batched] on the INT8 tensor cores (nspt_ozaki.cu) or on the FP64 tensor pipe
+// (nspt_zgemm.cu).  Automatic choice, measured on one B200: the INT8 path pays a slicing pass of O(N^2 L) bytes
+// for a product kernel that is about twice as fast, so it wins from N = 192 up; it is limited to L <= 128 (N_trunc <= 63),
+// where its error stays two orders of magnitude below the 1e-11 tolerance on series shaped like the paper's (at N_trunc = 127
+// the margin shrinks to a factor of five: that range stays on the FP64 pipe unless the variant is forced).
+bool use_int8(const FreqLayout& f) {
+    if (f.L < 16) return false;   // the slicing pass takes its maxima from the TMA transform kernels
+    if (g.gemm_variant == 2 || g.gemm_variant == 4) return true;
+    if (g.gemm_variant != -1) return false;
+    return f.N >= 192 && f.L >= 32 && f.L <= 128;
+}
+
 size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
-    if (op == NSPT_OP_SERIES_MUL && (g.gemm_variant == 2 || g.gemm_variant >= 4)) return 3 * spectrum_bytes(f, batch) + WS_PAD + ozaki_workspace_bytes(f, batch);
+    if (op == NSPT_OP_SERIES_MUL && use_int8(f)) return 3 * spectrum_bytes(f, batch) + WS_PAD + ozaki_workspace_bytes(f, batch);
     if (op == NSPT_OP_STAPLE) return 30 * spectrum_bytes(f, 1) + WS_PAD;
     if (op == NSPT_OP_SERIES_EXP) {
         int s, r;
@@ -314,16 +325,19 @@ int k_dagger(const FreqLayout& f, int batch, const double* src, double* dst) {
     NSPT_CUDA(launch_freq_dagger(f, batch, src, dst, g.stream));
     return tm.end();
 }
+// kernel of nspt_zgemm.cu behind the staple, the exponential and the FP64 products: 0 = debug, 1 = block-scheduled, 3 = persistent
+int dmma_variant() { return (g.gemm_variant == 0 || g.gemm_variant == 3) ? g.gemm_variant : 1; }
+
 int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, const GemmOut& out) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_GEMM));
-    NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, out, (g.gemm_variant == 2 || g.gemm_variant >= 4) ? 1 : g.gemm_variant, g.stream));
+    NSPT_CUDA(launch_zgemm_modes(f, batch, A, B, out, dmma_variant(), g.stream));
     return tm.end();
 }
 int k_gemm_groups(const FreqLayout& f, const GemmGroup* groups, int ngroups, int batch = 1) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_GEMM));
-    NSPT_CUDA(launch_zgemm_groups(f, batch, groups, ngroups, (g.gemm_variant == 2 || g.gemm_variant >= 4) ? 1 : g.gemm_variant, g.stream));
+    NSPT_CUDA(launch_zgemm_groups(f, batch, groups, ngroups, dmma_variant(), g.stream));
     return tm.end();
 }
 int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, double* C) {
@@ -338,7 +352,7 @@ int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, dou
 // launch- or transform-bound (see DESIGN.md 5.5 for the measured crossover).  It reads A and B while it writes C, so an
 // output that aliases an input always takes FFT-CONV.
 bool use_naive_conv(const FreqLayout& f, const nspt_c128* A, const nspt_c128* B, const nspt_c128* C) {
-    if (C == A || C == B || (g.gemm_variant != 1 && g.gemm_variant != 3)) return false;
+    if (C == A || C == B || g.gemm_variant == 0 || g.gemm_variant == 2 || g.gemm_variant == 4) return false;
     if (g.conv_algorithm == 1) return false;
     if (g.conv_algorithm == 2) return true;
     // measured crossover (one B200, time per product through the binding): the direct form is one launch
@@ -371,67 +385,34 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
     double* At = reinterpret_cast<double*>(ws);
     double* Bt = reinterpret_cast<double*>(ws + sb);
     double* Ct = reinterpret_cast<double*>(ws + 2 * sb);
-    // gemm variants: 1 = FP64 tensor pipe; 2 = INT8 tensor cores (forward transform tracks the per-mode maxima, slicing pass,
-    // persistent tcgen05 kernel); diagnostics: 4 = first-generation INT8 path, 5 = forward transform writes the slices itself,
-    // 6 = variant 2 with CTA pairs (cta_group::2)
-    const int gv = g.gemm_variant;
-    const bool int8 = gv == 2 || gv >= 4;
-    if (gv == 5 && fft_slices_supported(f.L)) {
+    if (use_int8(f)) {
         void* oz = ws + 3 * sb + WS_PAD;
-        OzSliceDst da, db;
-        ozaki_slice_targets(f, batch, oz, &da, &db);
-        {
-            StageTimer tm;
-            NSPT_TRY(tm.begin(ST_FWD));
-            NSPT_CUDA(launch_fft_forward_slices(f, t, batch, A, da, B, db, g.stream));
-            NSPT_TRY(tm.end());
-        }
-        StageTimer tm;
-        NSPT_TRY(tm.begin(ST_GEMM));
-        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream, 1));
-        NSPT_TRY(tm.end());
-    } else if (int8 && gv != 4 && f.L >= 16) {
-        void* oz = ws + 3 * sb + WS_PAD;
-        OzSliceDst da, db;
-        ozaki_slice_targets(f, batch, oz, &da, &db);
+        unsigned long long* mbA = ozaki_maxbits(f, batch, oz, 0);
         {
             // Steps 1-2 (eqs. 2.6-2.7); the transform also records max(|re|, |im|) of every mode of both spectra
             StageTimer tm;
             NSPT_TRY(tm.begin(ST_FWD));
-            NSPT_CUDA(cudaMemsetAsync(da.maxbits, 0, sizeof(unsigned long long) * 2 * batch * f.L, g.stream));
-            NSPT_CUDA(launch_fft_forward(f, t, batch, A, At, B, Bt, g.stream, false, da.maxbits, db.maxbits));
+            NSPT_CUDA(cudaMemsetAsync(mbA, 0, sizeof(unsigned long long) * 2 * batch * f.L, g.stream));
+            NSPT_CUDA(launch_fft_forward(f, t, batch, A, At, B, Bt, g.stream, false, mbA, ozaki_maxbits(f, batch, oz, 1)));
             NSPT_TRY(tm.end());
         }
         {
-            StageTimer tm;
-            NSPT_TRY(tm.begin(ST_SLICE));
-            NSPT_CUDA(launch_ozaki_slice2(f, batch, At, Bt, oz, g.stream));
-            NSPT_TRY(tm.end());
-        }
-        // Step 3 (eq. 2.8) on the INT8 tensor cores
-        StageTimer tm;
-        NSPT_TRY(tm.begin(ST_GEMM));
-        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream, gv == 6 ? 2 : 1));
-        NSPT_TRY(tm.end());
-    } else {
-    // Steps 1-2 (eqs. 2.6-2.7): zero-padded forward transforms of A and B, one launch
-    NSPT_TRY(k_forward(f, t, batch, A, At, B, Bt));
-    // Step 3 (eq. 2.8): mode-wise matrix products
-    if (int8) {
-        void* oz = ws + 3 * sb + WS_PAD;
-        {
+            // both spectra cut into seven int8 slices per plane, fixed point relative to the largest element of each mode
             StageTimer tm;
             NSPT_TRY(tm.begin(ST_SLICE));
             NSPT_CUDA(launch_ozaki_slice(f, batch, At, Bt, oz, g.stream));
             NSPT_TRY(tm.end());
         }
+        // Step 3 (eq. 2.8): exact integer products on the INT8 tensor cores, recombined in FP64
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_GEMM));
-        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream, 0));
+        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream, g.gemm_variant == 4));
         NSPT_TRY(tm.end());
     } else {
+        // Steps 1-2 (eqs. 2.6-2.7): zero-padded forward transforms of A and B, one launch
+        NSPT_TRY(k_forward(f, t, batch, A, At, B, Bt));
+        // Step 3 (eq. 2.8): mode-wise matrix products on the FP64 tensor pipe
         NSPT_TRY(k_gemm(f, batch, At, Bt, Ct));
-    }
     }
     // Steps 4-5 (eq. 2.9): inverse transform, 1/L, truncation
     NSPT_TRY(k_inverse(f, t, batch, Ct, C));
@@ -815,7 +796,7 @@ int nspt_set_workspace(void* dptr, size_t bytes) {
 
 int nspt_set_gemm_variant(int variant) {
     NSPT_LOCK();
-    if (variant < 0 || variant > 6) return NSPT_EINVAL;
+    if (variant < -1 || variant > 4) return NSPT_EINVAL;
     g.gemm_variant = variant;
     return NSPT_OK;
 }

@@ -29,7 +29,6 @@
 // beyond N^2 are zero-filled by TMA, which is exactly the zero padding of Step 1.  Results leave
 // with coalesced 16-byte stores (fire and forget).  L <= 8 needs one thread per element and no
 // shared memory; those kernels use plain loads.
-#include <cstdlib>
 #include <map>
 #include <mutex>
 
@@ -506,223 +505,6 @@ __global__ void __launch_bounds__(T* S, 1) fft_forward_tma_kernel(const __grid_c
     if (threadIdx.x == 0) tma_store_wait_read<0>();
 }
 
-// =================================================================================================
-// Forward transform that writes the int8 slices of the spectrum for the INT8 tensor-core product (nspt_ozaki.cu) instead
-// of the FP64 spectrum.  Tiles are aligned to matrix rows -- T consecutive columns of one row -- so that every (mode,
-// plane, slice) of a tile is one aligned run of T bytes in either slice layout; columns beyond N are zero-filled by TMA and
-// give zero digits (the explicit k padding of the QUAD layout).  The slices are fixed point relative to a power of two above
-// the largest element of the MODE, which is only known once every element has been transformed: the MAXONLY instance of
-// the same kernel runs first, transforms and keeps nothing but max(|re|, |im|) per mode (a running maximum per CTA,
-// one atomicMax per mode and CTA at the end).
-// After phase 2 the exchange buffer holds the [mode][T] tile; the slicing pass re-maps the threads to (mode, four
-// consecutive columns): four 16-byte shared loads (rotated by the lane so that a quarter warp covers all banks), three
-// planes x seven digits per element, and one 32-bit store per (plane, slice) carrying the digits of the four columns.
-// =================================================================================================
-struct SliceParams {
-    int8_t* slices[2];
-    unsigned long long* maxbits[2];   // [batch * L] per operand
-    int* exps[2];
-    int layout[2];
-    int pitch[2];                     // bytes per matrix row of a slice (ROWS) / per matrix row of all slices (QUAD)
-    int chunks;                       // tiles per matrix row = ceil(N / T)
-};
-
-template <int R, int S, int T>
-struct SliceCfg {
-    static constexpr int L = R * S;
-    static constexpr int THREADS = T * S;
-    static constexpr int HALF_TILE_BYTES = (L / 2) * T * 16;
-    static constexpr int FULL_TILE_BYTES = L * T * 16;
-    // one input stage is enough: it is read into registers at the start of a tile and refilled at once, so the next tile's
-    // load has the whole transform and slicing pass of this tile to arrive; 96 KB at L = 128 lets two CTAs share an SM,
-    // one in its shared-memory phases while the other computes
-    static constexpr int STAGES = 1;
-    static constexpr int SMEM = STAGES * HALF_TILE_BYTES + FULL_TILE_BYTES + 64 + 128 + L * 8;
-    static constexpr int MIN_CTAS = (2 * SMEM <= 220 * 1024 && 2 * THREADS <= 1024) ? 2 : 1;
-};
-
-template <int R, int S, int T, bool MAXONLY>
-__global__ void __launch_bounds__(T* S, SliceCfg<R, S, T>::MIN_CTAS) fft_forward_slice_kernel(const __grid_constant__ CUtensorMap in0,
-                                                                const __grid_constant__ CUtensorMap in1,
-                                                                const XformParams P, const SliceParams Q) {
-    using C = SliceCfg<R, S, T>;
-    constexpr int NS = C::STAGES, L = C::L, THREADS = C::THREADS;
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
-    uint8_t* sgen = smem_raw + (base - smem_u32(smem_raw));
-    double2* exch = reinterpret_cast<double2*>(sgen + NS * C::HALF_TILE_BYTES);
-    const uint32_t bar = base + NS * C::HALF_TILE_BYTES + C::FULL_TILE_BYTES;   // NS 8-byte mbarriers
-    unsigned long long* smax = reinterpret_cast<unsigned long long*>(sgen + NS * C::HALF_TILE_BYTES + C::FULL_TILE_BYTES + 64);
-
-    const int c = threadIdx.x % T, s = threadIdx.x / T;
-    // the exchange buffer is swizzled within each row (T = 32): column c lives at position c ^ (c >> 3), a permutation
-    // inside aligned groups of four that keeps the phases conflict-free and makes the slicing pass conflict-free too
-    constexpr bool SWZ = (T == 32);
-    const int cs = SWZ ? (c ^ (c >> 3)) : c;
-    const unsigned rows_x = (unsigned)P.N * (unsigned)Q.chunks;   // tiles per (operand, batch element)
-
-    auto coords = [&](unsigned tile, unsigned& cx, unsigned& row, unsigned& b, unsigned& z) {
-        const unsigned tx = tile % rows_x, zb = tile / rows_x;
-        cx = tx % (unsigned)Q.chunks;
-        row = tx / (unsigned)Q.chunks;
-        b = zb % (unsigned)P.batch;
-        z = zb / (unsigned)P.batch;
-    };
-    auto issue = [&](unsigned tile, int stage) {
-        unsigned cx, row, b, z;
-        coords(tile, cx, row, b, z);
-        mbar_expect_tx(bar + 8 * stage, C::HALF_TILE_BYTES);
-        tma_load_4d(base + stage * C::HALF_TILE_BYTES, z ? &in1 : &in0, bar + 8 * stage, (int)(2 * cx * T), (int)row, 0, (int)b);
-    };
-
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int i = 0; i < NS; ++i) mbar_init(bar + 8 * i, 1);
-        mbar_fence_init();
-    }
-    if constexpr (MAXONLY) {
-        for (int m = threadIdx.x; m < L; m += THREADS) smax[m] = 0ull;
-    }
-    // a contiguous range of tiles per CTA: its tiles then share (operand, batch element) except at a few boundaries
-    const unsigned per = (P.total_tiles + gridDim.x - 1) / gridDim.x;
-    const unsigned first = blockIdx.x * per;
-    const unsigned last = first + per < P.total_tiles ? first + per : P.total_tiles;
-    pdl_wait();
-    pdl_trigger();
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int i = 0; i < NS; ++i)
-            if (first + i < last) issue(first + i, i);
-    }
-    if constexpr (!MAXONLY) {
-        // exponents of all modes for the product kernel (one CTA writes them)
-        if (blockIdx.x == 0) {
-            for (int z = 0; z < 2; ++z)
-                if (Q.exps[z])
-                    for (int m = threadIdx.x; m < P.batch * L; m += THREADS) Q.exps[z][m] = oz_exponent(Q.maxbits[z][m]);
-        }
-    }
-    __syncthreads();
-
-    double2 twr[R];
-#pragma unroll
-    for (int p1 = 0; p1 < R; ++p1) twr[p1] = __ldg(&P.tw_fwd[s * p1]);
-    unsigned it = 0;
-    unsigned cur_zb = 0xffffffffu;
-    for (unsigned tile = first; tile < last; ++tile, ++it) {
-        const int stage = it % NS;
-        unsigned cx, row, b, z;
-        coords(tile, cx, row, b, z);
-        if constexpr (!MAXONLY) {
-            const unsigned zb = z * (unsigned)P.batch + b;
-            if (zb != cur_zb) {   // the scales 2^(54 - e) of the modes of this series, from the maxima of the first pass
-                __syncthreads();
-                for (int m = threadIdx.x; m < L; m += THREADS)
-                    smax[m] = (unsigned long long)__double_as_longlong(oz_pow2(OZ_FRAC_BITS - oz_exponent(Q.maxbits[z][b * L + m])));
-                cur_zb = zb;   // made visible by the barriers of the transform below
-            }
-        }
-        if constexpr (MAXONLY) {
-            const unsigned zb = z * (unsigned)P.batch + b;
-            if (zb != cur_zb) {   // flush the running maxima when the CTA moves on to another series
-                if (cur_zb != 0xffffffffu) {
-                    const unsigned oz = cur_zb / (unsigned)P.batch, ob = cur_zb % (unsigned)P.batch;
-                    for (int m = threadIdx.x; m < L; m += THREADS) {
-                        if (smax[m]) atomicMax(Q.maxbits[oz] + ob * L + m, smax[m]);
-                        smax[m] = 0ull;
-                    }
-                    __syncthreads();
-                }
-                cur_zb = zb;
-            }
-        }
-        mbar_wait(bar + 8 * stage, (it / NS) & 1);
-        const double2* in = reinterpret_cast<const double2*>(sgen + stage * C::HALF_TILE_BYTES);
-        double2 x[R];
-#pragma unroll
-        for (int r = 0; r < R / 2; ++r) {
-            const int k = S * r + s;
-            double2 v = in[k * T + c];  // orders >= n and columns >= N were zero-filled by TMA (Step 1's padding)
-            if (P.use_scale && k < P.n) {
-                const double sc = __ldg(&P.scale_in[k]);
-                v.x *= sc;
-                v.y *= sc;
-            }
-            if (P.skip_order0 && k == 0) v = make_double2(0.0, 0.0);
-            x[r] = v;
-        }
-#pragma unroll
-        for (int r = R / 2; r < R; ++r) x[r] = make_double2(0.0, 0.0);
-        __syncthreads();  // input stage consumed by everyone; the previous tile's slicing pass has left the exchange buffer
-        if (threadIdx.x == 0) {
-            const unsigned next = tile + NS;
-            if (next < last) issue(next, stage);
-        }
-        forward_phase1_smem<R, S, T, true>(x, s, cs, P.tw_fwd, exch, twr);
-        __syncthreads();
-        forward_phase2_smem<R, S, T>(s, cs, exch);
-        __syncthreads();
-        // ---- second mapping: task = (mode, four consecutive columns)
-        constexpr int PARTS = T / 4, TASKS = L * PARTS;
-        static_assert(TASKS % THREADS == 0, "tasks per thread");
-#pragma unroll 1
-        for (int q = 0; q < TASKS / THREADS; ++q) {
-            const int id = q * THREADS + threadIdx.x;
-            const int mode = id / PARTS, part = id % PARTS;
-            double2 v[4];
-            // column 4 part + e sits at position 4 part + (e ^ (part >> 1)) of the row (swizzle of the exchange buffer):
-            // for a fixed e the eight lanes of a quarter warp hit eight different 16-byte bank groups
-#pragma unroll
-            for (int e = 0; e < 4; ++e) v[e] = exch[mode * T + 4 * part + (SWZ ? (e ^ ((part >> 1) & 3)) : e)];
-            if constexpr (MAXONLY) {
-                double m = 0.0;
-#pragma unroll
-                for (int e = 0; e < 4; ++e) m = fmax(m, fmax(fabs(v[e].x), fabs(v[e].y)));
-#pragma unroll
-                for (int o = PARTS / 2; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-                if (part == 0) {
-                    const unsigned long long mb = (unsigned long long)__double_as_longlong(m);
-                    if (mb > smax[mode]) smax[mode] = mb;   // one thread per mode and tile: no race
-                }
-            } else {
-                const double sc = __longlong_as_double((long long)smax[mode]), sc_sum = 0.5 * sc;
-                unsigned int lo[OZ_PLANES][4], hi[OZ_PLANES][4];
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    oz_digits2(v[e].x, sc, lo[0][e], hi[0][e]);
-                    oz_digits2(v[e].y, sc, lo[1][e], hi[1][e]);
-                    oz_digits2(v[e].x + v[e].y, sc_sum, lo[2][e], hi[2][e]);
-                }
-                const int col = (int)cx * T + 4 * part;
-                const bool quad = Q.layout[z] == OZ_QUAD;
-                const size_t plane_stride = quad ? (size_t)P.N * Q.pitch[z] : (size_t)OZ_S * P.N * Q.pitch[z];
-                const size_t slice_stride = quad ? (size_t)32 : (size_t)P.N * Q.pitch[z];
-                int8_t* dst = Q.slices[z] + (size_t)(b * L + mode) * OZ_PLANES * plane_stride + (size_t)row * Q.pitch[z] +
-                              (quad ? (size_t)(col >> 5) * 256 + (col & 31) : (size_t)col);
-                // ROWS: columns >= N inside the pitch receive zeros as well (never read: the tensor map ends at N)
-#pragma unroll
-                for (int pl = 0; pl < OZ_PLANES; ++pl) {
-                    // 4 x 4 byte transposes: word d = digit d (weight 256^d) of the four columns = slice 6 - d
-                    unsigned int w[8];
-                    transpose4x4(lo[pl], w);
-                    transpose4x4(hi[pl], w + 4);
-#pragma unroll
-                    for (int d = 0; d < OZ_S; ++d)
-                        *reinterpret_cast<unsigned int*>(dst + (size_t)pl * plane_stride + (size_t)(OZ_S - 1 - d) * slice_stride) = w[d];
-                }
-            }
-        }
-    }
-    if constexpr (MAXONLY) {
-        __syncthreads();
-        if (cur_zb != 0xffffffffu) {
-            const unsigned oz = cur_zb / (unsigned)P.batch, ob = cur_zb % (unsigned)P.batch;
-            for (int m = threadIdx.x; m < L; m += THREADS)
-                if (smax[m]) atomicMax(Q.maxbits[oz] + ob * L + m, smax[m]);
-        }
-    }
-}
-
 // Inverse (+ 1/L, truncation, unscale) and, with RETRUNC, the fused inverse -> truncate -> forward pass.
 template <int R, int S, int T, bool RETRUNC>
 __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_constant__ CUtensorMap in_map,
@@ -975,34 +757,6 @@ cudaError_t run_tma(Which w, XformParams P, int nops, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-template <int R, int S, int T>
-cudaError_t run_slices(XformParams P, SliceParams Q, int nops, cudaStream_t st) {
-    using C = SliceCfg<R, S, T>;
-    Q.chunks = ((P.N + 31) / 32 * 32 + T - 1) / T;   // whole 32-column k-chunks of the QUAD layout
-    P.tiles_x = (unsigned)P.N * (unsigned)Q.chunks;
-    P.total_tiles = P.tiles_x * (unsigned)P.batch * (unsigned)nops;
-    cudaError_t e;
-    // series viewed as doubles: (2 N per matrix row, N rows, n orders, batch)
-    const uint64_t dims[4] = {(uint64_t)(2 * P.N), (uint64_t)P.N, (uint64_t)P.n, (uint64_t)P.batch};
-    const uint64_t strides[3] = {(uint64_t)P.N * 16, (uint64_t)P.NN * 16, (uint64_t)P.n * P.NN * 16};
-    const uint32_t box[4] = {2 * T, 1, (uint32_t)(C::L / 2), 1};
-    CUtensorMap in[2];
-    for (int z = 0; z < 2; ++z) {
-        const void* src = P.src_series[z] ? (const void*)P.src_series[z] : (const void*)P.src_series[0];
-        if ((e = tma_encode_f64(&in[z], src, 4, dims, strides, box, false)) != cudaSuccess) return e;
-    }
-    unsigned grid = 0;
-    auto kmax = fft_forward_slice_kernel<R, S, T, true>;
-    if ((e = persistent_grid(kmax, C::THREADS, C::SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
-    static const int dbg = getenv("NSPT_FS_DBG") ? atoi(getenv("NSPT_FS_DBG")) : 0;   // 1: no max pass, 2: no slicing pass
-    if (!(dbg & 1))
-    if ((e = launch_pdl(kmax, grid, C::THREADS, C::SMEM, st, in[0], in[1], P, Q)) != cudaSuccess) return e;
-    if (dbg & 2) return cudaSuccess;
-    auto kslice = fft_forward_slice_kernel<R, S, T, false>;
-    if ((e = persistent_grid(kslice, C::THREADS, C::SMEM, P.total_tiles, &grid)) != cudaSuccess) return e;
-    return launch_pdl(kslice, grid, C::THREADS, C::SMEM, st, in[0], in[1], P, Q);
-}
-
 cudaError_t dispatch(int L, Which w, const XformParams& P, int nops, cudaStream_t st) {
     switch (L) {
         case 1: return run_small<1, 128>(w, P, nops, st);
@@ -1054,41 +808,6 @@ cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int bat
     P.dst_freq[1] = reinterpret_cast<double2*>(dst1);
     P.use_scale = (t.scale_in != nullptr) ? 1 : 0;
     return dispatch(f.L, W_FWD, P, src1 ? 2 : 1, st);
-}
-
-bool fft_slices_supported(int L) { return L >= 16 && L <= 256 && (L & (L - 1)) == 0; }
-
-// Forward transforms of one or two operands straight into int8 slices: a max-only pass (per-mode exponents), then the
-// slicing pass.  dst[z].maxbits is cleared here.
-cudaError_t launch_fft_forward_slices(const FreqLayout& f, const PlanTables& t, int batch, const nspt_c128* src0,
-                                      const OzSliceDst& dst0, const nspt_c128* src1, const OzSliceDst& dst1, cudaStream_t st,
-                                      bool skip_order0) {
-    XformParams P = base_params(f, t, batch);
-    P.skip_order0 = skip_order0 ? 1 : 0;
-    P.src_series[0] = reinterpret_cast<const double2*>(src0);
-    P.src_series[1] = reinterpret_cast<const double2*>(src1);
-    P.use_scale = (t.scale_in != nullptr) ? 1 : 0;
-    SliceParams Q{};
-    const OzSliceDst* d[2] = {&dst0, &dst1};
-    const int nops = src1 ? 2 : 1;
-    cudaError_t e;
-    for (int z = 0; z < nops; ++z) {
-        Q.slices[z] = d[z]->slices;
-        Q.maxbits[z] = d[z]->maxbits;
-        Q.exps[z] = d[z]->exps;
-        Q.layout[z] = d[z]->layout;
-        Q.pitch[z] = d[z]->layout == OZ_QUAD ? oz_pitch_quad(f.N) : oz_pitch_rows(f.N);
-        if ((e = cudaMemsetAsync(d[z]->maxbits, 0, sizeof(unsigned long long) * batch * f.L, st)) != cudaSuccess) return e;
-    }
-    static const int tsel = getenv("NSPT_FS_T") ? atoi(getenv("NSPT_FS_T")) : 32;
-    switch (f.L) {
-        case 16: return run_slices<4, 4, 32>(P, Q, nops, st);
-        case 32: return run_slices<8, 4, 32>(P, Q, nops, st);
-        case 64: return tsel == 16 ? run_slices<8, 8, 16>(P, Q, nops, st) : run_slices<8, 8, 32>(P, Q, nops, st);
-        case 128: return tsel == 16 ? run_slices<16, 8, 16>(P, Q, nops, st) : run_slices<16, 8, 32>(P, Q, nops, st);
-        case 256: return run_slices<16, 16, 16>(P, Q, nops, st);
-        default: return cudaErrorInvalidValue;
-    }
 }
 
 cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int batch, const double* src,

@@ -124,12 +124,14 @@ cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup*
 cudaError_t launch_naive_conv(const FreqLayout& f, int batch, const nspt_c128* A, const nspt_c128* B, nspt_c128* C,
                               cudaStream_t st);
 
-// ---- mode-wise matrix product on the INT8 tensor cores (nspt_ozaki.cu; gemm variant 2) -------------------------
-// Plain C~(p) = A~(p) B~(p) only (no alpha / accumulate / dagger epilogues): FP64 spectra are cut into int8 slices
-// (launch_ozaki_slice), multiplied exactly by tcgen05.mma.kind::i8 and recombined in FP64 (launch_ozaki_gemm).
+// ---- mode-wise matrix product on the INT8 tensor cores (nspt_ozaki.cu) -----------------------------------------
+// Plain C~(p) = A~(p) B~(p) only (no alpha / accumulate / dagger epilogues): the FP64 spectra, whose per-mode maxima the
+// forward transform has recorded in the slice workspace (ozaki_maxbits), are cut into int8 slices (launch_ozaki_slice),
+// multiplied exactly by tcgen05.mma.kind::i8 and recombined in FP64 (launch_ozaki_gemm).
 size_t ozaki_workspace_bytes(const FreqLayout& f, int batch);
+// where the forward transform records max(|re|, |im|) of every mode of operand z (0 = A, 1 = B): batch * L entries each
+unsigned long long* ozaki_maxbits(const FreqLayout& f, int batch, void* ws, int z);
 cudaError_t launch_ozaki_slice(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st);
-cudaError_t launch_ozaki_slice2(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st);
-cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st, int kernel = -1);
+cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st, bool pairs = false);
 
 }  // namespace nspt

@@ -11,17 +11,23 @@
 // each [..] an INT8 x INT8 -> INT32 matrix product that the tensor core evaluates EXACTLY (|q q'| <= 2^14, K <= 2^11 terms,
 // <= 7 pairs per d: < 2^28).  Pairs with s + t > 6 are dropped (their total is below 2^-51 of the leading term), 28 pairs
 // remain.  Only two roundings are not exact: the digit extraction (relative 2^-55 of the mode's largest element) and the
-// final FP64 recombination.
+// final FP64 recombination.  The exponents e come from the forward transform, which records max(|re|, |im|) of every mode
+// while it writes the FP64 spectra (nspt_fft.cu); one slicing pass then cuts both spectra.
 //
-// Kernel.  CTA tile 64 rows x 128 columns of one mode, computed transposed (see OZ_BM below); K-chunks of 32 arrive by TMA
-// (SWIZZLE_128B) in a four-stage ring, all seven slices of both operands at once (44 KB per stage).  One thread issues
-// tcgen05.mma.kind::i8 (M=128, N=64, K=32): 28 per stage, into seven TMEM accumulators (d = 0..6, 64 columns each, 448 of
-// the 512 columns); runs of MMAs with the same M-side slice fetch it once (collector reuse).  The three planes run one
-// after the other through the same accumulators; eight epilogue warps drain them with tcgen05.ld, recombine the seven
-// INT32 sums in FP64 (Horner in 2^-8) and keep the running real / imaginary parts of the 3M product in registers.
+// Product kernel.  Persistent CTAs, tile = 64 rows x 128 columns of one mode, computed transposed (the M side of the MMA,
+// 128 TMEM lanes, runs over output columns j and reads B~ slices MN-major; the N side runs over output rows i and reads
+// A~ slices K-major); K-chunks of 32 arrive by TMA (SWIZZLE_128B) in a ring, all seven slices of both operands at once
+// (44 KB per stage).  One lane of warp 1 issues tcgen05.mma.kind::i8 (M=128, N=64, K=32): 28 per stage, into seven TMEM
+// accumulators (d = 0..6, 64 columns each, 448 of the 512 columns); runs of MMAs with the same M-side slice fetch it once
+// (collector reuse).  The three planes run one after the other through the same accumulators; eight epilogue warps drain
+// them with tcgen05.ld, recombine the seven INT32 sums in FP64 (Horner in 2^-8) and keep the running real / imaginary
+// parts of the 3M product in registers; the scaling and stores of a tile overlap the next tile's MMAs.  With CG = 2 a CTA
+// PAIR computes 256 columns x 64 rows (tcgen05.mma.cta_group::2, M = 256): each CTA stages its own 128 columns of the
+// M side and half of the N-side rows.  Measured on B200 at N = 225, L = 128: a stage of 28 MMAs takes
+// 1200 cycles with one CTA per tile (bound by shared-memory bandwidth: 84 KB read by the tensor core + 44 KB written by
+// TMA per stage) and 980 with pairs (the tensor-core rate), the drain of the seven accumulators 2200-2900 cycles per
+// plane; 166 us per product either way against 325 us on the FP64 tensor pipe.
 #include <cuda.h>
-#include <cstdio>
-#include <cstdlib>
 
 #include "nspt_internal.cuh"
 #include "nspt_ozaki.cuh"
@@ -30,104 +36,27 @@
 namespace nspt {
 namespace {
 
-// Operand staging, measured on B200 with probes of the TMA unit and of tcgen05.mma.kind::i8: the TMA unit is row-rate bound
-// (1.9 cycles per row of <= 128 bytes with all SMs loading), so every shared-memory row is 128 bytes; a 128 x 64 x 32 MMA
-// takes 46-58 cycles depending on the operand layouts (32 would be the tensor rate, reached only from N = 128 up, which the
-// seven accumulators leave no room for in TMEM).  The tensor core computes the TRANSPOSED tile D[j][i] = sum_k B~[k][j] A~[i][k]:
-// its M side (128 TMEM lanes) runs over output columns j and reads B~ slices MN-major -- the row-major layout the transforms
-// write -- and its N side (64 TMEM columns) runs over output rows i and reads A~ slices K-major from 128-byte rows that carry
-// four slices of one 32-column k-chunk (QUAD layout below; the slice is selected by a 32-byte offset inside the swizzled
-// row).  The epilogue then writes 512 contiguous bytes of a row of C~ per warp.  (The untransposed arrangement, 64-byte rows
-// for B~ and per-thread row segments in the epilogue, measured 9 % slower.)
-constexpr int OZ_BM = 128, OZ_BN = 64, OZ_KC = 32;   // CTA tile (j x i) and K per stage = K of one tcgen05.mma.kind::i8
-constexpr int OZ_STAGES = 4;
+// Operand staging, measured on B200 with probes of the TMA unit and of tcgen05.mma.kind::i8: the TMA unit is
+// row-rate bound (1.9 cycles per row of <= 128 bytes with all SMs loading), so every shared-memory row is 128 bytes; a
+// 128 x 64 x 32 MMA takes 35 cycles in a run that reuses the M-side operand from the collector and 48 without (32 is the
+// tensor rate; N = 128 and 256 reach it, but seven accumulators of 128 columns do not fit the 512 columns of TMEM).  The tensor
+// core computes the TRANSPOSED tile D[j][i] = sum_k B~[k][j] A~[i][k]: its M side (128 TMEM lanes) runs over output columns j
+// and reads B~ slices MN-major -- the row-major layout the transforms write -- and its N side (64 TMEM columns) runs over
+// output rows i and reads A~ slices K-major from 128-byte rows that carry four slices of one 32-column k-chunk (QUAD layout;
+// the slice is selected by a 32-byte offset inside the swizzled row).  The epilogue then writes 512 contiguous bytes of a row of
+// C~ per warp.  (The untransposed arrangement, 64-byte rows for B~ and per-thread row segments in the epilogue, measured 9 %
+// slower.)
+constexpr int OZ_BM = 128, OZ_BN = 64, OZ_KC = 32;   // tile of one CTA (j x i) and K per stage = K of one tcgen05.mma.kind::i8
 constexpr int OZ_M_SLICE = OZ_KC * OZ_BM;            // B~ slice of a stage: [32 k][128 bytes of j] = 4096
 constexpr int OZ_M_STAGE = OZ_S * OZ_M_SLICE;        // 28672
-constexpr int OZ_N_HALF = OZ_BN * 128;               // A~ slices 4h..4h+3 of a stage: [64 i][4 slices x 32 bytes of k] = 8192
-constexpr int OZ_N_STAGE = 2 * OZ_N_HALF;            // 16384
-constexpr int OZ_STAGE = OZ_M_STAGE + OZ_N_STAGE;    // 45056
-constexpr int OZ_SMEM = OZ_STAGES * OZ_STAGE + 1024 + 128;
 constexpr int OZ_THREADS = 384;                      // warp 0 TMA, warp 1 MMA, warp 2 TMEM allocator, warps 4-11 epilogue
 constexpr int OZ_TMEM_COLS = 512;
 
-static_assert(OZ_STAGE % 1024 == 0 && OZ_M_STAGE % 1024 == 0, "stage alignment");
-
 // ---- slicing ------------------------------------------------------------------------------------------------
-// max over a mode of max(|re|, |im|) as the bit pattern of a non-negative double (ordered like an unsigned integer)
-__global__ void __launch_bounds__(256) oz_absmax_kernel(const double2* __restrict__ X, unsigned long long* __restrict__ maxbits,
-                                                      size_t NN, int modes) {
-    __shared__ double red[8];
-    for (int mode = blockIdx.y; mode < modes; mode += gridDim.y) {   // the grid's y extent is capped at 65535
-    const double2* x = X + (size_t)mode * NN;
-    double m = 0.0;
-    for (size_t e = (size_t)blockIdx.x * 256 + threadIdx.x; e < NN; e += (size_t)gridDim.x * 256) {
-        const double2 v = x[e];
-        m = fmax(m, fmax(fabs(v.x), fabs(v.y)));
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int w = 1; w < 8; ++w) m = fmax(m, red[w]);
-        atomicMax(maxbits + mode, (unsigned long long)__double_as_longlong(m));
-    }
-    }
-}
-
-// Slice layouts in global memory (both from row-major FP64 spectra X[mode][row][col]):
-//   ROWS layout (right factor B~, read MN-major):  [mode][plane][slice][row k][pitch bytes of col j]
-//   QUAD layout (left factor A~, read K-major):    [mode][plane][row i][k-chunk of 32][8 slots][32 bytes of col k]
-//     slot s < 7 holds slice s (slot 7 is padding): a 128-byte shared-memory row carries four slices of one k-chunk, and
-//     the k-step of a tcgen05.mma selects the slice by a 32-byte offset inside the swizzled row.  k is padded to a multiple
-//     of 32 with explicit zeros.
-// thread = 4 consecutive columns of a row
-template <bool QUAD>
-__global__ void __launch_bounds__(256) oz_slice_kernel(const double2* __restrict__ X, int8_t* __restrict__ out,
-                                                      const unsigned long long* __restrict__ maxbits, int* __restrict__ exps,
-                                                      int N, int pitch, int modes) {
-    for (int mode = blockIdx.y; mode < modes; mode += gridDim.y) {   // the grid's y extent is capped at 65535
-    const int qpr = QUAD ? (pitch >> 5) : ((N + 3) >> 2);   // 4-column groups per row (QUAD: 256 bytes of pitch per 32 columns, k padded)
-    const int t = blockIdx.x * 256 + threadIdx.x;
-    const int e = oz_exponent(maxbits[mode]);
-    if (t == 0) exps[mode] = e;
-    if (t >= N * qpr) continue;
-    const int row = t / qpr, j0 = (t % qpr) * 4;
-    const double sc = oz_pow2(OZ_FRAC_BITS - e), sc_sum = oz_pow2(OZ_FRAC_BITS - e - 1);
-    const double2* x = X + ((size_t)mode * N + row) * N + j0;
-    unsigned long long w[OZ_PLANES][4];
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        double2 v = make_double2(0.0, 0.0);
-        if (j0 + c < N) v = x[c];
-        w[0][c] = oz_digits(v.x, sc);
-        w[1][c] = oz_digits(v.y, sc);
-        w[2][c] = oz_digits(v.x + v.y, sc_sum);
-    }
-    const size_t plane_stride = QUAD ? (size_t)N * pitch : (size_t)OZ_S * N * pitch;
-    int8_t* base = out + (size_t)mode * OZ_PLANES * plane_stride + (size_t)row * pitch +
-                   (QUAD ? (size_t)(j0 >> 5) * 256 + (j0 & 31) : (size_t)j0);
-#pragma unroll
-    for (int q = 0; q < OZ_PLANES; ++q) {
-#pragma unroll
-        for (int s = 0; s < OZ_S; ++s) {
-            const int byte = OZ_S - 1 - s;   // slice s has weight 2^(-6-8s): digit 6 - s
-            unsigned int word = 0;
-#pragma unroll
-            for (int c = 0; c < 4; ++c) word |= (unsigned int)((w[q][c] >> (8 * byte)) & 0xffull) << (8 * c);
-            // ROWS: pitch is a multiple of 64 and j0 of 4; pad columns N..pitch-1 receive zeros (never read: TMA clips at N)
-            *reinterpret_cast<unsigned int*>(base + (size_t)q * plane_stride + (QUAD ? (size_t)s * 32 : (size_t)s * N * pitch)) = word;
-        }
-    }
-    }
-}
-
-// Second-generation slicing pass: both operands in one launch (blockIdx.z), the per-mode maxima come from the forward
-// transform (maxbits), digits without 64-bit conversions (oz_digits2), 4 x 4 byte transposes for the packing.
+// Slicing pass: both operands in one launch (blockIdx.z), the per-mode maxima come from the forward transform (maxbits),
+// digits without 64-bit conversions (oz_fixed), 4 x 4 byte transposes for the packing.
 // thread = 4 consecutive columns of a row of one mode; a warp writes 128 contiguous bytes per (plane, slice).
-struct Slice2Params {
+struct SliceParams {
     const double2* X[2];
     int8_t* out[2];
     const unsigned long long* maxbits[2];
@@ -174,7 +103,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // warp (stride four elements) cover all banks
 __device__ __forceinline__ int oz_swz(int p) { return p ^ ((p >> 3) & 3); }
 
-__global__ void __launch_bounds__(256) oz_slice2_kernel(const Slice2Params P) {
+__global__ void __launch_bounds__(256) oz_slice_kernel(const SliceParams P) {
     __shared__ double2 stage[2][OZ_SLICE_BUF];
     __shared__ double ssc[OZ_SLICE_MODES];
     const int z = blockIdx.z;
@@ -243,39 +172,9 @@ __device__ __forceinline__ void tc_alloc(uint32_t smem_dst, uint32_t cols) {
 __device__ __forceinline__ void tc_dealloc(uint32_t taddr, uint32_t cols) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
 }
-// COLLECT: use of the A-operand (M side) collector buffer -- consecutive MMAs with the same M-side slice read it from shared
-// memory once: 0 = no reuse, 1 = fill (first of a run), 2 = use (middle), 3 = last use.  Without it a 128 x 64 x 32 MMA
-// reads 6 KB of shared memory in 32 cycles, more than the 128 bytes per cycle an SM delivers.
-template <int COLLECT>
-__device__ __forceinline__ void tc_mma_i8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-#define NSPT_OZ_MMA(Q)                                                                             \
-    asm volatile(                                                                                  \
-        "{\n"                                                                                      \
-        ".reg .pred p;\n"                                                                          \
-        "setp.ne.b32 p, %4, 0;\n"                                                                  \
-        "tcgen05.mma.cta_group::1.kind::i8" Q " [%0], %1, %2, %3, p;\n"                            \
-        "}\n" ::"r"(d_tmem),                                                                       \
-        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)                                      \
-        : "memory")
-    if constexpr (COLLECT == 1)
-        NSPT_OZ_MMA(".collector::a::fill");
-    else if constexpr (COLLECT == 2)
-        NSPT_OZ_MMA(".collector::a::use");
-    else if constexpr (COLLECT == 3)
-        NSPT_OZ_MMA(".collector::a::lastuse");
-    else
-        NSPT_OZ_MMA("");
-#undef NSPT_OZ_MMA
-}
 // arrive on an mbarrier once every tcgen05.mma issued so far by this thread has completed
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void tc_ld8(uint32_t taddr, int (&r)[8]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                 : "r"(taddr)
-                 : "memory");
 }
 __device__ __forceinline__ void tc_ld4(uint32_t taddr, int (&r)[4]) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
@@ -299,189 +198,25 @@ __device__ __forceinline__ uint64_t oz_desc(uint32_t addr, uint32_t lbo_bytes, u
     const uint32_t hi = ((sbo_bytes >> 4) & 0x3fffu) | (1u << 14) /* version 1 (sm_100) */ | (2u << 29) /* SWIZZLE_128B */;
     return ((uint64_t)hi << 32) | lo;
 }
-// instruction descriptor: D = S32, A = B = signed int8, A (M side) MN-major, B (N side) K-major, N = 64, M = 128
-constexpr uint32_t OZ_IDESC = (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (0u << 16) | ((OZ_BN >> 3) << 17) | ((OZ_BM >> 4) << 24);
-
 // exact int32 -> double (no I2F): 2^52 + 2^31 + x has x + 2^31 in its low mantissa word
 __device__ __forceinline__ double oz_i2d(int x) {
     return __hiloint2double(0x43300000, (int)((unsigned)x ^ 0x80000000u)) - 4503601774854144.0;
 }
 
-// All pairs (t, s), s + t <= 6, of one stage: B~ slice t (M side) times A~ slice s (N side) into accumulator d = s + t.
-// Runs of equal t are consecutive (collector reuse of the M-side operand).
-//   M side, slice t: [32 rows of k][128 bytes of j], MN-major: 8-row k groups 1024 bytes apart
-//   N side, slice s: rows of [64 i][128 bytes] in half s / 4, K-major: 8-row groups 1024 bytes apart, slice = +32 (s % 4) bytes
-template <int T0, int S0>
-__device__ __forceinline__ void oz_issue_pairs(uint32_t tmem, uint32_t sm, uint32_t sn, bool not_first_k) {
-    constexpr int LAST = OZ_S - 1 - T0;
-    constexpr int COLLECT = (LAST == 0) ? 0 : (S0 == 0 ? 1 : (S0 == LAST ? 3 : 2));
-    const uint64_t dm = oz_desc(sm + T0 * OZ_M_SLICE, 4096, 1024);
-    const uint64_t dn = oz_desc(sn + (S0 >> 2) * OZ_N_HALF + (S0 & 3) * 32, 16, 1024);
-    tc_mma_i8<COLLECT>(tmem + (uint32_t)((S0 + T0) * OZ_BN), dm, dn, OZ_IDESC, (not_first_k || T0 != 0) ? 1u : 0u);
-    if constexpr (S0 < LAST)
-        oz_issue_pairs<T0, S0 + 1>(tmem, sm, sn, not_first_k);
-    else if constexpr (T0 + 1 < OZ_S)
-        oz_issue_pairs<T0 + 1, 0>(tmem, sm, sn, not_first_k);
-}
-
-struct OzParams {
-    double2* C;
-    const int* expA;
-    const int* expB;
-    size_t NN;
-    int N;
-    int tiles_i, tiles_j;
-    int nkc;
-};
-
-__global__ void __launch_bounds__(OZ_THREADS, 1)
-zgemm_modes_ozaki_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_constant__ CUtensorMap mapN, const OzParams P) {
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bar_full = base + OZ_STAGES * OZ_STAGE;          // OZ_STAGES barriers
-    const uint32_t bar_empty = bar_full + 8 * OZ_STAGES;
-    const uint32_t bar_acc_full = bar_empty + 8 * OZ_STAGES;
-    const uint32_t bar_acc_empty = bar_acc_full + 8;
-    const uint32_t tmem_slot = bar_acc_empty + 8;
-    volatile uint32_t* tmem_slot_gen =
-        reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int tiles = P.tiles_i * P.tiles_j;
-    const int mode = blockIdx.x / tiles, tile = blockIdx.x % tiles;
-    const int i0 = (tile / P.tiles_j) * OZ_BN, j0 = (tile % P.tiles_j) * OZ_BM;
-    const int nkc = P.nkc;
-
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int s = 0; s < OZ_STAGES; ++s) {
-            mbar_init(bar_full + 8 * s, 1);
-            mbar_init(bar_empty + 8 * s, 1);
-        }
-        mbar_init(bar_acc_full, 1);
-        mbar_init(bar_acc_empty, 8);
-        mbar_fence_init();
-    }
-    if (warp == 2) tc_alloc(tmem_slot, OZ_TMEM_COLS);
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem = *tmem_slot_gen;
-    pdl_wait();
-    pdl_trigger();
-
-    // the epilogue keeps a 128 x 64 complex FP64 tile in registers (128 per thread): take them from the warps that only issue
-    if (warp < 4) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-        if (warp == 0) {
-            // ------------------------------------------------------------ TMA producer
-            if (lane == 0) {
-                int it = 0;
-                for (int plane = 0; plane < OZ_PLANES; ++plane) {
-                    const int pidx = mode * OZ_PLANES + plane;
-                    for (int kc = 0; kc < nkc; ++kc, ++it) {
-                        const int slot = it % OZ_STAGES;
-                        mbar_wait(bar_empty + 8 * slot, ((it / OZ_STAGES) & 1) ^ 1);
-                        mbar_expect_tx(bar_full + 8 * slot, OZ_STAGE);
-                        const uint32_t st = base + slot * OZ_STAGE;
-                        tma_load_4d(st, &mapM, bar_full + 8 * slot, j0, kc * OZ_KC, 0, pidx);
-                        tma_load_5d(st + OZ_M_STAGE, &mapN, bar_full + 8 * slot, 0, i0, 0, kc, pidx);
-                    }
-                }
-            }
-        } else if (warp == 1) {
-            // ------------------------------------------------------------ MMA issuer (one thread)
-            if (lane == 0) {
-                int it = 0;
-                for (int plane = 0; plane < OZ_PLANES; ++plane) {
-                    if (plane > 0) mbar_wait(bar_acc_empty, (plane - 1) & 1);
-                    tc_fence_after();
-                    for (int kc = 0; kc < nkc; ++kc, ++it) {
-                        const int slot = it % OZ_STAGES;
-                        mbar_wait(bar_full + 8 * slot, (it / OZ_STAGES) & 1);
-                        tc_fence_after();
-                        const uint32_t sm = base + slot * OZ_STAGE;
-                        oz_issue_pairs<0, 0>(tmem, sm, sm + OZ_M_STAGE, kc != 0);
-                        tc_commit(bar_empty + 8 * slot);   // the stage may be refilled once these MMAs have read it
-                    }
-                    tc_commit(bar_acc_full);
-                }
-            }
-        }
-    } else {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
-        // ------------------------------------------------------------ epilogue: 8 warps, warp w reads TMEM lanes 32 (w % 4) ..
-        // lane of the accumulator = output column j, column of the accumulator = output row i
-        const int we = warp - 4, quarter = we & 3, half = we >> 2;
-        const int col = j0 + 32 * quarter + lane;
-        const int row0 = i0 + 32 * half;
-        double re[32], im[32];
-#pragma unroll
-        for (int j = 0; j < 32; ++j) re[j] = im[j] = 0.0;
-        for (int plane = 0; plane < OZ_PLANES; ++plane) {
-            // 3M: Cr = P1 - P2, Ci = 4 P3 - P1 - P2 (the sum planes carry one more exponent bit each)
-            const double cr = plane == 0 ? 1.0 : (plane == 1 ? -1.0 : 0.0);
-            const double ci = plane == 2 ? 4.0 : -1.0;
-            mbar_wait(bar_acc_full, plane & 1);
-            tc_fence_after();
-#pragma unroll
-            for (int cc = 0; cc < 4; ++cc) {
-                int a[OZ_S][8];
-#pragma unroll
-                for (int d = 0; d < OZ_S; ++d)
-                    tc_ld8(tmem + ((uint32_t)(32 * quarter) << 16) + (uint32_t)(d * OZ_BN + 32 * half + 8 * cc), a[d]);
-                tc_wait_ld();
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    double h = oz_i2d(a[OZ_S - 1][j]);
-#pragma unroll
-                    for (int d = OZ_S - 2; d >= 0; --d) h = fma(h, 0.00390625, oz_i2d(a[d][j]));
-                    re[8 * cc + j] = fma(cr, h, re[8 * cc + j]);
-                    im[8 * cc + j] = fma(ci, h, im[8 * cc + j]);
-                }
-            }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_acc_empty);
-        }
-        const int esum = P.expA[mode] + P.expB[mode];
-        const double sc = esum >= (1 << 20) ? __longlong_as_double(0x7ff8000000000000ll) : oz_pow2(esum - 12);
-        if (col < P.N) {
-            double2* c = P.C + (size_t)mode * P.NN + col;
-#pragma unroll
-            for (int j = 0; j < 32; ++j)   // the 32 lanes of a warp write 512 contiguous bytes of row row0 + j
-                if (row0 + j < P.N) c[(size_t)(row0 + j) * P.N] = make_double2(sc * re[j], sc * im[j]);
-        }
-    }
-    tc_fence_before();
-    __syncthreads();
-    if (warp == 2) tc_dealloc(tmem, OZ_TMEM_COLS);
-}
-
-
 // =====================================================================================================================
-// Second-generation kernel: persistent, one tile per CTA PAIR (tcgen05.mma.cta_group::2, M = 256) or per CTA (CG = 1).
-// The pair computes a 256 (j) x 64 (i) tile: each CTA keeps the seven 128 x 64 INT32 accumulators of its own 128 output
-// columns j in its own TMEM and stages its own half of both operands -- the M-side slices of its 128 columns and 32 of the 64
-// rows of the N-side slices -- so a stage is 36 KB per SM instead of 44 KB and every byte of the N-side operand is read from
-// shared memory by one SM only (the single-CTA kernel above is bound by shared-memory and L2 bandwidth, not by the tensor
-// core).  The leader CTA issues the MMAs for both; TMA loads of both CTAs report to the leader's "full" barrier, MMA
-// completion is multicast to both CTAs' "empty" / "accumulator full" barriers, and the epilogue warps of both CTAs report to
-// the leader's "accumulator empty" barrier.  CTAs are persistent (static round-robin schedule over tiles): barrier set-up and
-// the TMEM allocation happen once, the producer runs ahead into the next tile while the accumulators drain, and the final
-// scaling and stores of a tile overlap the next tile's MMAs.
+// The product kernel (see the head of the file).  Barrier protocol with CG = 2: TMA loads of both CTAs report to the
+// leader's "full" barrier, MMA completion is multicast to both CTAs' "empty" / "accumulator full" barriers, and the epilogue
+// warps of both CTAs report to the leader's "accumulator empty" barrier.
 // =====================================================================================================================
-constexpr int OZ2_BN = 64;
-constexpr int OZ2_THREADS = 384;
 template <int CG>
-struct Oz2 {
-    static constexpr int N_ROWS = OZ2_BN / CG;               // rows of the N-side operand staged by one CTA
+struct OzCfg {
+    static constexpr int N_ROWS = OZ_BN / CG;               // rows of the N-side operand staged by one CTA
     static constexpr int N_HALF = N_ROWS * 128;              // slices 4h..4h+3 of a stage
     static constexpr int N_STAGE = 2 * N_HALF;
     static constexpr int STAGE = OZ_M_STAGE + N_STAGE;       // 45056 (CG = 1) / 36864 (CG = 2)
-    static constexpr int STAGES = CG == 2 ? 5 : 4;
+    static constexpr int STAGES = CG == 2 ? 6 : 5;
     static constexpr int SMEM = STAGES * STAGE + 1024 + 256;
-    static constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (0u << 16) | ((OZ2_BN >> 3) << 17) |
+    static constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (0u << 16) | ((OZ_BN >> 3) << 17) |
                                       (((128 * CG) >> 4) << 24);
     static_assert(STAGE % 1024 == 0, "stage alignment");
 };
@@ -520,6 +255,9 @@ __device__ __forceinline__ void mbar_wait_wd(uint32_t bar, uint32_t parity) {
         if (spins > (1ull << 22)) __trap();
     }
 }
+// COLLECT: use of the A-operand (M side) collector buffer -- consecutive MMAs with the same M-side slice read it from shared
+// memory once: 0 = no reuse, 1 = fill (first of a run), 2 = use (middle), 3 = last use.  Without it a 128 x 64 x 32 MMA
+// reads 6 KB of shared memory in 32 cycles, more than the 128 bytes per cycle an SM delivers.
 template <int CG, int COLLECT>
 __device__ __forceinline__ void tc_mma_i8_cg(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
 #define NSPT_OZ_MMA2(G, Q)                                                                         \
@@ -613,69 +351,53 @@ __device__ __forceinline__ bool elect_one() {
     return pred != 0;
 }
 template <int CG, int T0, int S0, bool FIRSTK>
-__device__ __forceinline__ void oz2_issue_pairs(uint32_t tmem, uint64_t dm0, uint64_t dn0, bool elected) {
+__device__ __forceinline__ void oz_issue_pairs(uint32_t tmem, uint64_t dm0, uint64_t dn0, bool elected) {
     constexpr int LAST = OZ_S - 1 - T0;
     constexpr int COLLECT = (LAST == 0) ? 0 : (S0 == 0 ? 1 : (S0 == LAST ? 3 : 2));
     // descriptors differ from the stage's first ones by a constant in the 14-bit start-address field (no carry: < 256 KB)
     const uint64_t dm = dm0 + (uint64_t)((T0 * OZ_M_SLICE) >> 4);
-    const uint64_t dn = dn0 + (uint64_t)(((S0 >> 2) * Oz2<CG>::N_HALF + (S0 & 3) * 32) >> 4);
-    const uint32_t d = tmem + (uint32_t)((S0 + T0) * OZ2_BN);
-    if (elected) tc_mma_i8_cg<CG, COLLECT>(d, dm, dn, Oz2<CG>::IDESC, (!FIRSTK || T0 != 0) ? 1u : 0u);
+    const uint64_t dn = dn0 + (uint64_t)(((S0 >> 2) * OzCfg<CG>::N_HALF + (S0 & 3) * 32) >> 4);
+    const uint32_t d = tmem + (uint32_t)((S0 + T0) * OZ_BN);
+    if (elected) tc_mma_i8_cg<CG, COLLECT>(d, dm, dn, OzCfg<CG>::IDESC, (!FIRSTK || T0 != 0) ? 1u : 0u);
     if constexpr (S0 < LAST)
-        oz2_issue_pairs<CG, T0, S0 + 1, FIRSTK>(tmem, dm0, dn0, elected);
+        oz_issue_pairs<CG, T0, S0 + 1, FIRSTK>(tmem, dm0, dn0, elected);
     else if constexpr (T0 + 1 < OZ_S)
-        oz2_issue_pairs<CG, T0 + 1, 0, FIRSTK>(tmem, dm0, dn0, elected);
+        oz_issue_pairs<CG, T0 + 1, 0, FIRSTK>(tmem, dm0, dn0, elected);
 }
 
 // exact conversion of the weighted sum of the seven accumulators of one output element:
 //   h = sum_d a_d 2^(-8 d) = hi 2^-24 + lo 2^-48,  hi = a0 2^24 + a1 2^16 + a2 2^8 + a3,  lo = a4 2^16 + a5 2^8 + a6
 // (|a_d| < 2^26, so |hi| < 2^51 and |lo| < 2^43: both convert exactly with the 2^52 + 2^51 trick); returns h * 2^24
-__device__ __forceinline__ long long mad_wide(int a, int b, long long c) {
-    long long r;
-    asm("mad.wide.s32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(c));
-    return r;
-}
-// multipliers 2^24, 2^16, 2^8, 1 in registers the optimizer cannot see through: with literal powers of two ptxas rewrites every
-// 64-bit multiply-add as shifts and carry chains (about 20 instructions per output element instead of 7 IMAD.WIDE)
-struct OzMul {
-    int m24, m16, m8, m1;
-};
-__device__ __forceinline__ OzMul oz_multipliers() {
-    OzMul m;
-    asm volatile("mov.b32 %0, 0x1000000;" : "=r"(m.m24));
-    asm volatile("mov.b32 %0, 0x10000;" : "=r"(m.m16));
-    asm volatile("mov.b32 %0, 0x100;" : "=r"(m.m8));
-    asm volatile("mov.b32 %0, 0x1;" : "=r"(m.m1));
-    return m;
-}
-__device__ __forceinline__ double oz2_combine(const OzMul& k, int a0, int a1, int a2, int a3, int a4, int a5, int a6) {
-    // the 2^52 + 2^51 bias rides along as the addend of the first multiply-add: the chains produce the bit patterns of
-    // 2^52 + 2^51 + hi and 2^52 + 2^51 + lo directly (one IMAD.WIDE per accumulator)
-    constexpr long long BIAS = 0x4338000000000000ll;
-    const long long hi = mad_wide(a0, k.m24, mad_wide(a1, k.m16, mad_wide(a2, k.m8, mad_wide(a3, k.m1, BIAS))));
-    const long long lo = mad_wide(a4, k.m16, mad_wide(a5, k.m8, mad_wide(a6, k.m1, BIAS)));
-    const double dhi = __longlong_as_double(hi) - 6755399441055744.0;
-    const double dlo = __longlong_as_double(lo) - 6755399441055744.0;
-    return fma(dlo, 5.9604644775390625e-08, dhi);   // 2^-24
+// h = sum_d a_d 2^(-8 d) from the seven INT32 accumulators of one output element: every a_d converts exactly through the
+// 2^52 + 2^31 bit trick (one LOP3 and one DADD, no I2F), then Horner in 2^-8 -- 7 LOP3, 7 DADD, 6 DFMA.  (The all-integer
+// alternative, two 64-bit multiply-add chains, compiles to about 40 instructions per element on sm_100a: ptxas expands every
+// mad.wide.s32 with a 64-bit addend into IMAD.HI + IMAD + IADD3 + IADD3.X.)  Returns h * 2^24 for the common scale below.
+__device__ __forceinline__ double oz_combine(int a0, int a1, int a2, int a3, int a4, int a5, int a6) {
+    double h = oz_i2d(a6);
+    h = fma(h, 0.00390625, oz_i2d(a5));
+    h = fma(h, 0.00390625, oz_i2d(a4));
+    h = fma(h, 0.00390625, oz_i2d(a3));
+    h = fma(h, 0.00390625, oz_i2d(a2));
+    h = fma(h, 0.00390625, oz_i2d(a1));
+    h = fma(h, 0.00390625, oz_i2d(a0));
+    return h;
 }
 
-struct Oz2Params {
+struct OzParams {
     double2* C;
     const int* expA;
     const int* expB;
-    unsigned long long* dbg;   // optional per-CTA clock samples (diagnostics), may be null
     size_t NN;
     int N;
     int tiles_i, tiles_j;      // tiles per mode: rows in steps of 64, columns in steps of 128 * CG
     int total_tiles;
     int nkc;
-    int flags;                 // diagnostics: 1 = no MMAs, 2 = no accumulator drain / stores, 4 = no TMA loads
 };
 
 template <int CG>
-__global__ void __launch_bounds__(OZ2_THREADS, 1)
-zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_constant__ CUtensorMap mapN, const Oz2Params P) {
-    using K = Oz2<CG>;
+__global__ void __launch_bounds__(OZ_THREADS, 1)
+zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_constant__ CUtensorMap mapN, const OzParams P) {
+    using K = OzCfg<CG>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_full = base + K::STAGES * K::STAGE;
@@ -708,12 +430,6 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
     const uint32_t tmem = *tmem_slot_gen;
     pdl_wait();
     pdl_trigger();
-    if (P.dbg && blockIdx.x == 0 && threadIdx.x == 0) {
-        unsigned long long gt;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
-        P.dbg[200] = gt;
-        P.dbg[201] = clock64();
-    }
     // barriers of the leader CTA, as shared::cluster addresses (identity for CG = 1)
     const uint32_t lead_full = CG == 2 ? mapa_rank(bar_full, 0) : bar_full;
     const uint32_t lead_acc_empty = CG == 2 ? mapa_rank(bar_acc_empty, 0) : bar_acc_empty;
@@ -726,18 +442,13 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                 int it = 0;
                 for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
                     const int mode = tile / tiles_per_mode, rem = tile % tiles_per_mode;
-                    const int i0 = (rem / P.tiles_j) * OZ2_BN + (int)rank * K::N_ROWS;
+                    const int i0 = (rem / P.tiles_j) * OZ_BN + (int)rank * K::N_ROWS;
                     const int j0 = (rem % P.tiles_j) * (OZ_BM * CG) + (int)rank * OZ_BM;
                     for (int plane = 0; plane < OZ_PLANES; ++plane) {
                         const int pidx = mode * OZ_PLANES + plane;
                         for (int kc = 0; kc < nkc; ++kc, ++it) {
                             const int slot = it % K::STAGES;
-                            if (P.flags & 8) continue;
                             mbar_wait_wd(bar_empty + 8 * slot, ((it / K::STAGES) & 1) ^ 1);
-                            if (P.flags & 4) {
-                                if (rank == 0) mbar_arrive(bar_full + 8 * slot);
-                                continue;
-                            }
                             if (rank == 0) mbar_expect_tx(bar_full + 8 * slot, K::STAGE * CG);
                             const uint32_t st = base + slot * K::STAGE;
                             tma_load_4d_cg<CG>(st, &mapM, lead_full + 8 * slot, j0, kc * OZ_KC, 0, pidx);
@@ -753,28 +464,23 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                 int it = 0, acc_it = 0;
                 for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
                     for (int plane = 0; plane < OZ_PLANES; ++plane, ++acc_it) {
-                        if (P.dbg && blockIdx.x == 0 && acc_it < 8 && elected) P.dbg[acc_it * 16 + 0] = clock64();
                         if (acc_it > 0) mbar_wait_wd(bar_acc_empty, (acc_it - 1) & 1);
                         tc_fence_after();
-                        if (P.dbg && blockIdx.x == 0 && acc_it < 8 && elected) P.dbg[acc_it * 16 + 1] = clock64();
                         for (int kc = 0; kc < nkc; ++kc, ++it) {
                             const int slot = it % K::STAGES;
-                            if (!(P.flags & 8)) mbar_wait_wd(bar_full + 8 * slot, (it / K::STAGES) & 1);
+                            mbar_wait_wd(bar_full + 8 * slot, (it / K::STAGES) & 1);
                             tc_fence_after();
-                            if (P.dbg && blockIdx.x == 0 && acc_it < 8 && elected && kc < 8) P.dbg[acc_it * 16 + 4 + kc] = clock64();
                             const uint32_t sm = base + slot * K::STAGE;
                             const uint64_t dm0 = oz_desc(sm, 4096, 1024), dn0 = oz_desc(sm + OZ_M_STAGE, 16, 1024);
-                            if (P.flags & 1) {
-                            } else if (kc == 0)
-                                oz2_issue_pairs<CG, 0, 0, true>(tmem, dm0, dn0, elected);
+                            if (kc == 0)
+                                oz_issue_pairs<CG, 0, 0, true>(tmem, dm0, dn0, elected);
                             else
-                                oz2_issue_pairs<CG, 0, 0, false>(tmem, dm0, dn0, elected);
-                            if (elected && !(P.flags & 8)) tc_commit_cg<CG>(bar_empty + 8 * slot);
-                            if (!(P.flags & 16)) __syncwarp();
+                                oz_issue_pairs<CG, 0, 0, false>(tmem, dm0, dn0, elected);
+                            if (elected) tc_commit_cg<CG>(bar_empty + 8 * slot);   // the stage may be refilled once these MMAs have read it
+                            __syncwarp();
                         }
                         if (elected) tc_commit_cg<CG>(bar_acc_full);
                         __syncwarp();
-                        if (P.dbg && blockIdx.x == 0 && acc_it < 8 && elected) P.dbg[acc_it * 16 + 2] = clock64();
                     }
                 }
             }
@@ -782,46 +488,43 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
         // ------------------------------------------------------------ epilogue: 8 warps; warp w reads TMEM lanes 32 (w % 4) ..
+        // lane of the accumulator = output column j, column of the accumulator = output row i
         const int we = warp - 4, quarter = we & 3, half = we >> 2;
-        const OzMul mul = oz_multipliers();
         int acc_it = 0;
         for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
             const int mode = tile / tiles_per_mode, rem = tile % tiles_per_mode;
-            const int row0 = (rem / P.tiles_j) * OZ2_BN + 32 * half;
+            const int row0 = (rem / P.tiles_j) * OZ_BN + 32 * half;
             const int col = (rem % P.tiles_j) * (OZ_BM * CG) + (int)rank * OZ_BM + 32 * quarter + lane;
             double re[32], im[32];
 #pragma unroll
             for (int plane = 0; plane < OZ_PLANES; ++plane, ++acc_it) {
                 mbar_wait_wd(bar_acc_full, acc_it & 1);
                 tc_fence_after();
-                if (P.dbg && blockIdx.x == 0 && acc_it < 8 && threadIdx.x == 128) P.dbg[acc_it * 16 + 12] = clock64();
-                if (!(P.flags & 2)) {
-                    // eight chunks of four columns; the loads of the next chunk are in flight while one is combined
-                    const uint32_t tbase = tmem + ((uint32_t)(32 * quarter) << 16) + (uint32_t)(32 * half);
-                    int a[2][OZ_S][4];
+                // eight chunks of four columns; the loads of the next chunk are in flight while one is combined
+                const uint32_t tbase = tmem + ((uint32_t)(32 * quarter) << 16) + (uint32_t)(32 * half);
+                int a[2][OZ_S][4];
 #pragma unroll
-                    for (int d = 0; d < OZ_S; ++d) tc_ld4(tbase + (uint32_t)(d * OZ2_BN), a[0][d]);
+                for (int d = 0; d < OZ_S; ++d) tc_ld4(tbase + (uint32_t)(d * OZ_BN), a[0][d]);
 #pragma unroll
-                    for (int cc = 0; cc < 8; ++cc) {
-                        tc_wait_ld();
-                        if (cc + 1 < 8) {
+                for (int cc = 0; cc < 8; ++cc) {
+                    tc_wait_ld();
+                    if (cc + 1 < 8) {
 #pragma unroll
-                            for (int d = 0; d < OZ_S; ++d) tc_ld4(tbase + (uint32_t)(d * OZ2_BN + 4 * (cc + 1)), a[(cc + 1) & 1][d]);
-                        }
+                        for (int d = 0; d < OZ_S; ++d) tc_ld4(tbase + (uint32_t)(d * OZ_BN + 4 * (cc + 1)), a[(cc + 1) & 1][d]);
+                    }
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const int (&b)[OZ_S][4] = a[cc & 1];
-                            const double h = oz2_combine(mul, b[0][j], b[1][j], b[2][j], b[3][j], b[4][j], b[5][j], b[6][j]);
-                            // 3M: Cr = P1 - P2, Ci = 4 P3 - P1 - P2 (the sum planes carry one more exponent bit each)
-                            if (plane == 0) {
-                                re[4 * cc + j] = h;
-                                im[4 * cc + j] = -h;
-                            } else if (plane == 1) {
-                                re[4 * cc + j] -= h;
-                                im[4 * cc + j] -= h;
-                            } else {
-                                im[4 * cc + j] = fma(4.0, h, im[4 * cc + j]);
-                            }
+                    for (int j = 0; j < 4; ++j) {
+                        const int (&b)[OZ_S][4] = a[cc & 1];
+                        const double h = oz_combine(b[0][j], b[1][j], b[2][j], b[3][j], b[4][j], b[5][j], b[6][j]);
+                        // 3M: Cr = P1 - P2, Ci = 4 P3 - P1 - P2 (the sum planes carry one more exponent bit each)
+                        if (plane == 0) {
+                            re[4 * cc + j] = h;
+                            im[4 * cc + j] = -h;
+                        } else if (plane == 1) {
+                            re[4 * cc + j] -= h;
+                            im[4 * cc + j] -= h;
+                        } else {
+                            im[4 * cc + j] = fma(4.0, h, im[4 * cc + j]);
                         }
                     }
                 }
@@ -830,11 +533,11 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                 if (lane == 0) {
                     if (CG == 2) mbar_arrive_cluster(lead_acc_empty); else mbar_arrive(bar_acc_empty);
                 }
-                if (P.dbg && blockIdx.x == 0 && acc_it < 8 && threadIdx.x == 128) P.dbg[acc_it * 16 + 13] = clock64();
             }
+            // scaling and stores overlap the MMAs of the next tile
             const int esum = P.expA[mode] + P.expB[mode];
-            const double sc = esum >= (1 << 20) ? __longlong_as_double(0x7ff8000000000000ll) : oz_pow2(esum - 12 - 24);
-            if (col < P.N && !(P.flags & 2)) {
+            const double sc = esum >= (1 << 20) ? __longlong_as_double(0x7ff8000000000000ll) : oz_pow2(esum - 12);
+            if (col < P.N) {
                 double2* c = P.C + (size_t)mode * P.NN + col;
 #pragma unroll
                 for (int j = 0; j < 32; ++j)   // the 32 lanes of a warp write 512 contiguous bytes of row row0 + j
@@ -845,12 +548,6 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
     __syncwarp();
     tc_fence_before();
     if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
-    if (P.dbg && blockIdx.x == 0 && threadIdx.x == 0) {
-        unsigned long long gt;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
-        P.dbg[202] = gt;
-        P.dbg[203] = clock64();
-    }
     if (warp == 2) tc_dealloc_cg<CG>(tmem, OZ_TMEM_COLS);
 }
 
@@ -894,17 +591,8 @@ OzWs oz_carve(const FreqLayout& f, int batch, void* ws) {
 
 }  // namespace
 
-void ozaki_slice_targets(const FreqLayout& f, int batch, void* ws, OzSliceDst* a, OzSliceDst* b) {
-    const int modes = batch * f.L;
-    const OzWs w = oz_carve(f, batch, ws);
-    a->slices = w.sA;
-    a->layout = OZ_QUAD;
-    a->maxbits = w.maxbits;
-    a->exps = w.exps;
-    b->slices = w.sB;
-    b->layout = OZ_ROWS;
-    b->maxbits = w.maxbits + modes;
-    b->exps = w.exps + modes;
+unsigned long long* ozaki_maxbits(const FreqLayout& f, int batch, void* ws, int z) {
+    return oz_carve(f, batch, ws).maxbits + (size_t)z * batch * f.L;
 }
 
 size_t ozaki_workspace_bytes(const FreqLayout& f, int batch) {
@@ -912,31 +600,12 @@ size_t ozaki_workspace_bytes(const FreqLayout& f, int batch) {
     return oz_bytes_quad(f.N, modes) + oz_bytes_rows(f.N, modes) + 2 * modes * 16 + 256;
 }
 
-// FP64 spectra A~, B~ (all batch * L modes) -> int8 slices, exponents (in `ws`, ozaki_workspace_bytes)
+// FP64 spectra A~, B~ -> int8 slices, with the per-mode maxima already in the workspace (written by the forward transform)
 cudaError_t launch_ozaki_slice(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st) {
     const int modes = batch * f.L;
     const int N = f.N;
     const OzWs w = oz_carve(f, batch, ws);
-    cudaError_t e;
-    if ((e = cudaMemsetAsync(w.maxbits, 0, sizeof(unsigned long long) * 2 * modes, st)) != cudaSuccess) return e;
-    const unsigned chunks = (unsigned)((f.NN + 256 * 8 - 1) / (256 * 8));
-    const unsigned gy = (unsigned)(modes < 65535 ? modes : 65535);
-    oz_absmax_kernel<<<dim3(chunks, gy), 256, 0, st>>>(reinterpret_cast<const double2*>(A), w.maxbits, f.NN, modes);
-    oz_absmax_kernel<<<dim3(chunks, gy), 256, 0, st>>>(reinterpret_cast<const double2*>(B), w.maxbits + modes, f.NN, modes);
-    const int pq = oz_pitch_quad(N), pr = oz_pitch_rows(N);
-    oz_slice_kernel<true><<<dim3((unsigned)((N * (pq / 256 * 8) + 255) / 256), gy), 256, 0, st>>>(
-        reinterpret_cast<const double2*>(A), w.sA, w.maxbits, w.exps, N, pq, modes);
-    oz_slice_kernel<false><<<dim3((unsigned)((N * ((N + 3) / 4) + 255) / 256), gy), 256, 0, st>>>(
-        reinterpret_cast<const double2*>(B), w.sB, w.maxbits + modes, w.exps + modes, N, pr, modes);
-    return cudaGetLastError();
-}
-
-// FP64 spectra A~, B~ -> int8 slices, with the per-mode maxima already in the workspace (written by the forward transform)
-cudaError_t launch_ozaki_slice2(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st) {
-    const int modes = batch * f.L;
-    const int N = f.N;
-    const OzWs w = oz_carve(f, batch, ws);
-    Slice2Params P;
+    SliceParams P;
     P.X[0] = reinterpret_cast<const double2*>(A);
     P.X[1] = reinterpret_cast<const double2*>(B);
     P.out[0] = w.sA;
@@ -960,7 +629,7 @@ cudaError_t launch_ozaki_slice2(const FreqLayout& f, int batch, const double* A,
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, oz_slice2_kernel, P);
+    return cudaLaunchKernelEx(&cfg, oz_slice_kernel, P);
 }
 
 // launch with programmatic stream serialization and (CG = 2) clusters of two CTAs
@@ -1002,84 +671,22 @@ void oz_maps(const FreqLayout& f, int modes, const OzWs& w, int n_rows, CUtensor
 }
 
 template <int CG>
-cudaError_t launch_oz2(const FreqLayout& f, int modes, const OzWs& w, double* C, unsigned long long* dbg, cudaStream_t st) {
-    using K = Oz2<CG>;
+cudaError_t launch_oz(const FreqLayout& f, int modes, const OzWs& w, double* C, cudaStream_t st) {
+    using K = OzCfg<CG>;
     const int N = f.N;
     cudaError_t e;
     static bool attr_done[NSPT_MAX_DEVICES] = {};
+    static int sms[NSPT_MAX_DEVICES] = {};
     const int dev = current_device();
     if (!attr_done[dev]) {
         e = cudaFuncSetAttribute(zgemm_modes_i8_kernel<CG>, cudaFuncAttributeMaxDynamicSharedMemorySize, K::SMEM);
         if (e != cudaSuccess) return e;
+        sms[dev] = 148;
+        cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev);
         attr_done[dev] = true;
     }
     CUtensorMap mapM, mapN;
     oz_maps(f, modes, w, K::N_ROWS, &mapM, &mapN, &e);
-    if (e != cudaSuccess) return e;
-    Oz2Params P;
-    P.C = reinterpret_cast<double2*>(C);
-    P.expA = w.exps;
-    P.expB = w.exps + modes;
-    P.dbg = dbg;
-    P.NN = f.NN;
-    P.N = N;
-    P.tiles_i = (N + OZ2_BN - 1) / OZ2_BN;
-    P.tiles_j = (N + OZ_BM * CG - 1) / (OZ_BM * CG);
-    P.total_tiles = modes * P.tiles_i * P.tiles_j;
-    P.nkc = (N + OZ_KC - 1) / OZ_KC;
-    {
-        const char* fl = getenv("NSPT_OZ_DBG");
-        P.flags = fl ? atoi(fl) : 0;
-    }
-    int sms = 148;
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    int clusters = sms / CG;
-    if (clusters > P.total_tiles) clusters = P.total_tiles;
-    return launch_pdl_cluster(zgemm_modes_i8_kernel<CG>, (unsigned)(clusters * CG), OZ2_THREADS, K::SMEM, CG, st, mapM, mapN, P);
-}
-
-// C~(p) = A~(p) B~(p) for all batch * L modes from the slices in `ws`.  kernel: 0 = first-generation kernel (one tile per CTA),
-// 1 = persistent single-CTA tiles, 2 = persistent CTA pairs (cta_group::2), -1 = automatic (pairs when N > 128).
-cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st, int kernel) {
-    const int modes = batch * f.L;
-    const int N = f.N;
-    const OzWs w = oz_carve(f, batch, const_cast<void*>(ws));
-    if (kernel < 0) kernel = N > 128 ? 2 : 1;
-    if (kernel == 1 || kernel == 2) {
-        static unsigned long long* dbg = nullptr;
-        const bool trace = getenv("NSPT_OZ_TRACE") != nullptr;
-        if (trace && !dbg) {
-            cudaMalloc(&dbg, 256 * 8);
-        }
-        if (trace) cudaMemsetAsync(dbg, 0, 256 * 8, st);
-        cudaError_t e = kernel == 2 ? launch_oz2<2>(f, modes, w, C, trace ? dbg : nullptr, st)
-                                    : launch_oz2<1>(f, modes, w, C, trace ? dbg : nullptr, st);
-        if (trace && e == cudaSuccess) {
-            unsigned long long h[256];
-            cudaStreamSynchronize(st);
-            cudaMemcpy(h, dbg, sizeof(h), cudaMemcpyDeviceToHost);
-            const unsigned long long t0 = h[0];
-            printf("CTA 0: %lld cycles in %lld ns = %.0f MHz\n", (long long)(h[203] - h[201]), (long long)(h[202] - h[200]),
-                   1e3 * (double)(h[203] - h[201]) / (double)(h[202] - h[200]));
-            for (int a = 0; a < 7; ++a) {
-                printf("acc_it %d: mma[wait_begin %lld wait_end %lld issued %lld] stages:", a, (long long)(h[a * 16] - t0),
-                       (long long)(h[a * 16 + 1] - t0), (long long)(h[a * 16 + 2] - t0));
-                for (int k = 0; k < 8; ++k) printf(" %lld", (long long)(h[a * 16 + 4 + k] - t0));
-                printf(" | epi[full_seen %lld drained %lld]\n", (long long)(h[a * 16 + 12] - t0), (long long)(h[a * 16 + 13] - t0));
-            }
-        }
-        return e;
-    }
-    cudaError_t e;
-    static bool attr_done[NSPT_MAX_DEVICES] = {};
-    const int dev = current_device();
-    if (!attr_done[dev]) {
-        e = cudaFuncSetAttribute(zgemm_modes_ozaki_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, OZ_SMEM);
-        if (e != cudaSuccess) return e;
-        attr_done[dev] = true;
-    }
-    CUtensorMap mapM, mapN;
-    oz_maps(f, modes, w, OZ_BN, &mapM, &mapN, &e);
     if (e != cudaSuccess) return e;
     OzParams P;
     P.C = reinterpret_cast<double2*>(C);
@@ -1088,10 +695,20 @@ cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, do
     P.NN = f.NN;
     P.N = N;
     P.tiles_i = (N + OZ_BN - 1) / OZ_BN;
-    P.tiles_j = (N + OZ_BM - 1) / OZ_BM;
+    P.tiles_j = (N + OZ_BM * CG - 1) / (OZ_BM * CG);
+    P.total_tiles = modes * P.tiles_i * P.tiles_j;
     P.nkc = (N + OZ_KC - 1) / OZ_KC;
-    const unsigned grid = (unsigned)(modes * P.tiles_i * P.tiles_j);
-    return launch_pdl(zgemm_modes_ozaki_kernel, grid, OZ_THREADS, OZ_SMEM, st, mapM, mapN, P);
+    int clusters = sms[dev] / CG;
+    if (clusters > P.total_tiles) clusters = P.total_tiles;
+    return launch_pdl_cluster(zgemm_modes_i8_kernel<CG>, (unsigned)(clusters * CG), OZ_THREADS, K::SMEM, CG, st, mapM, mapN, P);
+}
+
+// C~(p) = A~(p) B~(p) for all batch * L modes from the slices in `ws`; pairs = true runs the tiles on CTA pairs
+// (tcgen05.mma.cta_group::2)
+cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st, bool pairs) {
+    const int modes = batch * f.L;
+    const OzWs w = oz_carve(f, batch, const_cast<void*>(ws));
+    return pairs ? launch_oz<2>(f, modes, w, C, st) : launch_oz<1>(f, modes, w, C, st);
 }
 
 }  // namespace nspt

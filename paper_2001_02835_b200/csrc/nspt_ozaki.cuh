@@ -1,5 +1,5 @@
-// nspt_ozaki.cuh -- number format of the INT8-sliced mode-wise product (nspt_ozaki.cu) shared with the transforms that
-// write the slices directly (nspt_fft.cu).  See nspt_ozaki.cu for the derivation.
+// nspt_ozaki.cuh -- number format of the INT8-sliced mode-wise product (nspt_ozaki.cu); the transforms (nspt_fft.cu) use
+// oz_abs_hi to record the per-mode maxima the format is relative to.  See nspt_ozaki.cu for the derivation.
 #pragma once
 #include <cstdint>
 
@@ -35,31 +35,8 @@ __device__ __forceinline__ double oz_pow2(int k) {   // 2^k, k in [-1022, 1023]
     k = k < -1022 ? -1022 : (k > 1023 ? 1023 : k);
     return __longlong_as_double((long long)(k + 1023) << 52);
 }
-// the seven digits of v = rint(x * scale), |v| <= 2^54, packed in bytes 0..6 of the result: byte j holds the balanced digit
-// of weight 256^j (two's-complement int8), byte 6 the leading digit in [-64, 64]
-__device__ __forceinline__ unsigned long long oz_digits(double x, double scale) {
-    const long long v = __double2ll_rn(x * scale);
-    const unsigned long long u = (unsigned long long)v + 0x0000808080808080ull;   // + 128 at digits 0..5
-    return u ^ 0x0000808080808080ull;                                              // digit - 128 as int8
-}
-// Digits of v = rint(x * scale), |v| <= 2^54, without a 64-bit float-to-int conversion: v = H 2^32 + l with
-// H = rint(x scale 2^-32) and l = rint(x scale - H 2^32) (|l| <= 2^31), both read off the mantissa of a sum with
-// M = 2^52 + 2^51.  Returns the balanced base-256 digits as bytes: lo = digits 0..3, hi = digits 4..6 (byte 3 of hi is junk).
-__device__ __forceinline__ void oz_digits2(double x, double scale, unsigned int& lo, unsigned int& hi) {
-    constexpr double M = 6755399441055744.0;
-    const double xs = x * scale;
-    const double t1 = fma(xs, 2.3283064365386963e-10, M);           // 2^-32
-    const double hf = t1 - M;                                          // H as a double (exact)
-    const double l = fma(hf, -4294967296.0, xs);                       // exact: the low part of the mantissa of xs
-    const double t2 = l + M;
-    // u = v + 0x0000808080808080 = bits(t2) - bits(M) + 0x0000808080808080 + (H << 32)
-    constexpr unsigned long long K = 0x0000808080808080ull - 0x4338000000000000ull;
-    const unsigned long long u = (unsigned long long)__double_as_longlong(t2) + K +
-                                 ((unsigned long long)(unsigned int)__double2loint(t1) << 32);
-    lo = (unsigned int)u ^ 0x80808080u;
-    hi = (unsigned int)(u >> 32) ^ 0x00008080u;
-}
-// v = rint(x * scale) itself (|v| <= 2^54), same construction
+// v = rint(x * scale), |v| <= 2^54, without a 64-bit float-to-int conversion: v = H 2^32 + l with H = rint(x scale 2^-32)
+// and l = rint(x scale - H 2^32) (|l| <= 2^31), both read off the mantissa of a sum with M = 2^52 + 2^51
 __device__ __forceinline__ long long oz_fixed(double x, double scale) {
     constexpr double M = 6755399441055744.0;
     const double xs = x * scale;
@@ -93,22 +70,5 @@ __device__ __forceinline__ unsigned int oz_abs_hi(double2 v) {
     return a > b ? a : b;
 }
 #endif
-
-// Where the slices of one operand go (device pointers).  maxbits[mode] = bit pattern of max(|re|, |im|) over the mode (input
-// of the slicing pass), exps[mode] = the exponent derived from it (output, read by the product kernel).
-struct OzSliceDst {
-    int8_t* slices = nullptr;
-    int layout = OZ_QUAD;
-    unsigned long long* maxbits = nullptr;
-    int* exps = nullptr;
-};
-
-// Forward transforms (Steps 1-2) of one or two series straight into int8 slices (nspt_fft.cu): max-only pass, slicing pass.
-bool fft_slices_supported(int L);
-cudaError_t launch_fft_forward_slices(const FreqLayout& f, const PlanTables& t, int batch, const nspt_c128* src0,
-                                      const OzSliceDst& dst0, const nspt_c128* src1, const OzSliceDst& dst1, cudaStream_t st,
-                                      bool skip_order0 = false);
-// Carve the slice workspace of a product (ozaki_workspace_bytes): operand A in the QUAD layout, operand B in the ROWS layout.
-void ozaki_slice_targets(const FreqLayout& f, int batch, void* ws, OzSliceDst* a, OzSliceDst* b);
 
 }  // namespace nspt

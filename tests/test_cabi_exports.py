@@ -68,7 +68,7 @@ def test_argument_validation_without_a_gpu(lib):
     assert lib.nspt_force(None, None, 1.0, 4, 3) == -1
     assert lib.nspt_workspace_bytes(225, 31, 5, 2, ctypes.byref(out)) == 0 and out.value == 5 * 12 * 64 * 225 * 225 * 16 + 256   # Paterson-Stockmeyer: 6 powers + 6 block polynomials, + pad
     assert lib.nspt_set_order_scale(ctypes.c_double(-1.0)) == -1
-    assert lib.nspt_set_gemm_variant(9) == -1 and lib.nspt_set_gemm_variant(1) == 0
+    assert lib.nspt_set_gemm_variant(9) == -1 and lib.nspt_set_gemm_variant(-2) == -1 and lib.nspt_set_gemm_variant(1) == 0
     assert b"invalid" in lib.nspt_strerror(-1)
     assert lib.nspt_version() >= 100
 

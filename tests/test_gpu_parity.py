@@ -118,32 +118,36 @@ def test_reference_variant_agrees_with_tensor_core_variant(nspt):
     assert e0 < 1e-13 and e1 < 1e-13
 
 
-# ----------------------------------------------------------------------------- gemm variant 2: INT8 tensor cores (Ozaki)
+# ----------------------------------------------------------------------------- INT8 tensor cores (Ozaki slicing)
+# The fixture pins the suite to gemm variant 1 (FP64 tensor pipe everywhere); the tests below select the INT8 path explicitly
+# (2 = one CTA per tile, 4 = CTA pairs) or leave the choice to the library (-1, the default a user gets).
 
-@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (3, 2), (9, 7), (31, 4), (50, 12), (64, 15), (65, 3), (100, 31), (129, 3), (225, 7),
-                                      (33, 63)])
-def test_int8_sliced_product_matches_oracle(nspt, N, Ntrunc):
+@pytest.mark.parametrize("variant", [2, 4])
+@pytest.mark.parametrize("N,Ntrunc", [(1, 0), (3, 2), (9, 7), (9, 8), (31, 12), (50, 12), (64, 15), (65, 8), (100, 31), (129, 9), (225, 7),
+                                      (257, 8), (33, 63)])
+def test_int8_sliced_product_matches_oracle(nspt, N, Ntrunc, variant):
     # the mode-wise product on tcgen05.mma.kind::i8 with exact INT32 accumulation of seven int8 slices
-    # per operand plane; same tolerance as the FP64 tensor-pipe kernel
+    # per operand plane; same tolerance as the FP64 tensor-pipe kernel.  (L < 16 has no INT8 path and runs on the FP64 pipe.)
     from paper_2001_02835_b200 import workloads as wl
     rng = np.random.default_rng([3, N, Ntrunc])
     A = wl.gaussian_series(N, Ntrunc, rng)
     B = wl.gaussian_series(N, Ntrunc, rng)
-    nspt.nspt_set_gemm_variant(2)
+    nspt.nspt_set_gemm_variant(variant)
     try:
         check_product(nspt, A, B)
     finally:
         nspt.nspt_set_gemm_variant(1)
 
 
-def test_int8_sliced_product_integer_bit_exact(nspt):
+@pytest.mark.parametrize("variant", [2, 4])
+def test_int8_sliced_product_integer_bit_exact(nspt, variant):
     import oracle
     from paper_2001_02835_b200 import workloads as wl
     rng = np.random.default_rng([4, 70, 7])
-    A = wl.integer_series(70, 7, rng)
-    B = wl.integer_series(70, 7, rng)
+    A = wl.integer_series(70, 8, rng)
+    B = wl.integer_series(70, 8, rng)
     ref = oracle.series_mul(A, B)
-    nspt.nspt_set_gemm_variant(2)
+    nspt.nspt_set_gemm_variant(variant)
     try:
         got = gpu_mul(nspt, A, B)
     finally:
@@ -151,9 +155,68 @@ def test_int8_sliced_product_integer_bit_exact(nspt):
     assert np.array_equal(np.round(got.real), ref.real) and np.array_equal(np.round(got.imag), ref.imag)
 
 
-def test_int8_sliced_product_at_config2(nspt):
+def test_int8_sliced_product_zero_and_tiny_modes(nspt):
+    # a zero operand (all maxima zero) and an operand scaled by 2^-600 (exponents far from 1) go through the slicing unharmed
+    import oracle
     from paper_2001_02835_b200 import workloads as wl
-    A, B = wl.config_product(225, 31, seed=2)
+    rng = np.random.default_rng(77)
+    A = wl.gaussian_series(40, 9, rng)
+    B = wl.gaussian_series(40, 9, rng)
+    nspt.nspt_set_gemm_variant(2)
+    try:
+        assert np.array_equal(gpu_mul(nspt, np.zeros_like(A), B), np.zeros_like(A))
+        tiny = 2.0 ** -600
+        got = gpu_mul(nspt, A * tiny, B)
+        err = oracle.per_order_error(got / tiny, oracle.series_mul(A, B), oracle.product_bound(A, B))
+        assert err.max() <= TOL
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+
+
+@pytest.mark.parametrize("Ntrunc,seed", [(31, 2), (63, 3)])
+def test_automatic_choice_at_configs_2_and_3(nspt, Ntrunc, seed):
+    # BASELINE.json configs[1] and [2] through the library's default (automatic) kernel choice -- the INT8 tensor-core path at
+    # this size -- full matrices against the oracle at the north-star tolerance; the measured error stays below 1e-12
+    from paper_2001_02835_b200 import workloads as wl
+    A, B = wl.config_product(225, Ntrunc, seed=seed)
+    nspt.nspt_set_gemm_variant(-1)
+    try:
+        nspt.nspt_profile(True)
+        nspt.nspt_profile_read("int8_slicing")
+        err = check_product(nspt, A, B)
+        _, launches = nspt.nspt_profile_read("int8_slicing")
+        nspt.nspt_profile(False)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+    assert launches == 1, "the automatic choice at N = 225 is the INT8 path"
+    assert err <= 1e-12
+
+
+def test_automatic_choice_batched_at_n225(nspt):
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    batch, N, Ntrunc = 3, 225, 31
+    rng = np.random.default_rng(91)
+    A = np.stack([wl.unitary_series(N, Ntrunc, rng) for _ in range(batch)])
+    B = np.stack([wl.unitary_series(N, Ntrunc, rng) for _ in range(batch)])
+    nspt.nspt_set_gemm_variant(-1)
+    try:
+        C = nspt.nspt_series_mul_batched(to_dev(A), to_dev(B))
+        torch.cuda.synchronize()
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+    got = C.cpu().numpy()
+    for b in range(batch):
+        err = oracle.per_order_error(got[b], oracle.series_mul(A[b], B[b]), oracle.product_bound(A[b], B[b]))
+        assert err.max() <= TOL, (b, err.max())
+
+
+def test_int8_sliced_product_at_ntrunc_127_forced(nspt):
+    # N_trunc = 127 is outside the automatic range (the error of the seven-slice format is 2e-12 of the bound there, a factor
+    # of five below the tolerance); forced, it still has to meet the tolerance on the sweep's series
+    from paper_2001_02835_b200 import workloads as wl
+    A, B = wl.config_product(100, 127, seed=[5, 100, 127])
     nspt.nspt_set_gemm_variant(2)
     try:
         check_product(nspt, A, B)
