@@ -406,7 +406,7 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
         // Step 3 (eq. 2.8): exact integer products on the INT8 tensor cores, recombined in FP64
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_GEMM));
-        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, Ct, g.stream, g.gemm_variant == 4));
+        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, At, Bt, Ct, g.stream, g.gemm_variant == 4));
         NSPT_TRY(tm.end());
     } else {
         // Steps 1-2 (eqs. 2.6-2.7): zero-padded forward transforms of A and B, one launch

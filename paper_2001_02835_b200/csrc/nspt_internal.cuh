@@ -132,6 +132,7 @@ size_t ozaki_workspace_bytes(const FreqLayout& f, int batch);
 // where the forward transform records max(|re|, |im|) of every mode of operand z (0 = A, 1 = B): batch * L entries each
 unsigned long long* ozaki_maxbits(const FreqLayout& f, int batch, void* ws, int z);
 cudaError_t launch_ozaki_slice(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st);
-cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st, bool pairs = false);
+cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, const double* A, const double* B, double* C,
+                              cudaStream_t st, bool pairs = false);
 
 }  // namespace nspt

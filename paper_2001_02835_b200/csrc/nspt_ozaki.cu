@@ -214,7 +214,7 @@ struct OzCfg {
     static constexpr int N_HALF = N_ROWS * 128;              // slices 4h..4h+3 of a stage
     static constexpr int N_STAGE = 2 * N_HALF;
     static constexpr int STAGE = OZ_M_STAGE + N_STAGE;       // 45056 (CG = 1) / 36864 (CG = 2)
-    static constexpr int STAGES = CG == 2 ? 6 : 5;
+    static constexpr int STAGES = CG == 2 ? 5 : 4;
     static constexpr int SMEM = STAGES * STAGE + 1024 + 256;
     static constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (0u << 16) | ((OZ_BN >> 3) << 17) |
                                       (((128 * CG) >> 4) << 24);
@@ -385,14 +385,21 @@ __device__ __forceinline__ double oz_combine(int a0, int a1, int a2, int a3, int
 
 struct OzParams {
     double2* C;
+    const double2* At;         // FP64 spectra, read for the last `tail` columns of A~ / rows of B~ only
+    const double2* Bt;
     const int* expA;
     const int* expB;
     size_t NN;
     int N;
     int tiles_i, tiles_j;      // tiles per mode: rows in steps of 64, columns in steps of 128 * CG
     int total_tiles;
-    int nkc;
+    int nkc;                   // K-chunks of 32 that run on the tensor core
+    int tail;                  // k >= 32 nkc (0 .. OZ_TAIL_MAX of them) are added in FP64 by the epilogue
 };
+// Every odd-L TEK size has N = 1 mod 8, and N = 225, 289 are 1 mod 32: a full K-chunk of 28 MMAs per plane would serve ONE
+// column of A~.  When N mod 32 <= OZ_TAIL_MAX those columns are left out of the integer products and the epilogue adds
+// their rank-1 updates from the FP64 spectra (7 instead of 8 chunks at N = 225: 12 % fewer MMAs).
+constexpr int OZ_TAIL_MAX = 2;
 
 template <int CG>
 __global__ void __launch_bounds__(OZ_THREADS, 1)
@@ -496,6 +503,29 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
             const int row0 = (rem / P.tiles_j) * OZ_BN + 32 * half;
             const int col = (rem % P.tiles_j) * (OZ_BM * CG) + (int)rank * OZ_BM + 32 * quarter + lane;
             double re[32], im[32];
+            const int esum = P.expA[mode] + P.expB[mode];
+            const double sc = esum >= (1 << 20) ? __longlong_as_double(0x7ff8000000000000ll) : oz_pow2(esum - 12);
+            // The tail of K (k >= 32 nkc) in FP64, while the MMAs of the first plane run: lane l fetches A~[row0 + l][k] and its
+            // own column of B~[k][.]; the running sums start from the tail product in units of the common scale (a power of two)
+#pragma unroll
+            for (int j = 0; j < 32; ++j) re[j] = im[j] = 0.0;
+            if (P.tail) {
+                const double isc = oz_pow2(12 - esum);
+                for (int t = 0; t < P.tail; ++t) {
+                    const int k = OZ_KC * nkc + t;
+                    double2 at = make_double2(0.0, 0.0), bt = make_double2(0.0, 0.0);
+                    if (row0 + lane < P.N) at = __ldg(P.At + (size_t)mode * P.NN + (size_t)(row0 + lane) * P.N + k);
+                    if (col < P.N) bt = __ldg(P.Bt + (size_t)mode * P.NN + (size_t)k * P.N + col);
+                    bt.x *= isc;
+                    bt.y *= isc;
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        const double ax = __shfl_sync(0xffffffffu, at.x, j), ay = __shfl_sync(0xffffffffu, at.y, j);
+                        re[j] = fma(ax, bt.x, fma(-ay, bt.y, re[j]));
+                        im[j] = fma(ax, bt.y, fma(ay, bt.x, im[j]));
+                    }
+                }
+            }
 #pragma unroll
             for (int plane = 0; plane < OZ_PLANES; ++plane, ++acc_it) {
                 mbar_wait_wd(bar_acc_full, acc_it & 1);
@@ -518,8 +548,8 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                         const double h = oz_combine(b[0][j], b[1][j], b[2][j], b[3][j], b[4][j], b[5][j], b[6][j]);
                         // 3M: Cr = P1 - P2, Ci = 4 P3 - P1 - P2 (the sum planes carry one more exponent bit each)
                         if (plane == 0) {
-                            re[4 * cc + j] = h;
-                            im[4 * cc + j] = -h;
+                            re[4 * cc + j] += h;
+                            im[4 * cc + j] -= h;
                         } else if (plane == 1) {
                             re[4 * cc + j] -= h;
                             im[4 * cc + j] -= h;
@@ -535,8 +565,6 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                 }
             }
             // scaling and stores overlap the MMAs of the next tile
-            const int esum = P.expA[mode] + P.expB[mode];
-            const double sc = esum >= (1 << 20) ? __longlong_as_double(0x7ff8000000000000ll) : oz_pow2(esum - 12);
             if (col < P.N) {
                 double2* c = P.C + (size_t)mode * P.NN + col;
 #pragma unroll
@@ -671,7 +699,7 @@ void oz_maps(const FreqLayout& f, int modes, const OzWs& w, int n_rows, CUtensor
 }
 
 template <int CG>
-cudaError_t launch_oz(const FreqLayout& f, int modes, const OzWs& w, double* C, cudaStream_t st) {
+cudaError_t launch_oz(const FreqLayout& f, int modes, const OzWs& w, const double* At, const double* Bt, double* C, cudaStream_t st) {
     using K = OzCfg<CG>;
     const int N = f.N;
     cudaError_t e;
@@ -690,6 +718,8 @@ cudaError_t launch_oz(const FreqLayout& f, int modes, const OzWs& w, double* C, 
     if (e != cudaSuccess) return e;
     OzParams P;
     P.C = reinterpret_cast<double2*>(C);
+    P.At = reinterpret_cast<const double2*>(At);
+    P.Bt = reinterpret_cast<const double2*>(Bt);
     P.expA = w.exps;
     P.expB = w.exps + modes;
     P.NN = f.NN;
@@ -698,17 +728,23 @@ cudaError_t launch_oz(const FreqLayout& f, int modes, const OzWs& w, double* C, 
     P.tiles_j = (N + OZ_BM * CG - 1) / (OZ_BM * CG);
     P.total_tiles = modes * P.tiles_i * P.tiles_j;
     P.nkc = (N + OZ_KC - 1) / OZ_KC;
+    P.tail = 0;
+    if (At && Bt && N >= 2 * OZ_KC && N % OZ_KC != 0 && N % OZ_KC <= OZ_TAIL_MAX) {
+        P.nkc = N / OZ_KC;
+        P.tail = N % OZ_KC;
+    }
     int clusters = sms[dev] / CG;
     if (clusters > P.total_tiles) clusters = P.total_tiles;
     return launch_pdl_cluster(zgemm_modes_i8_kernel<CG>, (unsigned)(clusters * CG), OZ_THREADS, K::SMEM, CG, st, mapM, mapN, P);
 }
 
-// C~(p) = A~(p) B~(p) for all batch * L modes from the slices in `ws`; pairs = true runs the tiles on CTA pairs
-// (tcgen05.mma.cta_group::2)
-cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, double* C, cudaStream_t st, bool pairs) {
+// C~(p) = A~(p) B~(p) for all batch * L modes from the slices in `ws` (and, for the last N mod 32 <= 2 values of k, from the FP64
+// spectra A, B the slices were cut from); pairs = true runs the tiles on CTA pairs (tcgen05.mma.cta_group::2)
+cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, const double* A, const double* B, double* C,
+                              cudaStream_t st, bool pairs) {
     const int modes = batch * f.L;
     const OzWs w = oz_carve(f, batch, const_cast<void*>(ws));
-    return pairs ? launch_oz<2>(f, modes, w, C, st) : launch_oz<1>(f, modes, w, C, st);
+    return pairs ? launch_oz<2>(f, modes, w, A, B, C, st) : launch_oz<1>(f, modes, w, A, B, C, st);
 }
 
 }  // namespace nspt
