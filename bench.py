@@ -50,6 +50,7 @@ WORKLOADS = {
     "cfg2": ("product", 225, 31, 1, 2),
     "batched4": ("batched", 225, 31, 4, 2),
     "staple": ("staple", 225, 31, 1, 4),
+    "staple_split": ("staple", 225, 31, 1, 4),     # the paper's direction split: nspt_staple_dir per owned direction + all-gather
     "small": ("product", 9, 7, 1, 0),
     "sweep": ("sweep", 225, 31, 1, 5),
     "exp": ("exp", 225, 31, 1, 6),
@@ -62,6 +63,7 @@ WORKLOAD_DESC = {
     "cfg2": "single star-product A*B, N=225, N_trunc=31 (L=64), complex128 (BASELINE.json configs[1])",
     "batched4": "batch of 4 star-products, N=225, N_trunc=31 (the four P_mu*U_mu of a link update)",
     "staple": "full TEK staple S_mu, mu=1..4, N=225, N_trunc=31, k=4 twist (BASELINE.json configs[3]); 36 mode-wise products per step (literal eq. 2.3: 52)",
+    "staple_split": "full TEK staple S_mu, mu=1..4, N=225, N_trunc=31, k=4 twist (BASELINE.json configs[3]), directions split over the ranks (PAPER.md:140): 15 mode-wise products per owned direction, one all-gather of the four S_mu per step",
     "small": "single star-product A*B, N=9, N_trunc=7 (BASELINE.json configs[0])",
     "exp": "series exponential exp(X), X anti-Hermitian series, N=225, N_trunc=31 (link-update exponential; 10 mode-wise products, Paterson-Stockmeyer)",
     "exp4": "batch of 4 series exponentials (the four links of an update), N=225, N_trunc=31; 10 batched mode-wise products",
@@ -457,10 +459,22 @@ def run_cuda(args):
                 sets.append((U, S))
             z = inp["z"]
 
-            def step(i):
-                U, S = sets[i % R]
-                nspt.nspt_staple(U, z, S)
-            products_per_step = 36
+            if args.workload == "staple_split":
+                from paper_2001_02835_b200 import parallel
+                owned = parallel.owned_directions(rank, world if world in (1, 2, 4) else 1)
+
+                def step(i):
+                    U, S = sets[i % R]
+                    mine = [nspt.nspt_staple_dir(U, z, mu, S[mu]) for mu in owned]
+                    if world > 1:
+                        with torch.cuda.stream(stream):
+                            parallel.all_gather_series(mine, rank, world)
+                products_per_step = 15 * len(owned)
+            else:
+                def step(i):
+                    U, S = sets[i % R]
+                    nspt.nspt_staple(U, z, S)
+                products_per_step = 36
             units_name = "staples"
         else:
             per_set = 3 * series_bytes
@@ -510,6 +524,8 @@ def run_cuda(args):
     launches = nspt.nspt_launch_count() - launches0
     clocks = sampler.stop()
     units_per_step = 1 if kind == "staple" else (batch if kind == "exp" else products_per_step)
+    if args.workload == "staple_split":
+        units_per_step = 1.0 / world          # the ranks share ONE staple per step (strong scaling)
     value, ms_total = aggregate_throughput(K * units_per_step, ms_local, world, dev)
 
     # ---- timed region 2: the same K steps with the stage profiler on -> per-kernel durations
@@ -730,7 +746,7 @@ def run_cuda(args):
     line = {
         "metric": {"staple": "tek_staples_per_sec", "exp": "series_exponentials_per_sec"}.get(kind, METRIC),
         "value": value, "unit": f"{units_name}/s", "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "strong" if args.workload == "staple_split" else "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": desc, "N": N, "N_trunc": Ntrunc, "L": L, "batch": batch,
                    "parallelism": "replicas only (no data-path collective)" if world > 1 else "single GPU",

@@ -109,6 +109,15 @@ int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* c
                 int N, int Ntrunc);
 
 /*
+ * The staple of ONE direction mu (0..3), same definition and arguments: the unit of work of the paper's multi-GPU scheme
+ * ("we assign computational tasks, which are independent in the four-dimensional direction, on each GPU card";
+ * every * stays inside one card, the updated links are exchanged once per step).  S_mu: device pointer, must not alias any
+ * U[nu].  15 mode-wise products (nspt_staple shares intermediate products between directions: 36 for all four).
+ */
+int nspt_staple_dir(const nspt_c128* const U[4], const nspt_c128 z[16], int mu, nspt_c128* S_mu,
+                    int N, int Ntrunc);
+
+/*
  * E = exp(X) = sum_{m=0}^{Ntrunc} X^{*m} / m!, every power a chain of the star-product above, for a series
  * whose coefficient of g^0 vanishes; X^(0) is NOT read and is taken as zero (with X^(0) = 0 the power
  * X^{*m} starts at g^m, so the sum is finite and exact).  This is the exponential of the link update

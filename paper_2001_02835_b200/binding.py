@@ -24,7 +24,7 @@ STAGES = {"fft_forward": 0, "zgemm_modes": 1, "fft_inverse": 2, "fft_retruncate"
           "int8_slicing": 6}
 
 EXPORTS = [
-    "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_series_exp", "nspt_series_exp_batched", "nspt_force",
+    "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_staple_dir", "nspt_series_exp", "nspt_series_exp_batched", "nspt_force",
     "nspt_series_mul_host", "nspt_series_mul_batched_host", "nspt_staple_host",
     "nspt_set_stream", "nspt_set_order_scale", "nspt_workspace_bytes", "nspt_set_workspace",
     "nspt_set_gemm_variant", "nspt_set_conv_algorithm", "nspt_probe_fp64_peak", "nspt_profile", "nspt_profile_read", "nspt_launch_count",
@@ -48,6 +48,7 @@ _vp, _int, _dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
 _lib.nspt_series_mul.argtypes = [_vp, _vp, _vp, _int, _int]
 _lib.nspt_series_mul_batched.argtypes = [_vp, _vp, _vp, _int, _int, _int]
 _lib.nspt_staple.argtypes = [ctypes.POINTER(_vp), _vp, ctypes.POINTER(_vp), _int, _int]
+_lib.nspt_staple_dir.argtypes = [ctypes.POINTER(_vp), _vp, _int, _vp, _int, _int]
 _lib.nspt_series_exp.argtypes = [_vp, _vp, _int, _int]
 _lib.nspt_series_exp_batched.argtypes = [_vp, _vp, _int, _int, _int]
 _lib.nspt_force.argtypes = [_vp, _vp, _dbl, _int, _int]
@@ -181,6 +182,28 @@ def nspt_staple(U, z, S=None):
     Sp = (_vp * 4)(*[s.data_ptr() for s in S])
     _check(_lib.nspt_staple(Up, zz.ctypes.data, Sp, N, Ntrunc), "nspt_staple")
     return S
+
+
+def nspt_staple_dir(U, z, mu: int, S_mu=None):
+    """S_mu of eq. 2.3 for ONE direction (the per-GPU unit of the paper's direction split)."""
+    torch = _torch()
+    U = [_dev_series(u, "U") for u in U]
+    if len(U) != 4:
+        raise ValueError("four link series expected")
+    if not 0 <= int(mu) <= 3:
+        raise ValueError("mu must be 0..3")
+    _, Ntrunc, N = _shape(U[0], False)
+    for t in U[1:]:
+        _match(t, U[0], "U")
+    if S_mu is None:
+        S_mu = torch.empty_like(U[0])
+    _match(_dev_series(S_mu, "S_mu"), U[0], "S_mu")
+    if any(S_mu.data_ptr() == u.data_ptr() for u in U):
+        raise ValueError("S_mu must not alias a link series")
+    zz = _z_array(z)
+    Up = (_vp * 4)(*[u.data_ptr() for u in U])
+    _check(_lib.nspt_staple_dir(Up, zz.ctypes.data, int(mu), S_mu.data_ptr(), N, Ntrunc), "nspt_staple_dir")
+    return S_mu
 
 
 def nspt_series_exp(X, E=None):

@@ -632,6 +632,81 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     return NSPT_OK;
 }
 
+// The staple of ONE direction: the unit of work a GPU owns in the paper's four-GPU scheme ("we assign
+// computational tasks, which are independent in the four-dimensional direction, on each GPU card").  With W = U_mu U_nu^+,
+// Y = U_mu^+ U_nu, T = U_nu W (all *):
+//     S_mu = sum_{nu != mu} ( -z_{mu nu}^* W Y + z_{mu nu} (T U_mu^+)^+ ),
+// five mode-wise products per nu, 15 in all (the four-direction call shares W, Y, T between the two directions of a pair:
+// 36 for four directions).  Every contribution to S~_mu is its own launch, so the sum has a fixed order.
+int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu, nspt_c128* Smu, int N, int Ntrunc) {
+    NSPT_TRY(check_dims(N, Ntrunc, 1));
+    if (!U || !z || !Smu || mu < 0 || mu > 3 || !aligned16(Smu)) return NSPT_EINVAL;
+    for (int d = 0; d < 4; ++d)
+        if (!U[d] || !aligned16(U[d])) return NSPT_EINVAL;
+    NSPT_TRY(check_arch());
+    const FreqLayout f = make_layout(N, Ntrunc);
+    if (!fft_length_supported(f.L)) return NSPT_EINVAL;
+    PlanTables t;
+    NSPT_TRY(get_plan(f.L, f.n, g.order_scale, &t));
+    char* ws = nullptr;
+    NSPT_TRY(get_workspace(ws_bytes_for(f, 1, NSPT_OP_STAPLE), &ws));
+    const size_t sb = spectrum_bytes(f, 1);
+    auto spec = [&](int i) { return reinterpret_cast<double*>(ws + (size_t)i * sb); };
+    double* Ut[4] = {spec(0), spec(1), spec(2), spec(3)};
+    double* Ud[4] = {spec(4), spec(5), spec(6), spec(7)};
+    double* St = spec(8);
+    double *W[3], *Y[3], *T[3];
+    int nus[3], k = 0;
+    for (int nu = 0; nu < 4; ++nu)
+        if (nu != mu) {
+            nus[k] = nu;
+            W[k] = spec(9 + k);
+            Y[k] = spec(12 + k);
+            T[k] = spec(15 + k);
+            ++k;
+        }
+    NSPT_TRY(k_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1]));
+    NSPT_TRY(k_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3]));
+    NSPT_TRY(k_dagger(f, 4, Ut[0], Ud[0]));
+    {
+        GemmGroup gr[6];
+        for (int q = 0; q < 3; ++q) {
+            gr[q].A = Ut[mu];
+            gr[q].B = Ud[nus[q]];
+            gr[q].out.C = W[q];
+            gr[3 + q].A = Ud[mu];
+            gr[3 + q].B = Ut[nus[q]];
+            gr[3 + q].out.C = Y[q];
+        }
+        NSPT_TRY(k_gemm_groups(f, gr, 6));
+        NSPT_TRY(k_retrunc(f, t, 6, W[0], W[0]));   // W[0..2], Y[0..2] are contiguous
+    }
+    {
+        GemmGroup gr[3];
+        for (int q = 0; q < 3; ++q) {
+            gr[q].A = Ut[nus[q]];
+            gr[q].B = W[q];
+            gr[q].out.C = T[q];
+        }
+        NSPT_TRY(k_gemm_groups(f, gr, 3));
+        NSPT_TRY(k_retrunc(f, t, 3, T[0], T[0]));
+    }
+    for (int q = 0; q < 3; ++q) {
+        const Cplx zmn{z[4 * mu + nus[q]].re, z[4 * mu + nus[q]].im};
+        GemmOut r;   // S_mu -= z_{mu nu}^* W Y
+        r.C = St;
+        r.alpha = Cplx{-zmn.re, zmn.im};
+        r.accumulate = q > 0;
+        NSPT_TRY(k_gemm(f, 1, W[q], Y[q], r));
+        GemmOut p;   // S_mu += z_{mu nu} (T U_mu^+)^+ : conjugate-transposed accumulate into the mirrored mode
+        p.D = St;
+        p.beta = zmn;
+        p.accumulate_d = true;
+        NSPT_TRY(k_gemm(f, 1, T[q], Ud[mu], p));
+    }
+    return k_inverse(f, t, 1, St, Smu);
+}
+
 }  // namespace
 }  // namespace nspt
 
@@ -652,6 +727,11 @@ int nspt_series_mul_batched(const nspt_c128* A, const nspt_c128* B, nspt_c128* C
 int nspt_staple(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128* const S[4], int N, int Ntrunc) {
     NSPT_LOCK();
     return staple_device(U, z, S, N, Ntrunc);
+}
+
+int nspt_staple_dir(const nspt_c128* const U[4], const nspt_c128 z[16], int mu, nspt_c128* S_mu, int N, int Ntrunc) {
+    NSPT_LOCK();
+    return staple_dir_device(U, z, mu, S_mu, N, Ntrunc);
 }
 
 int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc) {

@@ -499,6 +499,30 @@ def test_staple_generic_links_and_z(nspt):
     check_staple(nspt, U, z)
 
 
+@pytest.mark.parametrize("N,Ntrunc", [(9, 7), (25, 5), (50, 12), (67, 3)])
+def test_staple_of_one_direction_matches_oracle(nspt, N, Ntrunc):
+    # nspt_staple_dir: the per-GPU unit of the paper's direction split, 15 products per
+    # direction, against the literal eq. 2.3 of the oracle and against the four-direction call
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([21, N, Ntrunc])
+    U = [wl.unitary_series(N, Ntrunc, rng) for _ in range(4)]
+    z = wl.twist_tensor(5, 2)
+    ref = oracle.staple(U, z)
+    bounds = oracle.staple_bound(U)
+    Ud = [to_dev(u) for u in U]
+    for mu in range(4):
+        S = nspt.nspt_staple_dir(Ud, z, mu)
+        torch.cuda.synchronize()
+        got = S.cpu().numpy()
+        assert oracle.per_order_error(got, ref[mu], bounds[mu]).max() <= TOL
+        scale = max(np.linalg.norm(ref[mu][k]) for k in range(Ntrunc + 1))
+        assert max(np.linalg.norm(got[k] - ref[mu][k]) for k in range(Ntrunc + 1)) <= STAPLE_REL * scale
+    with pytest.raises(ValueError):
+        nspt.nspt_staple_dir(Ud, z, 1, Ud[2])      # the output must not alias a link
+
+
 @pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("N,Ntrunc", [(1, 0), (1, 5), (3, 0), (57, 9), (8, 1)])
 def test_staple_edge_shapes_both_gemm_variants(nspt, N, Ntrunc, variant):
