@@ -200,9 +200,20 @@ bool use_int8(const FreqLayout& f) {
     return f.N >= 192 && f.L >= 32 && f.L <= 128;
 }
 
+// INT8 staple (staple_device): slice slots per layout and per-mode maxima tables (see the slot maps there)
+constexpr int STAPLE_NQ = 25, STAPLE_NR = 19, STAPLE_MAXBITS = 22;
+
+// per-mode maxima (one 64-bit pattern per mode) recorded by the transforms for the INT8 path
+size_t maxbits_bytes(int modes) { return align_up((size_t)modes * sizeof(unsigned long long), 256); }
+
 size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
-    if (op == NSPT_OP_SERIES_MUL && use_int8(f)) return 3 * spectrum_bytes(f, batch) + WS_PAD + ozaki_workspace_bytes(f, batch);
-    if (op == NSPT_OP_STAPLE) return 30 * spectrum_bytes(f, 1) + WS_PAD;
+    if (op == NSPT_OP_SERIES_MUL && use_int8(f))
+        return 3 * spectrum_bytes(f, batch) + WS_PAD + maxbits_bytes(2 * batch * f.L) + ozaki_store_bytes(f, batch * f.L, 1, 1);
+    if (op == NSPT_OP_STAPLE) {
+        size_t b = 30 * spectrum_bytes(f, 1) + WS_PAD;
+        if (use_int8(f)) b += maxbits_bytes(STAPLE_MAXBITS * f.L) + ozaki_store_bytes(f, f.L, STAPLE_NQ, STAPLE_NR);
+        return b;
+    }
     if (op == NSPT_OP_SERIES_EXP) {
         int s, r;
         exp_split(f.n - 1, &s, &r);
@@ -313,10 +324,23 @@ int k_inverse(const FreqLayout& f, const PlanTables& t, int batch, const double*
     NSPT_CUDA(launch_fft_inverse(f, t, batch, src, dst, g.stream));
     return tm.end();
 }
-int k_retrunc(const FreqLayout& f, const PlanTables& t, int batch, const double* src, double* dst) {
+int k_retrunc(const FreqLayout& f, const PlanTables& t, int batch, const double* src, double* dst,
+              unsigned long long* maxbits = nullptr) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_RETRUNC));
-    NSPT_CUDA(launch_fft_retruncate(f, t, batch, src, dst, g.stream));
+    NSPT_CUDA(launch_fft_retruncate(f, t, batch, src, dst, g.stream, maxbits));
+    return tm.end();
+}
+int k_slice(const FreqLayout& f, const OzStore& store, const OzSliceJob* jobs, int njobs) {
+    StageTimer tm;
+    NSPT_TRY(tm.begin(ST_SLICE));
+    NSPT_CUDA(launch_ozaki_slice(f, store, jobs, njobs, g.stream));
+    return tm.end();
+}
+int k_gemm_i8(const FreqLayout& f, const OzStore& store, const OzGemmGroup* groups, int ngroups) {
+    StageTimer tm;
+    NSPT_TRY(tm.begin(ST_GEMM));
+    NSPT_CUDA(launch_ozaki_gemm(f, store, groups, ngroups, g.stream, g.gemm_variant == 4));
     return tm.end();
 }
 int k_dagger(const FreqLayout& f, int batch, const double* src, double* dst) {
@@ -386,27 +410,43 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
     double* Bt = reinterpret_cast<double*>(ws + sb);
     double* Ct = reinterpret_cast<double*>(ws + 2 * sb);
     if (use_int8(f)) {
-        void* oz = ws + 3 * sb + WS_PAD;
-        unsigned long long* mbA = ozaki_maxbits(f, batch, oz, 0);
+        const int modes = batch * f.L;
+        unsigned long long* mbA = reinterpret_cast<unsigned long long*>(ws + 3 * sb + WS_PAD);
+        unsigned long long* mbB = mbA + modes;
+        const OzStore store = ozaki_store(f, modes, 1, 1, ws + 3 * sb + WS_PAD + maxbits_bytes(2 * modes));
         {
             // Steps 1-2 (eqs. 2.6-2.7); the transform also records max(|re|, |im|) of every mode of both spectra
             StageTimer tm;
             NSPT_TRY(tm.begin(ST_FWD));
-            NSPT_CUDA(cudaMemsetAsync(mbA, 0, sizeof(unsigned long long) * 2 * batch * f.L, g.stream));
-            NSPT_CUDA(launch_fft_forward(f, t, batch, A, At, B, Bt, g.stream, false, mbA, ozaki_maxbits(f, batch, oz, 1)));
+            NSPT_CUDA(cudaMemsetAsync(mbA, 0, sizeof(unsigned long long) * 2 * modes, g.stream));
+            NSPT_CUDA(launch_fft_forward(f, t, batch, A, At, B, Bt, g.stream, false, mbA, mbB));
             NSPT_TRY(tm.end());
         }
         {
-            // both spectra cut into seven int8 slices per plane, fixed point relative to the largest element of each mode
+            // both spectra cut into seven int8 slices per plane, fixed point relative to the largest element of each mode:
+            // A~ as a left factor (QUAD layout), B~ as a right factor (ROWS layout)
+            OzSliceJob jobs[2];
+            jobs[0].X = At;
+            jobs[0].maxbits = mbA;
+            jobs[0].quad_slot = 0;
+            jobs[1].X = Bt;
+            jobs[1].maxbits = mbB;
+            jobs[1].rows_slot = 0;
             StageTimer tm;
             NSPT_TRY(tm.begin(ST_SLICE));
-            NSPT_CUDA(launch_ozaki_slice(f, batch, At, Bt, oz, g.stream));
+            NSPT_CUDA(launch_ozaki_slice(f, store, jobs, 2, g.stream));
             NSPT_TRY(tm.end());
         }
         // Step 3 (eq. 2.8): exact integer products on the INT8 tensor cores, recombined in FP64
+        OzGemmGroup grp;
+        grp.quad_slot = 0;
+        grp.rows_slot = 0;
+        grp.A = At;
+        grp.B = Bt;
+        grp.out.C = Ct;
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_GEMM));
-        NSPT_CUDA(launch_ozaki_gemm(f, batch, oz, At, Bt, Ct, g.stream, g.gemm_variant == 4));
+        NSPT_CUDA(launch_ozaki_gemm(f, store, &grp, 1, g.stream, g.gemm_variant == 4));
         NSPT_TRY(tm.end());
     } else {
         // Steps 1-2 (eqs. 2.6-2.7): zero-padded forward transforms of A and B, one launch
@@ -566,31 +606,115 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     // Products that do not depend on one another share a launch (8 launches for the 36 products): a single
     // product at L = 64 is 3.6 waves of CTAs and loses a tenth of its time to the last, partly filled wave.
     // All four links are transformed before any output is written (S may alias U).
-    NSPT_TRY(k_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1]));
-    NSPT_TRY(k_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3]));
+    // The same launch plan runs on the FP64 tensor pipe or, from N = 192 (use_int8), on the INT8 tensor cores: there every
+    // spectrum is also cut into int8 slices -- in the QUAD layout where it is a left factor, in the ROWS layout where it is a
+    // right factor (one pass per wave of spectra, both layouts from one read) -- with the per-mode maxima the transforms record.
+    const bool i8 = use_int8(f);
+    const int L = f.L;
+    unsigned long long* mb = reinterpret_cast<unsigned long long*>(ws + 30 * sb + WS_PAD);   // [U 0..3][W 0..5][Y 0..5][T 0..5] x L
+    unsigned long long *mbU = mb, *mbW = mb + 4 * L, *mbY = mb + 10 * L, *mbT = mb + 16 * L;
+    OzStore store;
+    // slots.  QUAD (left factors): U~_mu -> mu, Ud_mu (mu < 3) -> 4 + mu, W_p -> 7 + p, Y_p -> 13 + p, T_p -> 19 + p;
+    //         ROWS (right factors): U~_mu (mu > 0) -> mu - 1, Ud_mu -> 3 + mu, W_p -> 7 + p, Y_p -> 13 + p
+    auto qU = [](int mu) { return mu; };
+    auto qUd = [](int mu) { return 4 + mu; };
+    auto rU = [](int mu) { return mu - 1; };
+    auto rUd = [](int mu) { return 3 + mu; };
+    if (i8) {
+        store = ozaki_store(f, L, STAPLE_NQ, STAPLE_NR, ws + 30 * sb + WS_PAD + maxbits_bytes(STAPLE_MAXBITS * L));
+        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * STAPLE_MAXBITS * L, g.stream));
+    }
+    auto gemm_groups = [&](const GemmGroup* gr, const int (*slots)[2], int n) -> int {
+        if (!i8) return k_gemm_groups(f, gr, n);
+        OzGemmGroup og[12];
+        for (int i = 0; i < n; ++i) {
+            og[i].quad_slot = slots[i][0];
+            og[i].rows_slot = slots[i][1];
+            og[i].A = gr[i].A;
+            og[i].B = gr[i].B;
+            og[i].out = gr[i].out;
+        }
+        return k_gemm_i8(f, store, og, n);
+    };
+    {
+        StageTimer tm;
+        NSPT_TRY(tm.begin(ST_FWD));
+        NSPT_CUDA(launch_fft_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1], g.stream, false, i8 ? mbU : nullptr, i8 ? mbU + L : nullptr));
+        NSPT_TRY(tm.end());
+        NSPT_TRY(tm.begin(ST_FWD));
+        NSPT_CUDA(launch_fft_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3], g.stream, false, i8 ? mbU + 2 * L : nullptr,
+                                     i8 ? mbU + 3 * L : nullptr));
+        NSPT_TRY(tm.end());
+    }
     NSPT_TRY(k_dagger(f, 4, Ut[0], Ud[0]));
+    if (i8) {
+        OzSliceJob jobs[8];
+        for (int mu = 0; mu < 4; ++mu) {
+            jobs[mu].X = Ut[mu];
+            jobs[mu].maxbits = mbU + mu * L;
+            jobs[mu].quad_slot = qU(mu);
+            jobs[mu].rows_slot = mu > 0 ? rU(mu) : -1;
+            jobs[4 + mu].X = Ud[mu];
+            jobs[4 + mu].maxbits = mbU + mu * L;   // |Ud(p)| = |U~((L - p) mod L)|
+            jobs[4 + mu].mirror = true;
+            jobs[4 + mu].quad_slot = mu < 3 ? qUd(mu) : -1;
+            jobs[4 + mu].rows_slot = rUd(mu);
+        }
+        NSPT_TRY(k_slice(f, store, jobs, 8));
+    }
     {   // W_p and Y_p for the six pairs: twelve products, one launch; then one re-truncation pass over all twelve
         GemmGroup gr[12];
+        int sl[12][2];
         for (int p = 0; p < 6; ++p) {
             gr[p].A = Ut[pmu[p]];
             gr[p].B = Ud[pnu[p]];
             gr[p].out.C = W[p];
+            sl[p][0] = qU(pmu[p]);
+            sl[p][1] = rUd(pnu[p]);
             gr[6 + p].A = Ud[pmu[p]];
             gr[6 + p].B = Ut[pnu[p]];
             gr[6 + p].out.C = Y[p];
+            sl[6 + p][0] = qUd(pmu[p]);
+            sl[6 + p][1] = rU(pnu[p]);
         }
-        NSPT_TRY(k_gemm_groups(f, gr, 12));
-        NSPT_TRY(k_retrunc(f, t, 12, W[0], W[0]));   // W[0..5], Y[0..5] are contiguous
+        NSPT_TRY(gemm_groups(gr, sl, 12));
+        NSPT_TRY(k_retrunc(f, t, 12, W[0], W[0], i8 ? mbW : nullptr));   // W[0..5], Y[0..5] are contiguous (and so are mbW, mbY)
+        if (i8) {
+            OzSliceJob jobs[12];
+            for (int p = 0; p < 6; ++p) {
+                jobs[p].X = W[p];
+                jobs[p].maxbits = mbW + p * L;
+                jobs[p].quad_slot = 7 + p;
+                jobs[p].rows_slot = 7 + p;
+                jobs[6 + p].X = Y[p];
+                jobs[6 + p].maxbits = mbY + p * L;
+                jobs[6 + p].quad_slot = 13 + p;
+                jobs[6 + p].rows_slot = 13 + p;
+            }
+            NSPT_TRY(k_slice(f, store, jobs, 12));
+        }
     }
     {   // T_p = U_nu W_p: six products, one launch, one re-truncation pass
         GemmGroup gr[6];
+        int sl[6][2];
         for (int p = 0; p < 6; ++p) {
             gr[p].A = Ut[pnu[p]];
             gr[p].B = W[p];
             gr[p].out.C = T[p];
+            sl[p][0] = qU(pnu[p]);
+            sl[p][1] = 7 + p;
         }
-        NSPT_TRY(k_gemm_groups(f, gr, 6));
-        NSPT_TRY(k_retrunc(f, t, 6, T[0], T[0]));
+        NSPT_TRY(gemm_groups(gr, sl, 6));
+        NSPT_TRY(k_retrunc(f, t, 6, T[0], T[0], i8 ? mbT : nullptr));
+        if (i8) {
+            OzSliceJob jobs[6];
+            for (int p = 0; p < 6; ++p) {
+                jobs[p].X = T[p];
+                jobs[p].maxbits = mbT + p * L;
+                jobs[p].quad_slot = 19 + p;
+            }
+            NSPT_TRY(k_slice(f, store, jobs, 6));
+        }
     }
     // Accumulation into S~: three rounds, each a perfect matching of the four directions, so that the products of
     // one launch write different S~_mu.  Round r: pairs (0, r+1) and the complementary pair.
@@ -598,6 +722,7 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     const int match[3][2] = {{0, 5}, {1, 4}, {2, 3}};   // pair indices: (0,1)+(2,3), (0,2)+(1,3), (0,3)+(1,2)
     for (int r = 0; r < 3; ++r) {
         GemmGroup ga[4], gb[2];
+        int sa[4][2], sbk[2][2];
         for (int q = 0; q < 2; ++q) {
             const int p = match[r][q], mu = pmu[p], nu = pnu[p];
             const Cplx zmn{z[4 * mu + nu].re, z[4 * mu + nu].im};
@@ -608,12 +733,16 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
             ga[2 * q].out.C = St[mu];
             ga[2 * q].out.alpha = Cplx{-zmn.re, zmn.im};
             ga[2 * q].out.accumulate = touched[mu];
+            sa[2 * q][0] = 7 + p;
+            sa[2 * q][1] = 13 + p;
             // S_nu -= z_{nu mu}^* R_{nu mu},  R_{nu mu} = (Y W)^+
             ga[2 * q + 1].A = Y[p];
             ga[2 * q + 1].B = W[p];
             ga[2 * q + 1].out.D = St[nu];
             ga[2 * q + 1].out.beta = Cplx{-znm.re, znm.im};
             ga[2 * q + 1].out.accumulate_d = touched[nu];
+            sa[2 * q + 1][0] = 13 + p;
+            sa[2 * q + 1][1] = 7 + p;
             // S_nu += z_{nu mu} P_{nu mu},  S_mu += z_{mu nu} P_{nu mu}^+,  P_{nu mu} = T U_mu^+
             gb[q].A = T[p];
             gb[q].B = Ud[mu];
@@ -623,10 +752,12 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
             gb[q].out.D = St[mu];
             gb[q].out.beta = zmn;
             gb[q].out.accumulate_d = true;
+            sbk[q][0] = 19 + p;
+            sbk[q][1] = rUd(mu);
         }
-        NSPT_TRY(k_gemm_groups(f, ga, 4));
+        NSPT_TRY(gemm_groups(ga, sa, 4));
         for (int q = 0; q < 2; ++q) touched[pmu[match[r][q]]] = touched[pnu[match[r][q]]] = true;
-        NSPT_TRY(k_gemm_groups(f, gb, 2));
+        NSPT_TRY(gemm_groups(gb, sbk, 2));
     }
     for (int mu = 0; mu < 4; ++mu) NSPT_TRY(k_inverse(f, t, 1, St[mu], S[mu]));
     return NSPT_OK;

@@ -558,6 +558,13 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
                 sco[a][k2] = (k < P.n) ? __ldg(&P.scale_out[k]) : 0.0;
             }
     }
+    unsigned int mx[RETRUNC ? R : 1];   // re-truncation for the INT8 path: running maxima of the modes written (see the forward kernel)
+    const bool track = RETRUNC && P.maxbits[0] != nullptr;
+    unsigned cur_b = 0xffffffffu;
+    if constexpr (RETRUNC) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) mx[i] = 0u;
+    }
     // re-truncation: the forward twiddles too where the register budget allows (R <= 8)
     constexpr bool FWD_TWREG = RETRUNC && (R <= 8);
     double2 twf[FWD_TWREG ? R : 1];
@@ -584,12 +591,19 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
         InvRegs<R, S, T> q;
         inverse_from_regs<R, S, T, true>(x, s, c, P.tw_inv, exch, q, twr);
         if constexpr (RETRUNC) {
+            if (track && b != cur_b) {   // the spectra of a launch are its batch elements
+                if (cur_b != 0xffffffffu) flush_mode_max<R, S, T>(mx, s, c, P.maxbits[0] + (size_t)cur_b * C::L);
+                cur_b = b;
+            }
             double2 xf[R];
             retruncate_regs<R, S, T>(q, s, P.n, P.inv_L, xf);
             __syncthreads();  // phase-2 reads of the inverse are done
             forward_phase1_smem<R, S, T, FWD_TWREG>(xf, s, c, P.tw_fwd, exch, twf);
             __syncthreads();
-            forward_phase2_smem<R, S, T>(s, c, exch);
+            if (track)
+                forward_phase2_smem<R, S, T, true>(s, c, exch, mx);
+            else
+                forward_phase2_smem<R, S, T>(s, c, exch);
             fence_proxy_async_smem();
             __syncthreads();
             if (threadIdx.x == 0) {
@@ -615,6 +629,9 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
                 tma_store_commit();
             }
         }
+    }
+    if constexpr (RETRUNC) {
+        if (track && cur_b != 0xffffffffu) flush_mode_max<R, S, T>(mx, s, c, P.maxbits[0] + (size_t)cur_b * C::L);
     }
     if (threadIdx.x == 0) tma_store_wait_read<0>();
 }
@@ -819,8 +836,9 @@ cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int bat
 }
 
 cudaError_t launch_fft_retruncate(const FreqLayout& f, const PlanTables& t, int batch, const double* src,
-                                  double* dst, cudaStream_t st) {
+                                  double* dst, cudaStream_t st, unsigned long long* maxbits) {
     XformParams P = base_params(f, t, batch);
+    P.maxbits[0] = P.maxbits[1] = maxbits;
     P.src_freq = reinterpret_cast<const double2*>(src);
     P.dst_freq[0] = reinterpret_cast<double2*>(dst);
     return dispatch(f.L, W_RET, P, 1, st);

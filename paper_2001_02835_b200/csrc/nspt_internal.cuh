@@ -76,8 +76,10 @@ cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int bat
 cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int batch,
                                const double* src, nspt_c128* dst, cudaStream_t st);
 // Re-truncation in place in frequency space: inverse, zero orders > Ntrunc, forward.
+// maxbits (optional, INT8 path): [batch][L] entries that receive, by atomicMax, the per-mode maxima of the spectra written
+// (L >= 16 only; the caller clears them).
 cudaError_t launch_fft_retruncate(const FreqLayout& f, const PlanTables& t, int batch,
-                                  const double* src, double* dst, cudaStream_t st);
+                                  const double* src, double* dst, cudaStream_t st, unsigned long long* maxbits = nullptr);
 // Spectrum of the daggered series: Xd~(p) = (X~((L - p) mod L))^H.
 cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src, double* dst,
                                cudaStream_t st);
@@ -125,14 +127,35 @@ cudaError_t launch_naive_conv(const FreqLayout& f, int batch, const nspt_c128* A
                               cudaStream_t st);
 
 // ---- mode-wise matrix product on the INT8 tensor cores (nspt_ozaki.cu) -----------------------------------------
-// Plain C~(p) = A~(p) B~(p) only (no alpha / accumulate / dagger epilogues): the FP64 spectra, whose per-mode maxima the
-// forward transform has recorded in the slice workspace (ozaki_maxbits), are cut into int8 slices (launch_ozaki_slice),
-// multiplied exactly by tcgen05.mma.kind::i8 and recombined in FP64 (launch_ozaki_gemm).
-size_t ozaki_workspace_bytes(const FreqLayout& f, int batch);
-// where the forward transform records max(|re|, |im|) of every mode of operand z (0 = A, 1 = B): batch * L entries each
-unsigned long long* ozaki_maxbits(const FreqLayout& f, int batch, void* ws, int z);
-cudaError_t launch_ozaki_slice(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st);
-cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, const double* A, const double* B, double* C,
-                              cudaStream_t st, bool pairs = false);
+// FP64 spectra, whose per-mode maxima the transforms have recorded (maxbits), are cut into int8 slices (launch_ozaki_slice),
+// multiplied exactly by tcgen05.mma.kind::i8 and recombined in FP64 (launch_ozaki_gemm, same epilogues as launch_zgemm_groups).
+// A left factor must be sliced in the QUAD layout, a right factor in the ROWS layout; the store holds nq + nr such slots of
+// `modes` = batch * L modes each.
+struct OzStore {
+    int8_t* quad = nullptr;
+    int8_t* rows = nullptr;
+    int* exps_q = nullptr;     // [nq][modes]: exponent of every mode of a QUAD slot (written by the slicing pass)
+    int* exps_r = nullptr;     // [nr][modes]
+    size_t quad_slot_bytes = 0, rows_slot_bytes = 0;
+    int nq = 0, nr = 0, modes = 0;
+};
+size_t ozaki_store_bytes(const FreqLayout& f, int modes, int nq, int nr);
+OzStore ozaki_store(const FreqLayout& f, int modes, int nq, int nr, void* ws);
+struct OzSliceJob {
+    const double* X = nullptr;                      // FP64 spectrum, modes x N x N
+    const unsigned long long* maxbits = nullptr;    // [modes] maxima of the modes of X ...
+    bool mirror = false;                            // ... or of the series X is the dagger spectrum of: mode p takes entry (L - p) % L
+    int quad_slot = -1, rows_slot = -1;             // -1: not needed in that layout
+};
+cudaError_t launch_ozaki_slice(const FreqLayout& f, const OzStore& S, const OzSliceJob* jobs, int njobs, cudaStream_t st);
+struct OzGemmGroup {
+    int quad_slot = -1;        // left factor
+    int rows_slot = -1;        // right factor
+    const double* A = nullptr; // the FP64 spectra the two slots were cut from
+    const double* B = nullptr;
+    GemmOut out;
+};
+cudaError_t launch_ozaki_gemm(const FreqLayout& f, const OzStore& S, const OzGemmGroup* groups, int ngroups, cudaStream_t st,
+                              bool pairs = false);
 
 }  // namespace nspt

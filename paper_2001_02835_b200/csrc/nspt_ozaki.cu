@@ -53,21 +53,31 @@ constexpr int OZ_THREADS = 384;                      // warp 0 TMA, warp 1 MMA, 
 constexpr int OZ_TMEM_COLS = 512;
 
 // ---- slicing ------------------------------------------------------------------------------------------------
-// Slicing pass: both operands in one launch (blockIdx.z), the per-mode maxima come from the forward transform (maxbits),
-// digits without 64-bit conversions (oz_fixed), 4 x 4 byte transposes for the packing.
-// thread = 4 consecutive columns of a row of one mode; a warp writes 128 contiguous bytes per (plane, slice).
+// Slicing pass: up to OZ_MAX_JOBS spectra in one launch (blockIdx.z), each into the QUAD and / or the ROWS layout (a spectrum
+// that serves as left factor of one product and as right factor of another is read and converted once); the per-mode maxima
+// come from the transform that wrote the spectrum (maxbits); digits without 64-bit conversions (oz_fixed), 4 x 4 byte
+// transposes for the packing.  thread = 4 consecutive columns of a row of one mode; a warp writes 128 contiguous bytes per
+// (plane, slice).
+constexpr int OZ_MAX_JOBS = 12;
+struct SliceJobDev {
+    const double2* X;
+    const unsigned long long* maxbits;
+    int8_t* quad;      // slot base or null
+    int8_t* rows;      // slot base or null
+    int* exps_q;
+    int* exps_r;
+    int mirror_L;      // 0, or L: mode b L + p takes the maximum of entry b L + (L - p) % L (X is a dagger spectrum)
+};
 struct SliceParams {
-    const double2* X[2];
-    int8_t* out[2];
-    const unsigned long long* maxbits[2];
-    int* exps[2];
-    int pitch[2];
+    SliceJobDev job[OZ_MAX_JOBS];
+    int pitch_q, pitch_r;
     int N, modes;
 };
 constexpr int OZ_SLICE_MODES = 8;   // consecutive modes per thread: the loads of the next mode are in flight while one is cut
 // the 21 slice words of four columns of one mode: re and im planes from the fixed-point integers V1, V2, the re + im plane from
-// floor((V1 + V2) / 2) (same accuracy as rounding (re + im) / 2, without a third conversion)
-__device__ __forceinline__ void oz_slice_store4(const double2 (&v)[4], double sc, int8_t* base, size_t plane_stride, size_t slice_stride) {
+// floor((V1 + V2) / 2) (same accuracy as rounding (re + im) / 2, without a third conversion); w[plane][d] = digit of weight
+// 256^d of the four columns = slice 6 - d
+__device__ __forceinline__ void oz_slice4(const double2 (&v)[4], double sc, unsigned int (&w)[OZ_PLANES][8]) {
     unsigned int lo[OZ_PLANES][4], hi[OZ_PLANES][4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
@@ -78,13 +88,17 @@ __device__ __forceinline__ void oz_slice_store4(const double2 (&v)[4], double sc
     }
 #pragma unroll
     for (int q = 0; q < OZ_PLANES; ++q) {
-        unsigned int w[8];
-        transpose4x4(lo[q], w);
-        transpose4x4(hi[q], w + 4);
+        transpose4x4(lo[q], w[q]);
+        transpose4x4(hi[q], w[q] + 4);
+    }
+}
+__device__ __forceinline__ void oz_store_words(const unsigned int (&w)[OZ_PLANES][8], int8_t* base, size_t plane_stride, size_t slice_stride) {
+#pragma unroll
+    for (int q = 0; q < OZ_PLANES; ++q) {
         int8_t* p = base + (size_t)q * plane_stride + (size_t)(OZ_S - 1) * slice_stride;
 #pragma unroll
-        for (int d = 0; d < OZ_S; ++d) {   // word d = digit of weight 256^d of the four columns = slice 6 - d
-            *reinterpret_cast<unsigned int*>(p) = w[d];
+        for (int d = 0; d < OZ_S; ++d) {
+            *reinterpret_cast<unsigned int*>(p) = w[q][d];
             p -= slice_stride;
         }
     }
@@ -103,19 +117,17 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // warp (stride four elements) cover all banks
 __device__ __forceinline__ int oz_swz(int p) { return p ^ ((p >> 3) & 3); }
 
-__global__ void __launch_bounds__(256) oz_slice_kernel(const SliceParams P) {
+__global__ void __launch_bounds__(256) oz_slice_kernel(const __grid_constant__ SliceParams P) {
     __shared__ double2 stage[2][OZ_SLICE_BUF];
     __shared__ double ssc[OZ_SLICE_MODES];
-    const int z = blockIdx.z;
-    const bool quad = (z == 0);
-    const double2* X = z ? P.X[1] : P.X[0];
-    int8_t* O = z ? P.out[1] : P.out[0];
-    const unsigned long long* MB = z ? P.maxbits[1] : P.maxbits[0];
-    int* EX = z ? P.exps[1] : P.exps[0];
-    const int N = P.N, pitch = z ? P.pitch[1] : P.pitch[0];
-    const int qpr = quad ? (pitch >> 5) : ((N + 3) >> 2);   // 4-column groups per row (QUAD: the k padding is written too)
+    const SliceJobDev& J = P.job[blockIdx.z];
+    const int N = P.N;
+    const bool quad = J.quad != nullptr, rows = J.rows != nullptr;
+    // 4-column groups per row: the QUAD layout writes its k padding (zeros up to a multiple of 32 columns) as well
+    const int qpr = quad ? (P.pitch_q >> 5) : ((N + 3) >> 2);
     const int total = N * qpr;
     const int t0 = blockIdx.x * 256, t = t0 + threadIdx.x;
+    if (t0 >= total) return;
     const int m_begin = blockIdx.y * OZ_SLICE_MODES;
     const int nm = P.modes - m_begin < OZ_SLICE_MODES ? P.modes - m_begin : OZ_SLICE_MODES;
     // contiguous element range of this CTA: from the first column of its first group to the end of its last group
@@ -126,13 +138,21 @@ __global__ void __launch_bounds__(256) oz_slice_kernel(const SliceParams P) {
     pdl_wait();
     pdl_trigger();
     if (threadIdx.x < nm) {
-        const int e = oz_exponent(MB[m_begin + threadIdx.x]);
+        int m = m_begin + threadIdx.x;
+        if (J.mirror_L) {
+            const int p = m % J.mirror_L;
+            m = m - p + (J.mirror_L - p) % J.mirror_L;
+        }
+        const int e = oz_exponent(J.maxbits[m]);
         ssc[threadIdx.x] = oz_pow2(OZ_FRAC_BITS - e);
-        if (blockIdx.x == 0) EX[m_begin + threadIdx.x] = e;
+        if (blockIdx.x == 0) {
+            if (quad) J.exps_q[m_begin + threadIdx.x] = e;
+            if (rows) J.exps_r[m_begin + threadIdx.x] = e;
+        }
     }
     auto fetch = [&](int i) {   // mode m_begin + i -> stage i & 1
         if (i < nm) {
-            const double2* src = X + (size_t)(m_begin + i) * N * N + e0;
+            const double2* src = J.X + (size_t)(m_begin + i) * N * N + e0;
             const uint32_t dst = smem_u32(&stage[i & 1][0]);
             for (int p = threadIdx.x; p < count; p += 256) cp_async16(dst + 16u * (uint32_t)oz_swz(p), src + p);
         }
@@ -143,10 +163,10 @@ __global__ void __launch_bounds__(256) oz_slice_kernel(const SliceParams P) {
     const int row = active ? t / qpr : 0, j0 = active ? (t % qpr) * 4 : 0;
     const int nvalid = active ? N - j0 : 0;   // columns of this group inside the matrix (<= 0: k padding of the QUAD layout)
     const int p0 = row * N + j0 - e0;
-    const size_t plane_stride = quad ? (size_t)N * pitch : (size_t)OZ_S * N * pitch;
-    const size_t slice_stride = quad ? (size_t)32 : (size_t)N * pitch;
-    const size_t mode_stride = (size_t)OZ_PLANES * plane_stride;
-    int8_t* out = O + (size_t)m_begin * mode_stride + (size_t)row * pitch + (quad ? (size_t)(j0 >> 5) * 256 + (j0 & 31) : (size_t)j0);
+    const size_t q_plane = (size_t)N * P.pitch_q, q_mode = (size_t)OZ_PLANES * q_plane;
+    const size_t r_slice = (size_t)N * P.pitch_r, r_plane = (size_t)OZ_S * r_slice, r_mode = (size_t)OZ_PLANES * r_plane;
+    int8_t* outq = quad ? J.quad + (size_t)m_begin * q_mode + (size_t)row * P.pitch_q + (size_t)(j0 >> 5) * 256 + (j0 & 31) : nullptr;
+    int8_t* outr = (rows && j0 < P.pitch_r) ? J.rows + (size_t)m_begin * r_mode + (size_t)row * P.pitch_r + j0 : nullptr;
 #pragma unroll 1
     for (int i = 0; i < nm; ++i) {
         fetch(i + 1);
@@ -156,7 +176,10 @@ __global__ void __launch_bounds__(256) oz_slice_kernel(const SliceParams P) {
             double2 v[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) v[c] = c < nvalid ? stage[i & 1][oz_swz(p0 + c)] : make_double2(0.0, 0.0);
-            oz_slice_store4(v, ssc[i], out + (size_t)i * mode_stride, plane_stride, slice_stride);
+            unsigned int w[OZ_PLANES][8];
+            oz_slice4(v, ssc[i], w);
+            if (outq) oz_store_words(w, outq + (size_t)i * q_mode, q_plane, 32);
+            if (outr) oz_store_words(w, outr + (size_t)i * r_mode, r_plane, r_slice);
         }
         __syncthreads();   // stage i & 1 may be refilled
     }
@@ -383,16 +406,28 @@ __device__ __forceinline__ double oz_combine(int a0, int a1, int a2, int a3, int
     return h;
 }
 
-struct OzParams {
-    double2* C;
-    const double2* At;         // FP64 spectra, read for the last `tail` columns of A~ / rows of B~ only
+// One product of a launch: left factor = QUAD slot, right factor = ROWS slot (as (mode, plane) offsets of the tensor maps),
+// the FP64 spectra they were cut from (tail of K), their exponent tables, and the epilogue of nspt_zgemm.cu's GemmOut:
+//     C(p)            (+)= alpha * M(p) + diag * 1,        D((L - p) mod L) (+)= beta * M(p)^H.
+struct OzGroupDev {
+    const double2* At;
     const double2* Bt;
     const int* expA;
     const int* expB;
+    double2* C;
+    double2* D;
+    double alpha_re, alpha_im, beta_re, beta_im, diag;
+    int pbaseA, pbaseB;        // first (mode, plane) index of the slot in the N-side / M-side tensor map
+    int accumulate, accumulate_d;
+};
+constexpr int OZ_MAX_GROUPS = 12;
+struct OzParams {
+    OzGroupDev g[OZ_MAX_GROUPS];
     size_t NN;
-    int N;
+    int N, L;
+    int modes;                 // modes per group (batch * L)
     int tiles_i, tiles_j;      // tiles per mode: rows in steps of 64, columns in steps of 128 * CG
-    int total_tiles;
+    int total_tiles;           // groups * modes * tiles_i * tiles_j
     int nkc;                   // K-chunks of 32 that run on the tensor core
     int tail;                  // k >= 32 nkc (0 .. OZ_TAIL_MAX of them) are added in FP64 by the epilogue
 };
@@ -403,7 +438,8 @@ constexpr int OZ_TAIL_MAX = 2;
 
 template <int CG>
 __global__ void __launch_bounds__(OZ_THREADS, 1)
-zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_constant__ CUtensorMap mapN, const OzParams P) {
+zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_constant__ CUtensorMap mapN,
+                      const __grid_constant__ OzParams P) {
     using K = OzCfg<CG>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -448,18 +484,19 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
             if (lane == 0) {
                 int it = 0;
                 for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
-                    const int mode = tile / tiles_per_mode, rem = tile % tiles_per_mode;
+                    const int gm = tile / tiles_per_mode, rem = tile % tiles_per_mode;   // gm = group * modes + mode
+                    const int grp = gm / P.modes, mode = gm % P.modes;
                     const int i0 = (rem / P.tiles_j) * OZ_BN + (int)rank * K::N_ROWS;
                     const int j0 = (rem % P.tiles_j) * (OZ_BM * CG) + (int)rank * OZ_BM;
+                    const int pa = P.g[grp].pbaseA + mode * OZ_PLANES, pb = P.g[grp].pbaseB + mode * OZ_PLANES;
                     for (int plane = 0; plane < OZ_PLANES; ++plane) {
-                        const int pidx = mode * OZ_PLANES + plane;
                         for (int kc = 0; kc < nkc; ++kc, ++it) {
                             const int slot = it % K::STAGES;
                             mbar_wait_wd(bar_empty + 8 * slot, ((it / K::STAGES) & 1) ^ 1);
                             if (rank == 0) mbar_expect_tx(bar_full + 8 * slot, K::STAGE * CG);
                             const uint32_t st = base + slot * K::STAGE;
-                            tma_load_4d_cg<CG>(st, &mapM, lead_full + 8 * slot, j0, kc * OZ_KC, 0, pidx);
-                            tma_load_5d_cg<CG>(st + OZ_M_STAGE, &mapN, lead_full + 8 * slot, 0, i0, 0, kc, pidx);
+                            tma_load_4d_cg<CG>(st, &mapM, lead_full + 8 * slot, j0, kc * OZ_KC, 0, pb + plane);
+                            tma_load_5d_cg<CG>(st + OZ_M_STAGE, &mapN, lead_full + 8 * slot, 0, i0, 0, kc, pa + plane);
                         }
                     }
                 }
@@ -499,11 +536,13 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
         const int we = warp - 4, quarter = we & 3, half = we >> 2;
         int acc_it = 0;
         for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
-            const int mode = tile / tiles_per_mode, rem = tile % tiles_per_mode;
+            const int gm = tile / tiles_per_mode, rem = tile % tiles_per_mode;
+            const int mode = gm % P.modes;
+            const OzGroupDev& G = P.g[gm / P.modes];
             const int row0 = (rem / P.tiles_j) * OZ_BN + 32 * half;
             const int col = (rem % P.tiles_j) * (OZ_BM * CG) + (int)rank * OZ_BM + 32 * quarter + lane;
             double re[32], im[32];
-            const int esum = P.expA[mode] + P.expB[mode];
+            const int esum = G.expA[mode] + G.expB[mode];
             const double sc = esum >= (1 << 20) ? __longlong_as_double(0x7ff8000000000000ll) : oz_pow2(esum - 12);
             // The tail of K (k >= 32 nkc) in FP64, while the MMAs of the first plane run: lane l fetches A~[row0 + l][k] and its
             // own column of B~[k][.]; the running sums start from the tail product in units of the common scale (a power of two)
@@ -514,8 +553,8 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                 for (int t = 0; t < P.tail; ++t) {
                     const int k = OZ_KC * nkc + t;
                     double2 at = make_double2(0.0, 0.0), bt = make_double2(0.0, 0.0);
-                    if (row0 + lane < P.N) at = __ldg(P.At + (size_t)mode * P.NN + (size_t)(row0 + lane) * P.N + k);
-                    if (col < P.N) bt = __ldg(P.Bt + (size_t)mode * P.NN + (size_t)k * P.N + col);
+                    if (row0 + lane < P.N) at = __ldg(G.At + (size_t)mode * P.NN + (size_t)(row0 + lane) * P.N + k);
+                    if (col < P.N) bt = __ldg(G.Bt + (size_t)mode * P.NN + (size_t)k * P.N + col);
                     bt.x *= isc;
                     bt.y *= isc;
 #pragma unroll
@@ -564,12 +603,51 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                     if (CG == 2) mbar_arrive_cluster(lead_acc_empty); else mbar_arrive(bar_acc_empty);
                 }
             }
-            // scaling and stores overlap the MMAs of the next tile
+            // scaling, epilogue and stores overlap the MMAs of the next tile
             if (col < P.N) {
-                double2* c = P.C + (size_t)mode * P.NN + col;
+                if (G.C) {
+                    double2* c = G.C + (size_t)mode * P.NN + col;
+                    const bool plain = G.alpha_re == 1.0 && G.alpha_im == 0.0 && G.diag == 0.0 && !G.accumulate;
+                    if (plain) {
 #pragma unroll
-                for (int j = 0; j < 32; ++j)   // the 32 lanes of a warp write 512 contiguous bytes of row row0 + j
-                    if (row0 + j < P.N) c[(size_t)(row0 + j) * P.N] = make_double2(sc * re[j], sc * im[j]);
+                        for (int j = 0; j < 32; ++j)   // the 32 lanes of a warp write 512 contiguous bytes of row row0 + j
+                            if (row0 + j < P.N) c[(size_t)(row0 + j) * P.N] = make_double2(sc * re[j], sc * im[j]);
+                    } else {
+                        const double ar = sc * G.alpha_re, ai = sc * G.alpha_im;
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) {
+                            if (row0 + j < P.N) {
+                                double2 o = make_double2(ar * re[j] - ai * im[j], ar * im[j] + ai * re[j]);
+                                if (row0 + j == col) o.x += G.diag;
+                                double2* dst = c + (size_t)(row0 + j) * P.N;
+                                if (G.accumulate) {   // one contribution per element and launch: the sum keeps a fixed order
+                                    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&dst->x), "d"(o.x) : "memory");
+                                    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&dst->y), "d"(o.y) : "memory");
+                                } else {
+                                    *dst = o;
+                                }
+                            }
+                        }
+                    }
+                }
+                if (G.D) {
+                    // spectrum of the daggered product series: D((L - p) mod L)[j][i] (+)= beta conj(M(p)[i][j])
+                    const int pm = mode % P.L;
+                    double2* d = G.D + (size_t)(mode - pm + (P.L - pm) % P.L) * P.NN + (size_t)col * P.N + row0;
+                    const double br = sc * G.beta_re, bi = sc * G.beta_im;
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        if (row0 + j < P.N) {
+                            const double2 o = make_double2(br * re[j] + bi * im[j], bi * re[j] - br * im[j]);
+                            if (G.accumulate_d) {
+                                asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&d[j].x), "d"(o.x) : "memory");
+                                asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&d[j].y), "d"(o.y) : "memory");
+                            } else {
+                                d[j] = o;
+                            }
+                        }
+                    }
+                }
             }
         }
     }
@@ -601,64 +679,8 @@ cudaError_t encode_u8(CUtensorMap* map, const int8_t* basep, int rank, const cuu
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-struct OzWs {
-    int8_t* sA;                    // QUAD layout
-    int8_t* sB;                    // ROWS layout
-    unsigned long long* maxbits;   // [2][modes]
-    int* exps;                     // [2][modes]
-};
-OzWs oz_carve(const FreqLayout& f, int batch, void* ws) {
-    const size_t modes = (size_t)batch * f.L;
-    OzWs w;
-    w.sA = static_cast<int8_t*>(ws);
-    w.sB = w.sA + oz_bytes_quad(f.N, modes);
-    w.maxbits = reinterpret_cast<unsigned long long*>(w.sB + oz_bytes_rows(f.N, modes));
-    w.exps = reinterpret_cast<int*>(w.maxbits + 2 * modes);
-    return w;
-}
-
-}  // namespace
-
-unsigned long long* ozaki_maxbits(const FreqLayout& f, int batch, void* ws, int z) {
-    return oz_carve(f, batch, ws).maxbits + (size_t)z * batch * f.L;
-}
-
-size_t ozaki_workspace_bytes(const FreqLayout& f, int batch) {
-    const size_t modes = (size_t)batch * f.L;
-    return oz_bytes_quad(f.N, modes) + oz_bytes_rows(f.N, modes) + 2 * modes * 16 + 256;
-}
-
-// FP64 spectra A~, B~ -> int8 slices, with the per-mode maxima already in the workspace (written by the forward transform)
-cudaError_t launch_ozaki_slice(const FreqLayout& f, int batch, const double* A, const double* B, void* ws, cudaStream_t st) {
-    const int modes = batch * f.L;
-    const int N = f.N;
-    const OzWs w = oz_carve(f, batch, ws);
-    SliceParams P;
-    P.X[0] = reinterpret_cast<const double2*>(A);
-    P.X[1] = reinterpret_cast<const double2*>(B);
-    P.out[0] = w.sA;
-    P.out[1] = w.sB;
-    P.maxbits[0] = w.maxbits;
-    P.maxbits[1] = w.maxbits + modes;
-    P.exps[0] = w.exps;
-    P.exps[1] = w.exps + modes;
-    P.pitch[0] = oz_pitch_quad(N);
-    P.pitch[1] = oz_pitch_rows(N);
-    P.N = N;
-    P.modes = modes;
-    const int groups = N * (P.pitch[0] >> 5);   // the QUAD operand has the most 4-column groups per mode
-    cudaLaunchConfig_t cfg = {};
-    const int my = (modes + OZ_SLICE_MODES - 1) / OZ_SLICE_MODES;
-    cfg.gridDim = dim3((unsigned)((groups + 255) / 256), (unsigned)(my < 65535 ? my : 65535), 2);
-    cfg.blockDim = dim3(256, 1, 1);
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, oz_slice_kernel, P);
-}
+size_t quad_slot_bytes(const FreqLayout& f, int modes) { return oz_bytes_quad(f.N, (size_t)modes); }
+size_t rows_slot_bytes(const FreqLayout& f, int modes) { return oz_bytes_rows(f.N, (size_t)modes); }
 
 // launch with programmatic stream serialization and (CG = 2) clusters of two CTAs
 template <typename... KArgs, typename... Args>
@@ -681,25 +703,27 @@ cudaError_t launch_pdl_cluster(void (*kernel)(KArgs...), unsigned grid, unsigned
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
-void oz_maps(const FreqLayout& f, int modes, const OzWs& w, int n_rows, CUtensorMap* mapM, CUtensorMap* mapN, cudaError_t* err) {
+// tensor maps over ALL slots of the store: a product addresses its operands by (mode, plane) offset
+cudaError_t oz_maps(const FreqLayout& f, const OzStore& S, int n_rows, CUtensorMap* mapM, CUtensorMap* mapN) {
     const int N = f.N;
     const int pq = oz_pitch_quad(N), pr = oz_pitch_rows(N), nkc = (N + OZ_KC - 1) / OZ_KC;
-    {   // B~ slices, ROWS layout: (col j, row k, slice, mode * plane); box = [7 slices][32 k][128 bytes of j]
-        const cuuint64_t dims[4] = {(cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)OZ_S, (cuuint64_t)modes * OZ_PLANES};
+    cudaError_t e;
+    {   // right factors, ROWS layout: (col j, row k, slice, slot * mode * plane); box = [7 slices][32 k][128 bytes of j]
+        const cuuint64_t dims[4] = {(cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)OZ_S, (cuuint64_t)(S.nr > 0 ? S.nr : 1) * S.modes * OZ_PLANES};
         const cuuint64_t strides[3] = {(cuuint64_t)pr, (cuuint64_t)N * pr, (cuuint64_t)OZ_S * N * pr};
         const cuuint32_t box[4] = {(cuuint32_t)OZ_BM, (cuuint32_t)OZ_KC, (cuuint32_t)OZ_S, 1};
-        if ((*err = encode_u8(mapM, w.sB, 4, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) != cudaSuccess) return;
+        if ((e = encode_u8(mapM, S.rows, 4, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B)) != cudaSuccess) return e;
     }
-    {   // A~ slices, QUAD layout: (128 bytes = 4 slots, row i, half, k-chunk, mode * plane); box = [2 halves][rows][128 bytes]
-        const cuuint64_t dims[5] = {128, (cuuint64_t)N, 2, (cuuint64_t)nkc, (cuuint64_t)modes * OZ_PLANES};
+    {   // left factors, QUAD layout: (128 bytes = 4 slots, row i, half, k-chunk, slot * mode * plane); box = [2 halves][rows][128 bytes]
+        const cuuint64_t dims[5] = {128, (cuuint64_t)N, 2, (cuuint64_t)nkc, (cuuint64_t)(S.nq > 0 ? S.nq : 1) * S.modes * OZ_PLANES};
         const cuuint64_t strides[4] = {(cuuint64_t)pq, 128, 256, (cuuint64_t)N * pq};
         const cuuint32_t box[5] = {128, (cuuint32_t)n_rows, 2, 1, 1};
-        *err = encode_u8(mapN, w.sA, 5, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+        return encode_u8(mapN, S.quad, 5, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
     }
 }
 
 template <int CG>
-cudaError_t launch_oz(const FreqLayout& f, int modes, const OzWs& w, const double* At, const double* Bt, double* C, cudaStream_t st) {
+cudaError_t launch_oz(const FreqLayout& f, const OzStore& S, const OzGemmGroup* groups, int ngroups, cudaStream_t st) {
     using K = OzCfg<CG>;
     const int N = f.N;
     cudaError_t e;
@@ -714,37 +738,116 @@ cudaError_t launch_oz(const FreqLayout& f, int modes, const OzWs& w, const doubl
         attr_done[dev] = true;
     }
     CUtensorMap mapM, mapN;
-    oz_maps(f, modes, w, K::N_ROWS, &mapM, &mapN, &e);
-    if (e != cudaSuccess) return e;
-    OzParams P;
-    P.C = reinterpret_cast<double2*>(C);
-    P.At = reinterpret_cast<const double2*>(At);
-    P.Bt = reinterpret_cast<const double2*>(Bt);
-    P.expA = w.exps;
-    P.expB = w.exps + modes;
+    if ((e = oz_maps(f, S, K::N_ROWS, &mapM, &mapN)) != cudaSuccess) return e;
+    OzParams P{};
     P.NN = f.NN;
     P.N = N;
+    P.L = f.L;
+    P.modes = S.modes;
     P.tiles_i = (N + OZ_BN - 1) / OZ_BN;
     P.tiles_j = (N + OZ_BM * CG - 1) / (OZ_BM * CG);
-    P.total_tiles = modes * P.tiles_i * P.tiles_j;
+    P.total_tiles = ngroups * S.modes * P.tiles_i * P.tiles_j;
     P.nkc = (N + OZ_KC - 1) / OZ_KC;
     P.tail = 0;
-    if (At && Bt && N >= 2 * OZ_KC && N % OZ_KC != 0 && N % OZ_KC <= OZ_TAIL_MAX) {
+    if (N >= 2 * OZ_KC && N % OZ_KC != 0 && N % OZ_KC <= OZ_TAIL_MAX) {
         P.nkc = N / OZ_KC;
         P.tail = N % OZ_KC;
+    }
+    for (int i = 0; i < ngroups; ++i) {
+        const OzGemmGroup& g = groups[i];
+        if (g.quad_slot < 0 || g.quad_slot >= S.nq || g.rows_slot < 0 || g.rows_slot >= S.nr || !g.A || !g.B || (!g.out.C && !g.out.D))
+            return cudaErrorInvalidValue;
+        OzGroupDev& d = P.g[i];
+        d.At = reinterpret_cast<const double2*>(g.A);
+        d.Bt = reinterpret_cast<const double2*>(g.B);
+        d.expA = S.exps_q + (size_t)g.quad_slot * S.modes;
+        d.expB = S.exps_r + (size_t)g.rows_slot * S.modes;
+        d.C = reinterpret_cast<double2*>(g.out.C);
+        d.D = reinterpret_cast<double2*>(g.out.D);
+        d.alpha_re = g.out.alpha.re;
+        d.alpha_im = g.out.alpha.im;
+        d.beta_re = g.out.beta.re;
+        d.beta_im = g.out.beta.im;
+        d.diag = g.out.diag;
+        d.pbaseA = g.quad_slot * S.modes * OZ_PLANES;
+        d.pbaseB = g.rows_slot * S.modes * OZ_PLANES;
+        d.accumulate = g.out.accumulate ? 1 : 0;
+        d.accumulate_d = g.out.accumulate_d ? 1 : 0;
     }
     int clusters = sms[dev] / CG;
     if (clusters > P.total_tiles) clusters = P.total_tiles;
     return launch_pdl_cluster(zgemm_modes_i8_kernel<CG>, (unsigned)(clusters * CG), OZ_THREADS, K::SMEM, CG, st, mapM, mapN, P);
 }
 
-// C~(p) = A~(p) B~(p) for all batch * L modes from the slices in `ws` (and, for the last N mod 32 <= 2 values of k, from the FP64
-// spectra A, B the slices were cut from); pairs = true runs the tiles on CTA pairs (tcgen05.mma.cta_group::2)
-cudaError_t launch_ozaki_gemm(const FreqLayout& f, int batch, const void* ws, const double* A, const double* B, double* C,
-                              cudaStream_t st, bool pairs) {
-    const int modes = batch * f.L;
-    const OzWs w = oz_carve(f, batch, const_cast<void*>(ws));
-    return pairs ? launch_oz<2>(f, modes, w, A, B, C, st) : launch_oz<1>(f, modes, w, A, B, C, st);
+}  // namespace
+
+size_t ozaki_store_bytes(const FreqLayout& f, int modes, int nq, int nr) {
+    return (size_t)nq * quad_slot_bytes(f, modes) + (size_t)nr * rows_slot_bytes(f, modes) + (size_t)(nq + nr) * modes * sizeof(int) + 512;
+}
+
+OzStore ozaki_store(const FreqLayout& f, int modes, int nq, int nr, void* ws) {
+    OzStore S;
+    S.nq = nq;
+    S.nr = nr;
+    S.modes = modes;
+    S.quad_slot_bytes = quad_slot_bytes(f, modes);
+    S.rows_slot_bytes = rows_slot_bytes(f, modes);
+    S.quad = static_cast<int8_t*>(ws);
+    S.rows = S.quad + (size_t)nq * S.quad_slot_bytes;
+    S.exps_q = reinterpret_cast<int*>(S.rows + (size_t)nr * S.rows_slot_bytes);
+    S.exps_r = S.exps_q + (size_t)nq * modes;
+    return S;
+}
+
+// FP64 spectra -> int8 slices, with the per-mode maxima the transforms recorded; up to OZ_MAX_JOBS spectra per launch
+cudaError_t launch_ozaki_slice(const FreqLayout& f, const OzStore& S, const OzSliceJob* jobs, int njobs, cudaStream_t st) {
+    const int N = f.N;
+    for (int j0 = 0; j0 < njobs; j0 += OZ_MAX_JOBS) {
+        const int nj = njobs - j0 < OZ_MAX_JOBS ? njobs - j0 : OZ_MAX_JOBS;
+        SliceParams P{};
+        P.pitch_q = oz_pitch_quad(N);
+        P.pitch_r = oz_pitch_rows(N);
+        P.N = N;
+        P.modes = S.modes;
+        bool any_quad = false;
+        for (int j = 0; j < nj; ++j) {
+            const OzSliceJob& s = jobs[j0 + j];
+            if (!s.X || !s.maxbits || s.quad_slot >= S.nq || s.rows_slot >= S.nr || (s.quad_slot < 0 && s.rows_slot < 0))
+                return cudaErrorInvalidValue;
+            SliceJobDev& d = P.job[j];
+            d.X = reinterpret_cast<const double2*>(s.X);
+            d.maxbits = s.maxbits;
+            d.quad = s.quad_slot >= 0 ? S.quad + (size_t)s.quad_slot * S.quad_slot_bytes : nullptr;
+            d.rows = s.rows_slot >= 0 ? S.rows + (size_t)s.rows_slot * S.rows_slot_bytes : nullptr;
+            d.exps_q = s.quad_slot >= 0 ? S.exps_q + (size_t)s.quad_slot * S.modes : nullptr;
+            d.exps_r = s.rows_slot >= 0 ? S.exps_r + (size_t)s.rows_slot * S.modes : nullptr;
+            d.mirror_L = s.mirror ? f.L : 0;
+            any_quad = any_quad || s.quad_slot >= 0;
+        }
+        const int groups = N * (any_quad ? (P.pitch_q >> 5) : ((N + 3) >> 2));   // jobs without a QUAD target leave the rest of the grid at once
+        const int my = (S.modes + OZ_SLICE_MODES - 1) / OZ_SLICE_MODES;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)((groups + 255) / 256), (unsigned)(my < 65535 ? my : 65535), (unsigned)nj);
+        cfg.blockDim = dim3(256, 1, 1);
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        cudaError_t e = cudaLaunchKernelEx(&cfg, oz_slice_kernel, P);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+// Up to OZ_MAX_GROUPS independent products M(p) = A~(p) B~(p) of the same shape in one launch, operands from the slots of
+// the store (and, for the last N mod 32 <= 2 values of k, from the FP64 spectra they were cut from), epilogues as in
+// nspt_zgemm.cu; pairs = true runs every tile on a CTA pair (tcgen05.mma.cta_group::2)
+cudaError_t launch_ozaki_gemm(const FreqLayout& f, const OzStore& S, const OzGemmGroup* groups, int ngroups, cudaStream_t st,
+                              bool pairs) {
+    if (ngroups < 1 || ngroups > OZ_MAX_GROUPS) return cudaErrorInvalidValue;
+    return pairs ? launch_oz<2>(f, S, groups, ngroups, st) : launch_oz<1>(f, S, groups, ngroups, st);
 }
 
 }  // namespace nspt
