@@ -596,7 +596,7 @@ def run_cuda(args):
         if int8_path and gemm:
             # the dominant kernel is a contraction in INT8: 28 slice pairs x 3 planes of N^3 multiply-adds per mode, against
             # the INT8 peak = measured dense bf16 peak x the nominal ratio 2 (B200_PROFILING.md); beside it the FP64 work it stands for
-            int8_ops = 84 * 2.0 * N ** 3 * L * batch
+            int8_ops = 84 * 2.0 * N ** 3 * L * batch * gemm_products_per_step   # all mode-wise products of a step
             bf16 = peaks.get("bf16_tflops", 1630.0)
             int8_peak = 2.0 * bf16
             ach_i8 = int8_ops * K / (gemm["ms_total"] * 1e-3) * 1e-12
@@ -611,7 +611,11 @@ def run_cuda(args):
                                     "ratio_to_fp64_tensor_peak": (achieved / fp64_peak) if achieved else None},
                 "hbm_peak_GB_s": hbm, "hbm_peak_source": hbm_src,
             }
-            fft_step_bytes["int8_slicing"] = 2 * (16 + 21) * L * N * N * batch   # per operand: read L*e, write 21 bytes per element
+            if kind == "staple":
+                # 8 + 12 + 6 spectra are cut per staple: 18 of them into both layouts (read 16, write 2 x 21 bytes per element), 8 into one
+                fft_step_bytes["int8_slicing"] = (18 * (16 + 42) + 8 * (16 + 21)) * L * N * N
+            else:
+                fft_step_bytes["int8_slicing"] = 2 * (16 + 21) * L * N * N * batch   # per operand: read L*e, write 21 bytes per element
             if "int8_slicing" in stages_out and stage_ms["int8_slicing"]["ms_total"] > 0:
                 gbs = fft_step_bytes["int8_slicing"] * K / (stage_ms["int8_slicing"]["ms_total"] * 1e-3) * 1e-9
                 stages_out["int8_slicing"].update({"algorithmic_bytes_per_step": fft_step_bytes["int8_slicing"], "algorithmic_GB_s": gbs,

@@ -586,6 +586,62 @@ def test_config3_full(nspt):
     check_product(nspt, A, B)
 
 
+@pytest.mark.parametrize("variant", [2, 4])
+@pytest.mark.parametrize("N,Ntrunc,seed", [(9, 8, 60), (25, 15, 61), (50, 12, 62), (65, 8, 63), (129, 9, 64)])
+def test_staple_int8_tensor_cores(nspt, N, Ntrunc, seed, variant):
+    # the staple with all 36 products on the INT8 tensor cores (forced; L >= 16): twelve / six / four / two products per launch,
+    # operands as slots of the slice store, alpha / accumulating / conjugate-transposed epilogues, dagger spectra sliced with
+    # mirrored maxima, re-truncation passes that record the maxima -- against the literal eq. 2.3 of the oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(seed)
+    U = [wl.unitary_series(N, Ntrunc, rng) for _ in range(4)]
+    z = wl.twist_tensor(7, 3)
+    nspt.nspt_set_gemm_variant(variant)
+    try:
+        check_staple(nspt, U, z)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+
+
+def test_staple_int8_generic_twist_and_aliasing(nspt):
+    # non-unimodular, non-antisymmetric z (the library uses z as given) and S aliasing U, on the INT8 path
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(65)
+    N, Ntrunc = 40, 9
+    U = [wl.unitary_series(N, Ntrunc, rng) for _ in range(4)]
+    z = rng.standard_normal((4, 4)) + 1j * rng.standard_normal((4, 4))
+    ref = oracle.staple(U, z)
+    bounds = oracle.staple_bound(U)
+    Ud = [to_dev(u) for u in U]
+    nspt.nspt_set_gemm_variant(2)
+    try:
+        S = nspt.nspt_staple(Ud, z, Ud)      # in place
+        torch.cuda.synchronize()
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+    zmax = np.abs(z).max()
+    for mu in range(4):
+        assert oracle.per_order_error(S[mu].cpu().numpy(), ref[mu], zmax * bounds[mu]).max() <= TOL
+
+
+def test_config4_staple_full_automatic_choice(nspt):
+    # BASELINE.json configs[3] through the default kernel choice (INT8 tensor cores at N = 225), both criteria of check_staple
+    from paper_2001_02835_b200 import workloads as wl
+    U, z = wl.config_staple(225, 31, seed=4)
+    nspt.nspt_set_gemm_variant(-1)
+    try:
+        nspt.nspt_profile(True)
+        nspt.nspt_profile_read("int8_slicing")
+        check_staple(nspt, U, z)
+        _, launches = nspt.nspt_profile_read("int8_slicing")
+        nspt.nspt_profile(False)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+    assert launches == 3
+
+
 def test_config4_staple_full(nspt):
     from paper_2001_02835_b200 import workloads as wl
     U, z = wl.config_staple(225, 31, seed=4)
