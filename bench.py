@@ -614,6 +614,9 @@ def run_cuda(args):
             if kind == "staple":
                 # 8 + 12 + 6 spectra are cut per staple: 18 of them into both layouts (read 16, write 2 x 21 bytes per element), 8 into one
                 fft_step_bytes["int8_slicing"] = (18 * (16 + 42) + 8 * (16 + 21)) * L * N * N
+            elif kind == "exp":
+                # X^1..X^s into both layouts, the r-1 Horner left factors into one, and one max pass over B_{r-1}
+                fft_step_bytes["int8_slicing"] = (s_ps * (16 + 42) + (r_ps - 1) * (16 + 21) + 16) * L * N * N * batch
             else:
                 fft_step_bytes["int8_slicing"] = 2 * (16 + 21) * L * N * N * batch   # per operand: read L*e, write 21 bytes per element
             if "int8_slicing" in stages_out and stage_ms["int8_slicing"]["ms_total"] > 0:

@@ -217,7 +217,9 @@ size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
     if (op == NSPT_OP_SERIES_EXP) {
         int s, r;
         exp_split(f.n - 1, &s, &r);
-        return (size_t)(s ? s + r : 3) * spectrum_bytes(f, batch) + WS_PAD;
+        size_t b = (size_t)(s ? s + r : 3) * spectrum_bytes(f, batch) + WS_PAD;
+        if (s && use_int8(f)) b += maxbits_bytes((s + r) * batch * f.L) + ozaki_store_bytes(f, batch * f.L, s + r, s);
+        return b;
     }
     return 3 * spectrum_bytes(f, batch) + WS_PAD;
 }
@@ -483,28 +485,65 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
     double* Xt = reinterpret_cast<double*>(ws);
     double* Tt = reinterpret_cast<double*>(ws + sb);
     double* Pt = reinterpret_cast<double*>(ws + 2 * sb);
+    int ps, pr;
+    exp_split(Ntrunc, &ps, &pr);
+    const bool i8 = ps && use_int8(f);
+    const int modes = batch * f.L;
+    // INT8 path (use_int8): per-mode maxima of spectrum i (0-based: X^1..X^s, then B_0..B_{r-1}) and the slice store, QUAD slot
+    // = spectrum index (left factors: powers and Horner sums), ROWS slot = power index (right factors: X^1..X^s)
+    unsigned long long* mb = nullptr;
+    OzStore store;
+    if (i8) {
+        char* extra = ws + (size_t)(ps + pr) * sb + WS_PAD;
+        mb = reinterpret_cast<unsigned long long*>(extra);
+        store = ozaki_store(f, modes, ps + pr, ps, extra + maxbits_bytes((ps + pr) * modes));
+        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * (size_t)(ps + pr) * modes, g.stream));
+    }
     {   // X~ with the coefficient of g^0 taken as zero
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_FWD));
-        NSPT_CUDA(launch_fft_forward(f, t, batch, X, Xt, nullptr, nullptr, g.stream, true));
+        NSPT_CUDA(launch_fft_forward(f, t, batch, X, Xt, nullptr, nullptr, g.stream, true, mb, nullptr));
         NSPT_TRY(tm.end());
     }
-    int ps, pr;
-    exp_split(Ntrunc, &ps, &pr);
     if (ps) {
         auto pw = [&](int i) { return reinterpret_cast<double*>(ws + (size_t)(i - 1) * sb); };     // spectrum of X^i, i = 1..s
         auto bj = [&](int j) { return reinterpret_cast<double*>(ws + (size_t)(ps + j) * sb); };    // B_j, later the Horner sums
+        auto slice_powers = [&](int first, int cnt) -> int {   // X^first .. X^(first+cnt-1) into both layouts
+            OzSliceJob jobs[12];
+            for (int i = 0; i < cnt; ++i) {
+                jobs[i].X = pw(first + i);
+                jobs[i].maxbits = mb + (size_t)(first + i - 1) * modes;
+                jobs[i].quad_slot = first + i - 1;
+                jobs[i].rows_slot = first + i - 1;
+            }
+            return k_slice(f, store, jobs, cnt);
+        };
+        if (i8) NSPT_TRY(slice_powers(1, 1));
         // powers by doubling: with X^1..X^h known, X^(h+i) = X^h * X^i for i = 1..min(h, s-h)
         for (int h = 1; h < ps;) {
             const int cnt = (ps - h) < h ? (ps - h) : h;
-            GemmGroup gr[12];
-            for (int i = 1; i <= cnt; ++i) {
-                gr[i - 1].A = pw(h);
-                gr[i - 1].B = pw(i);
-                gr[i - 1].out.C = pw(h + i);
+            if (i8) {
+                OzGemmGroup gr[12];
+                for (int i = 1; i <= cnt; ++i) {
+                    gr[i - 1].quad_slot = h - 1;
+                    gr[i - 1].rows_slot = i - 1;
+                    gr[i - 1].A = pw(h);
+                    gr[i - 1].B = pw(i);
+                    gr[i - 1].out.C = pw(h + i);
+                }
+                NSPT_TRY(k_gemm_i8(f, store, gr, cnt));
+                NSPT_TRY(k_retrunc(f, t, cnt * batch, pw(h + 1), pw(h + 1), mb + (size_t)h * modes));
+                NSPT_TRY(slice_powers(h + 1, cnt));
+            } else {
+                GemmGroup gr[12];
+                for (int i = 1; i <= cnt; ++i) {
+                    gr[i - 1].A = pw(h);
+                    gr[i - 1].B = pw(i);
+                    gr[i - 1].out.C = pw(h + i);
+                }
+                NSPT_TRY(k_gemm_groups(f, gr, cnt, batch));
+                NSPT_TRY(k_retrunc(f, t, cnt * batch, pw(h + 1), pw(h + 1)));   // the new powers are contiguous
             }
-            NSPT_TRY(k_gemm_groups(f, gr, cnt, batch));
-            NSPT_TRY(k_retrunc(f, t, cnt * batch, pw(h + 1), pw(h + 1)));   // the new powers are contiguous
             h += cnt;
         }
         {   // all block polynomials in one pass over X^1..X^(s-1)
@@ -526,8 +565,32 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
             GemmOut o;
             o.C = bj(j);
             o.accumulate = true;
-            NSPT_TRY(k_gemm(f, batch, bj(j + 1), pw(ps), o));
-            if (j > 0) NSPT_TRY(k_retrunc(f, t, batch, bj(j), bj(j)));
+            if (i8) {
+                // the left factor: B_{r-1} (no transform has seen it: one max pass) or the re-truncated sum of the previous step
+                unsigned long long* mbl = mb + (size_t)(ps + j + 1) * modes;
+                if (j == pr - 2) {
+                    StageTimer tm;
+                    NSPT_TRY(tm.begin(ST_SLICE));
+                    NSPT_CUDA(launch_ozaki_absmax(f, modes, bj(j + 1), mbl, g.stream));
+                    NSPT_TRY(tm.end());
+                }
+                OzSliceJob job;
+                job.X = bj(j + 1);
+                job.maxbits = mbl;
+                job.quad_slot = ps + j + 1;
+                NSPT_TRY(k_slice(f, store, &job, 1));
+                OzGemmGroup gr;
+                gr.quad_slot = ps + j + 1;
+                gr.rows_slot = ps - 1;
+                gr.A = bj(j + 1);
+                gr.B = pw(ps);
+                gr.out = o;
+                NSPT_TRY(k_gemm_i8(f, store, &gr, 1));
+                if (j > 0) NSPT_TRY(k_retrunc(f, t, batch, bj(j), bj(j), mb + (size_t)(ps + j) * modes));
+            } else {
+                NSPT_TRY(k_gemm(f, batch, bj(j + 1), pw(ps), o));
+                if (j > 0) NSPT_TRY(k_retrunc(f, t, batch, bj(j), bj(j)));
+            }
         }
         return k_inverse(f, t, batch, bj(0), E);
     }

@@ -148,6 +148,8 @@ struct OzSliceJob {
     int quad_slot = -1, rows_slot = -1;             // -1: not needed in that layout
 };
 cudaError_t launch_ozaki_slice(const FreqLayout& f, const OzStore& S, const OzSliceJob* jobs, int njobs, cudaStream_t st);
+// maxbits[mode] = max(maxbits[mode], max over the mode of X) for spectra no transform kernel has written (caller clears)
+cudaError_t launch_ozaki_absmax(const FreqLayout& f, int modes, const double* X, unsigned long long* maxbits, cudaStream_t st);
 struct OzGemmGroup {
     int quad_slot = -1;        // left factor
     int rows_slot = -1;        // right factor

@@ -185,6 +185,30 @@ __global__ void __launch_bounds__(256) oz_slice_kernel(const __grid_constant__ S
     }
 }
 
+// Per-mode maxima of a spectrum that no transform kernel has written (the block polynomials of the series exponential):
+// max(|re|, |im|) as the high word of the bit pattern, one atomicMax per CTA and mode.
+__global__ void __launch_bounds__(256) oz_absmax_kernel(const double2* __restrict__ X, unsigned long long* __restrict__ maxbits,
+                                                      size_t NN, int modes) {
+    __shared__ unsigned int red[8];
+    for (int mode = blockIdx.y; mode < modes; mode += gridDim.y) {   // the grid's y extent is capped at 65535
+        const double2* x = X + (size_t)mode * NN;
+        unsigned int m = 0u;
+        for (size_t e = (size_t)blockIdx.x * 256 + threadIdx.x; e < NN; e += (size_t)gridDim.x * 256) {
+            const unsigned int a = oz_abs_hi(__ldg(&x[e]));
+            m = a > m ? a : m;
+        }
+        m = __reduce_max_sync(0xffffffffu, m);
+        __syncthreads();
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int w = 1; w < 8; ++w) m = red[w] > m ? red[w] : m;
+            if (m) atomicMax(maxbits + mode, (unsigned long long)m << 32);
+        }
+    }
+}
+
 // ---- tcgen05 wrappers ---------------------------------------------------------------------------------------
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -839,6 +863,13 @@ cudaError_t launch_ozaki_slice(const FreqLayout& f, const OzStore& S, const OzSl
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
+}
+
+cudaError_t launch_ozaki_absmax(const FreqLayout& f, int modes, const double* X, unsigned long long* maxbits, cudaStream_t st) {
+    const unsigned chunks = (unsigned)((f.NN + 256 * 8 - 1) / (256 * 8));
+    oz_absmax_kernel<<<dim3(chunks, (unsigned)(modes < 65535 ? modes : 65535)), 256, 0, st>>>(reinterpret_cast<const double2*>(X),
+                                                                                             maxbits, f.NN, modes);
+    return cudaGetLastError();
 }
 
 // Up to OZ_MAX_GROUPS independent products M(p) = A~(p) B~(p) of the same shape in one launch, operands from the slots of

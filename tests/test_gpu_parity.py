@@ -626,6 +626,44 @@ def test_staple_int8_generic_twist_and_aliasing(nspt):
         assert oracle.per_order_error(S[mu].cpu().numpy(), ref[mu], zmax * bounds[mu]).max() <= TOL
 
 
+@pytest.mark.parametrize("N,Ntrunc", [(33, 8), (50, 12), (65, 15), (40, 31)])
+def test_series_exp_int8_tensor_cores(nspt, N, Ntrunc):
+    # Paterson-Stockmeyer exponential with its products on the INT8 tensor cores (forced): powers by doubling (grouped launches,
+    # both slice layouts), accumulating Horner products, maxima from the forward / re-truncation passes and one max pass for the
+    # last block polynomial -- against the oracle's sum of powers
+    import oracle
+    X = anti_hermitian_series(N, Ntrunc, seed=[70, N, Ntrunc])
+    nspt.nspt_set_gemm_variant(2)
+    try:
+        got = gpu_exp(nspt, X)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+    err = oracle.per_order_error(got, oracle.series_exp(X), oracle.exp_bound(X))
+    assert err.max() <= TOL, err.max()
+
+
+def test_series_exp_batched_int8_automatic_choice(nspt):
+    import torch
+    import oracle
+    N, Ntrunc, batch = 200, 15, 2
+    X = np.stack([anti_hermitian_series(N, Ntrunc, seed=[71, b]) for b in range(batch)])
+    nspt.nspt_set_gemm_variant(-1)
+    try:
+        nspt.nspt_profile(True)
+        nspt.nspt_profile_read("int8_slicing")
+        E = nspt.nspt_series_exp_batched(to_dev(X))
+        torch.cuda.synchronize()
+        _, launches = nspt.nspt_profile_read("int8_slicing")
+        nspt.nspt_profile(False)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+    assert launches > 0, "the automatic choice at N = 200, L = 32 is the INT8 path"
+    got = E.cpu().numpy()
+    for b in range(batch):
+        err = oracle.per_order_error(got[b], oracle.series_exp(X[b]), oracle.exp_bound(X[b]))
+        assert err.max() <= TOL, (b, err.max())
+
+
 def test_config4_staple_full_automatic_choice(nspt):
     # BASELINE.json configs[3] through the default kernel choice (INT8 tensor cores at N = 225), both criteria of check_staple
     from paper_2001_02835_b200 import workloads as wl
