@@ -859,44 +859,127 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
             T[k] = spec(15 + k);
             ++k;
         }
-    NSPT_TRY(k_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1]));
-    NSPT_TRY(k_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3]));
+    // FP64 tensor pipe or, from N = 192 (use_int8), INT8 tensor cores -- see staple_device.  Slots of the slice store:
+    //   QUAD (left factors):  U~_d -> d, Ud_mu -> 4, W_q -> 5 + q, T_q -> 8 + q;   ROWS (right factors): Ud_d -> d, U~_d -> 4 + d,
+    //   W_q -> 8 + q, Y_q -> 11 + q
+    const bool i8 = use_int8(f);
+    const int L = f.L;
+    unsigned long long* mb = reinterpret_cast<unsigned long long*>(ws + 30 * sb + WS_PAD);   // [U 0..3][W 0..2][Y 0..2][T 0..2] x L
+    unsigned long long *mbU = mb, *mbW = mb + 4 * L, *mbY = mb + 7 * L, *mbT = mb + 10 * L;
+    OzStore store;
+    if (i8) {
+        store = ozaki_store(f, L, STAPLE_NQ, STAPLE_NR, ws + 30 * sb + WS_PAD + maxbits_bytes(STAPLE_MAXBITS * L));
+        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * 13 * L, g.stream));
+    }
+    auto gemm_groups = [&](const GemmGroup* gr, const int (*slots)[2], int n) -> int {
+        if (!i8) return n == 1 ? k_gemm(f, 1, gr[0].A, gr[0].B, gr[0].out) : k_gemm_groups(f, gr, n);
+        OzGemmGroup og[12];
+        for (int i = 0; i < n; ++i) {
+            og[i].quad_slot = slots[i][0];
+            og[i].rows_slot = slots[i][1];
+            og[i].A = gr[i].A;
+            og[i].B = gr[i].B;
+            og[i].out = gr[i].out;
+        }
+        return k_gemm_i8(f, store, og, n);
+    };
+    {
+        StageTimer tm;
+        NSPT_TRY(tm.begin(ST_FWD));
+        NSPT_CUDA(launch_fft_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1], g.stream, false, i8 ? mbU : nullptr, i8 ? mbU + L : nullptr));
+        NSPT_TRY(tm.end());
+        NSPT_TRY(tm.begin(ST_FWD));
+        NSPT_CUDA(launch_fft_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3], g.stream, false, i8 ? mbU + 2 * L : nullptr,
+                                     i8 ? mbU + 3 * L : nullptr));
+        NSPT_TRY(tm.end());
+    }
     NSPT_TRY(k_dagger(f, 4, Ut[0], Ud[0]));
+    if (i8) {
+        OzSliceJob jobs[8];
+        for (int d = 0; d < 4; ++d) {
+            jobs[d].X = Ut[d];
+            jobs[d].maxbits = mbU + d * L;
+            jobs[d].quad_slot = d;
+            jobs[d].rows_slot = d != mu ? 4 + d : -1;
+            jobs[4 + d].X = Ud[d];
+            jobs[4 + d].maxbits = mbU + d * L;   // |Ud(p)| = |U~((L - p) mod L)|
+            jobs[4 + d].mirror = true;
+            jobs[4 + d].quad_slot = d == mu ? 4 : -1;
+            jobs[4 + d].rows_slot = d;
+        }
+        NSPT_TRY(k_slice(f, store, jobs, 8));
+    }
     {
         GemmGroup gr[6];
+        int sl[6][2];
         for (int q = 0; q < 3; ++q) {
             gr[q].A = Ut[mu];
             gr[q].B = Ud[nus[q]];
             gr[q].out.C = W[q];
+            sl[q][0] = mu;
+            sl[q][1] = nus[q];
             gr[3 + q].A = Ud[mu];
             gr[3 + q].B = Ut[nus[q]];
             gr[3 + q].out.C = Y[q];
+            sl[3 + q][0] = 4;
+            sl[3 + q][1] = 4 + nus[q];
         }
-        NSPT_TRY(k_gemm_groups(f, gr, 6));
-        NSPT_TRY(k_retrunc(f, t, 6, W[0], W[0]));   // W[0..2], Y[0..2] are contiguous
+        NSPT_TRY(gemm_groups(gr, sl, 6));
+        NSPT_TRY(k_retrunc(f, t, 6, W[0], W[0], i8 ? mbW : nullptr));   // W[0..2], Y[0..2] are contiguous (and so are mbW, mbY)
+        if (i8) {
+            OzSliceJob jobs[6];
+            for (int q = 0; q < 3; ++q) {
+                jobs[q].X = W[q];
+                jobs[q].maxbits = mbW + q * L;
+                jobs[q].quad_slot = 5 + q;
+                jobs[q].rows_slot = 8 + q;
+                jobs[3 + q].X = Y[q];
+                jobs[3 + q].maxbits = mbY + q * L;
+                jobs[3 + q].rows_slot = 11 + q;
+            }
+            NSPT_TRY(k_slice(f, store, jobs, 6));
+        }
     }
     {
         GemmGroup gr[3];
+        int sl[3][2];
         for (int q = 0; q < 3; ++q) {
             gr[q].A = Ut[nus[q]];
             gr[q].B = W[q];
             gr[q].out.C = T[q];
+            sl[q][0] = nus[q];
+            sl[q][1] = 8 + q;
         }
-        NSPT_TRY(k_gemm_groups(f, gr, 3));
-        NSPT_TRY(k_retrunc(f, t, 3, T[0], T[0]));
+        NSPT_TRY(gemm_groups(gr, sl, 3));
+        NSPT_TRY(k_retrunc(f, t, 3, T[0], T[0], i8 ? mbT : nullptr));
+        if (i8) {
+            OzSliceJob jobs[3];
+            for (int q = 0; q < 3; ++q) {
+                jobs[q].X = T[q];
+                jobs[q].maxbits = mbT + q * L;
+                jobs[q].quad_slot = 8 + q;
+            }
+            NSPT_TRY(k_slice(f, store, jobs, 3));
+        }
     }
     for (int q = 0; q < 3; ++q) {
         const Cplx zmn{z[4 * mu + nus[q]].re, z[4 * mu + nus[q]].im};
-        GemmOut r;   // S_mu -= z_{mu nu}^* W Y
-        r.C = St;
-        r.alpha = Cplx{-zmn.re, zmn.im};
-        r.accumulate = q > 0;
-        NSPT_TRY(k_gemm(f, 1, W[q], Y[q], r));
-        GemmOut p;   // S_mu += z_{mu nu} (T U_mu^+)^+ : conjugate-transposed accumulate into the mirrored mode
-        p.D = St;
-        p.beta = zmn;
-        p.accumulate_d = true;
-        NSPT_TRY(k_gemm(f, 1, T[q], Ud[mu], p));
+        GemmGroup r;   // S_mu -= z_{mu nu}^* W Y
+        r.A = W[q];
+        r.B = Y[q];
+        r.out.C = St;
+        r.out.alpha = Cplx{-zmn.re, zmn.im};
+        r.out.accumulate = q > 0;
+        const int sr[1][2] = {{5 + q, 11 + q}};
+        NSPT_TRY(gemm_groups(&r, sr, 1));
+        GemmGroup p;   // S_mu += z_{mu nu} (T U_mu^+)^+ : conjugate-transposed accumulate into the mirrored mode
+        p.A = T[q];
+        p.B = Ud[mu];
+        p.out.D = St;
+        p.out.beta = zmn;
+        p.out.accumulate_d = true;
+        const int sp[1][2] = {{8 + q, mu}};
+        NSPT_TRY(gemm_groups(&p, sp, 1));
     }
     return k_inverse(f, t, 1, St, Smu);
 }

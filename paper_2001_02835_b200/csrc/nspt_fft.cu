@@ -24,11 +24,17 @@
 // Data movement.  The kernels are HBM-bound (about 1.5 flop per byte), so what matters is keeping
 // loads in flight while a tile is being transformed.  For L >= 16 the kernels are persistent: each
 // CTA walks over tiles of T elements, and the [order][T] input tile of the tile after next is
-// fetched by one TMA box load (cp.async.bulk.tensor, mbarrier complete_tx) into a two-deep ring of
-// shared-memory stages while the current tile is in registers.  Rows beyond Ntrunc and elements
-// beyond N^2 are zero-filled by TMA, which is exactly the zero padding of Step 1.  Results leave
-// with coalesced 16-byte stores (fire and forget).  L <= 8 needs one thread per element and no
-// shared memory; those kernels use plain loads.
+// fetched by one TMA box load (cp.async.bulk.tensor, mbarrier complete_tx) into a ring of
+// shared-memory stages (three deep in the forward pass, two in the others) while the current tile is
+// in registers.  Rows beyond Ntrunc and elements beyond N^2 are zero-filled by TMA, which is exactly
+// the zero padding of Step 1.  Output tiles are formed in place in the exchange buffer and leave by
+// one TMA box store each (double-buffered in the forward pass).  L <= 8 needs one thread per element
+// and no shared memory; those kernels use plain loads and stores.
+//
+// INT8 product (nspt_ozaki.cu).  The kernels that write spectra (forward, re-truncation) can also
+// record max(|re|, |im|) of every mode they write -- a running maximum of the high words per thread,
+// one redux.sync and one atomicMax per mode and CTA at the end -- which is the scale of the fixed-point
+// slices of that mode.
 #include <map>
 #include <mutex>
 

@@ -7,14 +7,17 @@
 // Arithmetic.  tcgen05.mma has no FP64 kind, so the FP64 tensor path on sm_100a is the warp-level
 // mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4); measured on B200 it sustains the full FP64 pipe rate
 // (37.2 TFLOP/s at 1965 MHz) with 1/8 of the instructions of a DFMA kernel.  The complex product
-// uses the 3-multiplication form on planar operands:
+// uses the 3-multiplication form on the interleaved (re, im) operands:
 //     P1 = Ar Br,  P2 = Ai Bi,  P3 = (Ar+Ai)(Br+Bi);   Cr = P1 - P2,  Ci = P3 - P1 - P2
 // (6 N^3 real flops instead of 8 N^3; normwise stable).  The sums Ar+Ai, Br+Bi are formed on the
-// register fragments (2 DADD per 9 DMMA).
+// register fragments (6 DADD per 27 DMMA).
+// This kernel runs the staple, the exponential and every product below N = 192; from there on
+// nspt_series_mul and friends use the INT8 tensor-core path of nspt_ozaki.cu (same epilogues).
 //
-// Tiling.  CTA tile 48 x 48, four warps in 2 x 2, warp tile 24 x 24 = 3 x 3 DMMA blocks and three
-// accumulator sets (108 registers); 128 threads and 168 registers per thread let three CTAs share an
-// SM (12 warps, 3 per scheduler).  Operands arrive through TMA (cp.async.bulk.tensor, mbarrier
+// Tiling.  Tiling A: CTA tile 48 x 48, four warps in 2 x 2, warp tile 24 x 24 = 3 x 3 DMMA blocks and
+// three accumulator sets (108 registers); 128 threads and 159 registers per thread let three CTAs
+// share an SM (12 warps, 3 per scheduler).  Tiling B: 32 x 32, warp tile 16 x 16, five CTAs per SM,
+// chosen where the 8-row blocks of N do not fill the last 48-tile.  Operands arrive through TMA (cp.async.bulk.tensor, mbarrier
 // complete_tx) in a ring of K-slices of 8; the refill of a slice is issued by the warps in turn, two
 // iterations after the slice was consumed, so nobody waits on it.  Out-of-range rows / columns / k
 // are zero-filled by TMA, so N need not be a multiple of anything; fully out-of-range 8-row /
@@ -22,8 +25,8 @@
 //
 // Shared-memory layout: every operand row is 8 complex128 = 128 bytes, written by TMA with
 // SWIZZLE_128B (16-byte chunk index XOR row index mod 8).  A slice: [m 0..47][k 0..7]; B slice: six
-// blocks [k 0..7][n 0..7], fetched by ONE box of a 4-D view of the operand (encode_operand_b4; seven TMA
-// instructions per slice instead of two cost 2.4 % of the kernel).  Lane (g = lane/4, t = lane%4) loads one complex element (re, im) per
+// blocks [k 0..7][n 0..7], fetched by ONE box of a 4-D view of the operand (encode_operand_b4: two TMA
+// instructions per slice; seven, one per block, cost 2.4 % of the kernel).  Lane (g = lane/4, t = lane%4) loads one complex element (re, im) per
 // fragment with a 16-byte ld.shared; a slice is consumed as two k4 sub-steps whose k-slots are
 // {0,2,4,6} and {1,3,5,7} (any k permutation is legal as long as A and B agree), which makes the
 // eight lanes of every quarter-warp hit eight different 16-byte chunks: no bank conflicts.

@@ -499,8 +499,9 @@ def test_staple_generic_links_and_z(nspt):
     check_staple(nspt, U, z)
 
 
-@pytest.mark.parametrize("N,Ntrunc", [(9, 7), (25, 5), (50, 12), (67, 3)])
-def test_staple_of_one_direction_matches_oracle(nspt, N, Ntrunc):
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("N,Ntrunc", [(9, 7), (25, 5), (50, 12), (67, 3), (65, 8)])
+def test_staple_of_one_direction_matches_oracle(nspt, N, Ntrunc, variant):
     # nspt_staple_dir: the per-GPU unit of the paper's direction split, 15 products per
     # direction, against the literal eq. 2.3 of the oracle and against the four-direction call
     import torch
@@ -512,13 +513,17 @@ def test_staple_of_one_direction_matches_oracle(nspt, N, Ntrunc):
     ref = oracle.staple(U, z)
     bounds = oracle.staple_bound(U)
     Ud = [to_dev(u) for u in U]
-    for mu in range(4):
-        S = nspt.nspt_staple_dir(Ud, z, mu)
-        torch.cuda.synchronize()
-        got = S.cpu().numpy()
-        assert oracle.per_order_error(got, ref[mu], bounds[mu]).max() <= TOL
-        scale = max(np.linalg.norm(ref[mu][k]) for k in range(Ntrunc + 1))
-        assert max(np.linalg.norm(got[k] - ref[mu][k]) for k in range(Ntrunc + 1)) <= STAPLE_REL * scale
+    nspt.nspt_set_gemm_variant(variant)     # 1 = FP64 tensor pipe, 2 = INT8 tensor cores (where L >= 16)
+    try:
+        for mu in range(4):
+            S = nspt.nspt_staple_dir(Ud, z, mu)
+            torch.cuda.synchronize()
+            got = S.cpu().numpy()
+            assert oracle.per_order_error(got, ref[mu], bounds[mu]).max() <= TOL
+            scale = max(np.linalg.norm(ref[mu][k]) for k in range(Ntrunc + 1))
+            assert max(np.linalg.norm(got[k] - ref[mu][k]) for k in range(Ntrunc + 1)) <= STAPLE_REL * scale
+    finally:
+        nspt.nspt_set_gemm_variant(1)
     with pytest.raises(ValueError):
         nspt.nspt_staple_dir(Ud, z, 1, Ud[2])      # the output must not alias a link
 
