@@ -66,7 +66,12 @@ def test_argument_validation_without_a_gpu(lib):
     assert lib.nspt_series_mul_batched(None, None, None, 4, 3, 70000) == -1
     lib.nspt_force.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.c_int]
     assert lib.nspt_force(None, None, 1.0, 4, 3) == -1
+    assert lib.nspt_set_gemm_variant(1) == 0     # FP64 tensor pipe: spectra only
     assert lib.nspt_workspace_bytes(225, 31, 5, 2, ctypes.byref(out)) == 0 and out.value == 5 * 12 * 64 * 225 * 225 * 16 + 256   # Paterson-Stockmeyer: 6 powers + 6 block polynomials, + pad
+    fp64_bytes = out.value
+    assert lib.nspt_set_gemm_variant(-1) == 0    # automatic: INT8 tensor cores at this size, the int8 slice store comes on top
+    assert lib.nspt_workspace_bytes(225, 31, 5, 2, ctypes.byref(out)) == 0 and out.value > fp64_bytes
+    assert lib.nspt_workspace_bytes(100, 31, 1, 0, ctypes.byref(out)) == 0 and out.value == 3 * 64 * 100 * 100 * 16 + 256      # below N = 192: FP64 pipe
     assert lib.nspt_set_order_scale(ctypes.c_double(-1.0)) == -1
     assert lib.nspt_set_gemm_variant(9) == -1 and lib.nspt_set_gemm_variant(-2) == -1 and lib.nspt_set_gemm_variant(1) == 0
     assert b"invalid" in lib.nspt_strerror(-1)
