@@ -46,6 +46,9 @@ struct Context {
     cudaStream_t h2d = nullptr, d2h = nullptr;
     std::vector<cudaEvent_t> copy_events;
     std::vector<Plan> plans;
+    // per-mode maxima of the INT8 product path that are known to be zero (left so by the last product kernel)
+    const void* clean_maxbits = nullptr;
+    size_t clean_maxbits_count = 0;
     // profiling
     bool profiling = false;
     std::vector<ProfEvent> prof_used;
@@ -204,7 +207,7 @@ bool use_int8(const FreqLayout& f) {
 constexpr int STAPLE_NQ = 25, STAPLE_NR = 19, STAPLE_MAXBITS = 22;
 
 // per-mode maxima (one 64-bit pattern per mode) recorded by the transforms for the INT8 path
-size_t maxbits_bytes(int modes) { return align_up((size_t)modes * sizeof(unsigned long long), 256); }
+size_t maxbits_bytes(int modes) { return align_up((size_t)NSPT_MAX_BUCKETS * modes * sizeof(unsigned long long), 256); }   // all copies
 
 size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
     if (op == NSPT_OP_SERIES_MUL && use_int8(f))
@@ -224,13 +227,15 @@ size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
     return 3 * spectrum_bytes(f, batch) + WS_PAD;
 }
 
-int get_workspace(size_t bytes, char** out) {
+int get_workspace(size_t bytes, char** out, bool keeps_maxima = false) {
+    if (!keeps_maxima) g.clean_maxbits = nullptr;   // every caller but the INT8 product overwrites the region of its maxima
     if (g.user_ws) {
         if (g.user_ws_bytes < bytes) return NSPT_ENOMEM;
         *out = static_cast<char*>(g.user_ws);
         return NSPT_OK;
     }
     if (g.own_ws_bytes < bytes) {
+        g.clean_maxbits = nullptr;
         if (g.own_ws) {
             NSPT_CUDA(cudaStreamSynchronize(g.stream));
             NSPT_CUDA(cudaFree(g.own_ws));
@@ -327,13 +332,15 @@ int k_inverse(const FreqLayout& f, const PlanTables& t, int batch, const double*
     return tm.end();
 }
 int k_retrunc(const FreqLayout& f, const PlanTables& t, int batch, const double* src, double* dst,
-              unsigned long long* maxbits = nullptr) {
+              unsigned long long* maxbits = nullptr, size_t maxbits_stride = 0) {
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_RETRUNC));
-    NSPT_CUDA(launch_fft_retruncate(f, t, batch, src, dst, g.stream, maxbits));
+    NSPT_CUDA(launch_fft_retruncate(f, t, batch, src, dst, g.stream, maxbits, maxbits_stride));
     return tm.end();
 }
-int k_slice(const FreqLayout& f, const OzStore& store, const OzSliceJob* jobs, int njobs) {
+// maxbits_stride: distance between the copies of the maxima of the calling operation (all its jobs share it)
+int k_slice(const FreqLayout& f, const OzStore& store, OzSliceJob* jobs, int njobs, size_t maxbits_stride) {
+    for (int i = 0; i < njobs; ++i) jobs[i].maxbits_stride = maxbits_stride;
     StageTimer tm;
     NSPT_TRY(tm.begin(ST_SLICE));
     NSPT_CUDA(launch_ozaki_slice(f, store, jobs, njobs, g.stream));
@@ -406,7 +413,7 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
     PlanTables t;
     NSPT_TRY(get_plan(f.L, f.n, g.order_scale, &t));
     char* ws = nullptr;
-    NSPT_TRY(get_workspace(ws_bytes_for(f, batch, NSPT_OP_SERIES_MUL), &ws));
+    NSPT_TRY(get_workspace(ws_bytes_for(f, batch, NSPT_OP_SERIES_MUL), &ws, use_int8(f)));
     const size_t sb = spectrum_bytes(f, batch);
     double* At = reinterpret_cast<double*>(ws);
     double* Bt = reinterpret_cast<double*>(ws + sb);
@@ -415,13 +422,17 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
         const int modes = batch * f.L;
         unsigned long long* mbA = reinterpret_cast<unsigned long long*>(ws + 3 * sb + WS_PAD);
         unsigned long long* mbB = mbA + modes;
+        const size_t mbs = (size_t)2 * modes, mbn = (size_t)NSPT_MAX_BUCKETS * mbs;   // stride between the copies, all entries
         const OzStore store = ozaki_store(f, modes, 1, 1, ws + 3 * sb + WS_PAD + maxbits_bytes(2 * modes));
         {
             // Steps 1-2 (eqs. 2.6-2.7); the transform also records max(|re|, |im|) of every mode of both spectra
+            // (the maxima start from zero: the product kernel of the previous call has cleared them, else a memset does)
+            if (g.clean_maxbits != mbA || g.clean_maxbits_count != mbn)
+                NSPT_CUDA(cudaMemsetAsync(mbA, 0, sizeof(unsigned long long) * mbn, g.stream));
+            g.clean_maxbits = nullptr;
             StageTimer tm;
             NSPT_TRY(tm.begin(ST_FWD));
-            NSPT_CUDA(cudaMemsetAsync(mbA, 0, sizeof(unsigned long long) * 2 * modes, g.stream));
-            NSPT_CUDA(launch_fft_forward(f, t, batch, A, At, B, Bt, g.stream, false, mbA, mbB));
+            NSPT_CUDA(launch_fft_forward(f, t, batch, A, At, B, Bt, g.stream, false, mbA, mbB, mbs));
             NSPT_TRY(tm.end());
         }
         {
@@ -430,9 +441,11 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
             OzSliceJob jobs[2];
             jobs[0].X = At;
             jobs[0].maxbits = mbA;
+            jobs[0].maxbits_stride = mbs;
             jobs[0].quad_slot = 0;
             jobs[1].X = Bt;
             jobs[1].maxbits = mbB;
+            jobs[1].maxbits_stride = mbs;
             jobs[1].rows_slot = 0;
             StageTimer tm;
             NSPT_TRY(tm.begin(ST_SLICE));
@@ -448,8 +461,10 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
         grp.out.C = Ct;
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_GEMM));
-        NSPT_CUDA(launch_ozaki_gemm(f, store, &grp, 1, g.stream, g.gemm_variant == 4));
+        NSPT_CUDA(launch_ozaki_gemm(f, store, &grp, 1, g.stream, g.gemm_variant == 4, mbA, (int)mbn));
         NSPT_TRY(tm.end());
+        g.clean_maxbits = mbA;
+        g.clean_maxbits_count = mbn;
     } else {
         // Steps 1-2 (eqs. 2.6-2.7): zero-padded forward transforms of A and B, one launch
         NSPT_TRY(k_forward(f, t, batch, A, At, B, Bt));
@@ -497,12 +512,13 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
         char* extra = ws + (size_t)(ps + pr) * sb + WS_PAD;
         mb = reinterpret_cast<unsigned long long*>(extra);
         store = ozaki_store(f, modes, ps + pr, ps, extra + maxbits_bytes((ps + pr) * modes));
-        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * (size_t)(ps + pr) * modes, g.stream));
+        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * NSPT_MAX_BUCKETS * (size_t)(ps + pr) * modes, g.stream));
     }
+    const size_t mbs = (size_t)(ps + pr) * modes;   // distance between the copies of the maxima
     {   // X~ with the coefficient of g^0 taken as zero
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_FWD));
-        NSPT_CUDA(launch_fft_forward(f, t, batch, X, Xt, nullptr, nullptr, g.stream, true, mb, nullptr));
+        NSPT_CUDA(launch_fft_forward(f, t, batch, X, Xt, nullptr, nullptr, g.stream, true, mb, nullptr, mbs));
         NSPT_TRY(tm.end());
     }
     if (ps) {
@@ -516,7 +532,7 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
                 jobs[i].quad_slot = first + i - 1;
                 jobs[i].rows_slot = first + i - 1;
             }
-            return k_slice(f, store, jobs, cnt);
+            return k_slice(f, store, jobs, cnt, mbs);
         };
         if (i8) NSPT_TRY(slice_powers(1, 1));
         // powers by doubling: with X^1..X^h known, X^(h+i) = X^h * X^i for i = 1..min(h, s-h)
@@ -532,7 +548,7 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
                     gr[i - 1].out.C = pw(h + i);
                 }
                 NSPT_TRY(k_gemm_i8(f, store, gr, cnt));
-                NSPT_TRY(k_retrunc(f, t, cnt * batch, pw(h + 1), pw(h + 1), mb + (size_t)h * modes));
+                NSPT_TRY(k_retrunc(f, t, cnt * batch, pw(h + 1), pw(h + 1), mb + (size_t)h * modes, mbs));
                 NSPT_TRY(slice_powers(h + 1, cnt));
             } else {
                 GemmGroup gr[12];
@@ -578,7 +594,7 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
                 job.X = bj(j + 1);
                 job.maxbits = mbl;
                 job.quad_slot = ps + j + 1;
-                NSPT_TRY(k_slice(f, store, &job, 1));
+                NSPT_TRY(k_slice(f, store, &job, 1, mbs));
                 OzGemmGroup gr;
                 gr.quad_slot = ps + j + 1;
                 gr.rows_slot = ps - 1;
@@ -586,7 +602,7 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
                 gr.B = pw(ps);
                 gr.out = o;
                 NSPT_TRY(k_gemm_i8(f, store, &gr, 1));
-                if (j > 0) NSPT_TRY(k_retrunc(f, t, batch, bj(j), bj(j), mb + (size_t)(ps + j) * modes));
+                if (j > 0) NSPT_TRY(k_retrunc(f, t, batch, bj(j), bj(j), mb + (size_t)(ps + j) * modes, mbs));
             } else {
                 NSPT_TRY(k_gemm(f, batch, bj(j + 1), pw(ps), o));
                 if (j > 0) NSPT_TRY(k_retrunc(f, t, batch, bj(j), bj(j)));
@@ -676,6 +692,7 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     const int L = f.L;
     unsigned long long* mb = reinterpret_cast<unsigned long long*>(ws + 30 * sb + WS_PAD);   // [U 0..3][W 0..5][Y 0..5][T 0..5] x L
     unsigned long long *mbU = mb, *mbW = mb + 4 * L, *mbY = mb + 10 * L, *mbT = mb + 16 * L;
+    const size_t mbs = (size_t)STAPLE_MAXBITS * L;   // distance between the copies of the maxima
     OzStore store;
     // slots.  QUAD (left factors): U~_mu -> mu, Ud_mu (mu < 3) -> 4 + mu, W_p -> 7 + p, Y_p -> 13 + p, T_p -> 19 + p;
     //         ROWS (right factors): U~_mu (mu > 0) -> mu - 1, Ud_mu -> 3 + mu, W_p -> 7 + p, Y_p -> 13 + p
@@ -685,7 +702,7 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     auto rUd = [](int mu) { return 3 + mu; };
     if (i8) {
         store = ozaki_store(f, L, STAPLE_NQ, STAPLE_NR, ws + 30 * sb + WS_PAD + maxbits_bytes(STAPLE_MAXBITS * L));
-        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * STAPLE_MAXBITS * L, g.stream));
+        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * NSPT_MAX_BUCKETS * STAPLE_MAXBITS * L, g.stream));
     }
     auto gemm_groups = [&](const GemmGroup* gr, const int (*slots)[2], int n) -> int {
         if (!i8) return k_gemm_groups(f, gr, n);
@@ -702,11 +719,11 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     {
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_FWD));
-        NSPT_CUDA(launch_fft_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1], g.stream, false, i8 ? mbU : nullptr, i8 ? mbU + L : nullptr));
+        NSPT_CUDA(launch_fft_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1], g.stream, false, i8 ? mbU : nullptr, i8 ? mbU + L : nullptr, mbs));
         NSPT_TRY(tm.end());
         NSPT_TRY(tm.begin(ST_FWD));
         NSPT_CUDA(launch_fft_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3], g.stream, false, i8 ? mbU + 2 * L : nullptr,
-                                     i8 ? mbU + 3 * L : nullptr));
+                                     i8 ? mbU + 3 * L : nullptr, mbs));
         NSPT_TRY(tm.end());
     }
     NSPT_TRY(k_dagger(f, 4, Ut[0], Ud[0]));
@@ -723,7 +740,7 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
             jobs[4 + mu].quad_slot = mu < 3 ? qUd(mu) : -1;
             jobs[4 + mu].rows_slot = rUd(mu);
         }
-        NSPT_TRY(k_slice(f, store, jobs, 8));
+        NSPT_TRY(k_slice(f, store, jobs, 8, mbs));
     }
     {   // W_p and Y_p for the six pairs: twelve products, one launch; then one re-truncation pass over all twelve
         GemmGroup gr[12];
@@ -741,7 +758,7 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
             sl[6 + p][1] = rU(pnu[p]);
         }
         NSPT_TRY(gemm_groups(gr, sl, 12));
-        NSPT_TRY(k_retrunc(f, t, 12, W[0], W[0], i8 ? mbW : nullptr));   // W[0..5], Y[0..5] are contiguous (and so are mbW, mbY)
+        NSPT_TRY(k_retrunc(f, t, 12, W[0], W[0], i8 ? mbW : nullptr, mbs));   // W[0..5], Y[0..5] are contiguous (and so are mbW, mbY)
         if (i8) {
             OzSliceJob jobs[12];
             for (int p = 0; p < 6; ++p) {
@@ -754,7 +771,7 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
                 jobs[6 + p].quad_slot = 13 + p;
                 jobs[6 + p].rows_slot = 13 + p;
             }
-            NSPT_TRY(k_slice(f, store, jobs, 12));
+            NSPT_TRY(k_slice(f, store, jobs, 12, mbs));
         }
     }
     {   // T_p = U_nu W_p: six products, one launch, one re-truncation pass
@@ -768,7 +785,7 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
             sl[p][1] = 7 + p;
         }
         NSPT_TRY(gemm_groups(gr, sl, 6));
-        NSPT_TRY(k_retrunc(f, t, 6, T[0], T[0], i8 ? mbT : nullptr));
+        NSPT_TRY(k_retrunc(f, t, 6, T[0], T[0], i8 ? mbT : nullptr, mbs));
         if (i8) {
             OzSliceJob jobs[6];
             for (int p = 0; p < 6; ++p) {
@@ -776,7 +793,7 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
                 jobs[p].maxbits = mbT + p * L;
                 jobs[p].quad_slot = 19 + p;
             }
-            NSPT_TRY(k_slice(f, store, jobs, 6));
+            NSPT_TRY(k_slice(f, store, jobs, 6, mbs));
         }
     }
     // Accumulation into S~: three rounds, each a perfect matching of the four directions, so that the products of
@@ -866,10 +883,11 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
     const int L = f.L;
     unsigned long long* mb = reinterpret_cast<unsigned long long*>(ws + 30 * sb + WS_PAD);   // [U 0..3][W 0..2][Y 0..2][T 0..2] x L
     unsigned long long *mbU = mb, *mbW = mb + 4 * L, *mbY = mb + 7 * L, *mbT = mb + 10 * L;
+    const size_t mbs = (size_t)STAPLE_MAXBITS * L;   // distance between the copies of the maxima
     OzStore store;
     if (i8) {
         store = ozaki_store(f, L, STAPLE_NQ, STAPLE_NR, ws + 30 * sb + WS_PAD + maxbits_bytes(STAPLE_MAXBITS * L));
-        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * 13 * L, g.stream));
+        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * NSPT_MAX_BUCKETS * STAPLE_MAXBITS * L, g.stream));
     }
     auto gemm_groups = [&](const GemmGroup* gr, const int (*slots)[2], int n) -> int {
         if (!i8) return n == 1 ? k_gemm(f, 1, gr[0].A, gr[0].B, gr[0].out) : k_gemm_groups(f, gr, n);
@@ -886,11 +904,11 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
     {
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_FWD));
-        NSPT_CUDA(launch_fft_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1], g.stream, false, i8 ? mbU : nullptr, i8 ? mbU + L : nullptr));
+        NSPT_CUDA(launch_fft_forward(f, t, 1, U[0], Ut[0], U[1], Ut[1], g.stream, false, i8 ? mbU : nullptr, i8 ? mbU + L : nullptr, mbs));
         NSPT_TRY(tm.end());
         NSPT_TRY(tm.begin(ST_FWD));
         NSPT_CUDA(launch_fft_forward(f, t, 1, U[2], Ut[2], U[3], Ut[3], g.stream, false, i8 ? mbU + 2 * L : nullptr,
-                                     i8 ? mbU + 3 * L : nullptr));
+                                     i8 ? mbU + 3 * L : nullptr, mbs));
         NSPT_TRY(tm.end());
     }
     NSPT_TRY(k_dagger(f, 4, Ut[0], Ud[0]));
@@ -907,7 +925,7 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
             jobs[4 + d].quad_slot = d == mu ? 4 : -1;
             jobs[4 + d].rows_slot = d;
         }
-        NSPT_TRY(k_slice(f, store, jobs, 8));
+        NSPT_TRY(k_slice(f, store, jobs, 8, mbs));
     }
     {
         GemmGroup gr[6];
@@ -925,7 +943,7 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
             sl[3 + q][1] = 4 + nus[q];
         }
         NSPT_TRY(gemm_groups(gr, sl, 6));
-        NSPT_TRY(k_retrunc(f, t, 6, W[0], W[0], i8 ? mbW : nullptr));   // W[0..2], Y[0..2] are contiguous (and so are mbW, mbY)
+        NSPT_TRY(k_retrunc(f, t, 6, W[0], W[0], i8 ? mbW : nullptr, mbs));   // W[0..2], Y[0..2] are contiguous (and so are mbW, mbY)
         if (i8) {
             OzSliceJob jobs[6];
             for (int q = 0; q < 3; ++q) {
@@ -937,7 +955,7 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
                 jobs[3 + q].maxbits = mbY + q * L;
                 jobs[3 + q].rows_slot = 11 + q;
             }
-            NSPT_TRY(k_slice(f, store, jobs, 6));
+            NSPT_TRY(k_slice(f, store, jobs, 6, mbs));
         }
     }
     {
@@ -951,7 +969,7 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
             sl[q][1] = 8 + q;
         }
         NSPT_TRY(gemm_groups(gr, sl, 3));
-        NSPT_TRY(k_retrunc(f, t, 3, T[0], T[0], i8 ? mbT : nullptr));
+        NSPT_TRY(k_retrunc(f, t, 3, T[0], T[0], i8 ? mbT : nullptr, mbs));
         if (i8) {
             OzSliceJob jobs[3];
             for (int q = 0; q < 3; ++q) {
@@ -959,7 +977,7 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
                 jobs[q].maxbits = mbT + q * L;
                 jobs[q].quad_slot = 8 + q;
             }
-            NSPT_TRY(k_slice(f, store, jobs, 3));
+            NSPT_TRY(k_slice(f, store, jobs, 3, mbs));
         }
     }
     for (int q = 0; q < 3; ++q) {
@@ -1146,6 +1164,7 @@ int nspt_set_workspace(void* dptr, size_t bytes) {
     NSPT_LOCK();
     if (dptr && (reinterpret_cast<uintptr_t>(dptr) & 255)) return NSPT_EINVAL;
     if (!dptr && bytes) return NSPT_EINVAL;
+    g.clean_maxbits = nullptr;
     g.user_ws = dptr;
     g.user_ws_bytes = dptr ? bytes : 0;
     return NSPT_OK;
@@ -1201,6 +1220,7 @@ int nspt_release(void) {
     if (g.own_ws) cudaFree(g.own_ws);
     g.own_ws = nullptr;
     g.own_ws_bytes = 0;
+    g.clean_maxbits = nullptr;
     if (g.stage_dev) cudaFree(g.stage_dev);
     g.stage_dev = nullptr;
     g.stage_dev_bytes = 0;

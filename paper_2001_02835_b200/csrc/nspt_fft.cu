@@ -157,6 +157,7 @@ struct XformParams {
     // forward / re-truncation, optional (INT8 product): maxbits[z][b * L + p] receives, by atomicMax, the high word (shifted
     // to the high half of a 64-bit pattern) of max(|re|, |im|) over mode p of the spectrum written for operand z
     unsigned long long* maxbits[2];
+    size_t maxbits_stride;         // distance (entries) between the NSPT_MAX_BUCKETS copies of the maxima
 };
 
 // ---- forward phases: registers x[r] = coefficient of order S*r + s (r < R/2 non-zero) -> spectrum.
@@ -387,10 +388,8 @@ __device__ __forceinline__ void forward_phase2_smem(int s, int c, double2* exch,
 #pragma unroll
         for (int p2 = 0; p2 < S; ++p2) {
             exch[(p2 * R + p1) * T + c] = X[p2];
-            if constexpr (TRACK) {   // running maximum of mode p1 + R p2 over the elements this thread has transformed
-                const unsigned int m = oz_abs_hi(X[p2]);
-                if (m > mx[a * S + p2]) mx[a * S + p2] = m;
-            }
+            if constexpr (TRACK)   // running maximum of mode p1 + R p2 over the elements this thread has transformed
+                mx[a * S + p2] = oz_max_hi2(mx[a * S + p2], X[p2]);
         }
     }
 }
@@ -404,7 +403,7 @@ __device__ __forceinline__ void flush_mode_max(unsigned int (&mx)[R], int s, int
     for (int a = 0; a < R / S; ++a)
 #pragma unroll
         for (int p2 = 0; p2 < S; ++p2) {
-            const unsigned int v = __reduce_max_sync(mask, mx[a * S + p2]);
+            const unsigned int v = __reduce_max_sync(mask, mx[a * S + p2]) >> 1;   // the running values carry 2 |x|_hi (oz_max_hi2)
             if (c == 0 && v) atomicMax(dst + ((s + S * a) + R * p2), (unsigned long long)v << 32);
             mx[a * S + p2] = 0u;
         }
@@ -454,6 +453,7 @@ __global__ void __launch_bounds__(T* S, 1) fft_forward_tma_kernel(const __grid_c
 #pragma unroll
     for (int i = 0; i < R; ++i) mx[i] = 0u;
     const bool track = P.maxbits[0] != nullptr;
+    const size_t bucket = (size_t)(blockIdx.x % NSPT_MAX_BUCKETS) * P.maxbits_stride;
     unsigned cur_zb = 0xffffffffu;
     unsigned it = 0;
     for (unsigned tile = blockIdx.x; tile < P.total_tiles; tile += gridDim.x, ++it) {
@@ -464,7 +464,7 @@ __global__ void __launch_bounds__(T* S, 1) fft_forward_tma_kernel(const __grid_c
             const unsigned zb = z * (unsigned)P.batch + b;
             if (zb != cur_zb) {
                 if (cur_zb != 0xffffffffu)
-                    flush_mode_max<R, S, T>(mx, s, c, P.maxbits[cur_zb / (unsigned)P.batch] + (size_t)(cur_zb % (unsigned)P.batch) * C::L);
+                    flush_mode_max<R, S, T>(mx, s, c, P.maxbits[cur_zb / (unsigned)P.batch] + bucket + (size_t)(cur_zb % (unsigned)P.batch) * C::L);
                 cur_zb = zb;
             }
         }
@@ -507,7 +507,7 @@ __global__ void __launch_bounds__(T* S, 1) fft_forward_tma_kernel(const __grid_c
         }
     }
     if (track && cur_zb != 0xffffffffu)
-        flush_mode_max<R, S, T>(mx, s, c, P.maxbits[cur_zb / (unsigned)P.batch] + (size_t)(cur_zb % (unsigned)P.batch) * C::L);
+        flush_mode_max<R, S, T>(mx, s, c, P.maxbits[cur_zb / (unsigned)P.batch] + bucket + (size_t)(cur_zb % (unsigned)P.batch) * C::L);
     if (threadIdx.x == 0) tma_store_wait_read<0>();
 }
 
@@ -566,6 +566,7 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
     }
     unsigned int mx[RETRUNC ? R : 1];   // re-truncation for the INT8 path: running maxima of the modes written (see the forward kernel)
     const bool track = RETRUNC && P.maxbits[0] != nullptr;
+    const size_t bucket = (size_t)(blockIdx.x % NSPT_MAX_BUCKETS) * P.maxbits_stride;
     unsigned cur_b = 0xffffffffu;
     if constexpr (RETRUNC) {
 #pragma unroll
@@ -598,7 +599,7 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
         inverse_from_regs<R, S, T, true>(x, s, c, P.tw_inv, exch, q, twr);
         if constexpr (RETRUNC) {
             if (track && b != cur_b) {   // the spectra of a launch are its batch elements
-                if (cur_b != 0xffffffffu) flush_mode_max<R, S, T>(mx, s, c, P.maxbits[0] + (size_t)cur_b * C::L);
+                if (cur_b != 0xffffffffu) flush_mode_max<R, S, T>(mx, s, c, P.maxbits[0] + bucket + (size_t)cur_b * C::L);
                 cur_b = b;
             }
             double2 xf[R];
@@ -637,7 +638,7 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
         }
     }
     if constexpr (RETRUNC) {
-        if (track && cur_b != 0xffffffffu) flush_mode_max<R, S, T>(mx, s, c, P.maxbits[0] + (size_t)cur_b * C::L);
+        if (track && cur_b != 0xffffffffu) flush_mode_max<R, S, T>(mx, s, c, P.maxbits[0] + bucket + (size_t)cur_b * C::L);
     }
     if (threadIdx.x == 0) tma_store_wait_read<0>();
 }
@@ -820,11 +821,12 @@ bool fft_length_supported(int L) { return L >= 1 && L <= 256 && (L & (L - 1)) ==
 
 cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int batch, const nspt_c128* src0,
                                double* dst0, const nspt_c128* src1, double* dst1, cudaStream_t st, bool skip_order0,
-                               unsigned long long* maxbits0, unsigned long long* maxbits1) {
+                               unsigned long long* maxbits0, unsigned long long* maxbits1, size_t maxbits_stride) {
     XformParams P = base_params(f, t, batch);
     P.skip_order0 = skip_order0 ? 1 : 0;
     P.maxbits[0] = maxbits0;
     P.maxbits[1] = maxbits1 ? maxbits1 : maxbits0;
+    P.maxbits_stride = maxbits_stride;
     P.src_series[0] = reinterpret_cast<const double2*>(src0);
     P.src_series[1] = reinterpret_cast<const double2*>(src1);
     P.dst_freq[0] = reinterpret_cast<double2*>(dst0);
@@ -842,9 +844,10 @@ cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int bat
 }
 
 cudaError_t launch_fft_retruncate(const FreqLayout& f, const PlanTables& t, int batch, const double* src,
-                                  double* dst, cudaStream_t st, unsigned long long* maxbits) {
+                                  double* dst, cudaStream_t st, unsigned long long* maxbits, size_t maxbits_stride) {
     XformParams P = base_params(f, t, batch);
     P.maxbits[0] = P.maxbits[1] = maxbits;
+    P.maxbits_stride = maxbits_stride;
     P.src_freq = reinterpret_cast<const double2*>(src);
     P.dst_freq[0] = reinterpret_cast<double2*>(dst);
     return dispatch(f.L, W_RET, P, 1, st);

@@ -71,7 +71,7 @@ cudaError_t launch_fft_forward(const FreqLayout& f, const PlanTables& t, int bat
                                const nspt_c128* src0, double* dst0,
                                const nspt_c128* src1, double* dst1, cudaStream_t st,
                                bool skip_order0 = false, unsigned long long* maxbits0 = nullptr,
-                               unsigned long long* maxbits1 = nullptr);
+                               unsigned long long* maxbits1 = nullptr, size_t maxbits_stride = 0);
 // Inverse + 1/L + truncation (+ unscale): spectrum -> series.
 cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int batch,
                                const double* src, nspt_c128* dst, cudaStream_t st);
@@ -79,7 +79,12 @@ cudaError_t launch_fft_inverse(const FreqLayout& f, const PlanTables& t, int bat
 // maxbits (optional, INT8 path): [batch][L] entries that receive, by atomicMax, the per-mode maxima of the spectra written
 // (L >= 16 only; the caller clears them).
 cudaError_t launch_fft_retruncate(const FreqLayout& f, const PlanTables& t, int batch,
-                                  const double* src, double* dst, cudaStream_t st, unsigned long long* maxbits = nullptr);
+                                  const double* src, double* dst, cudaStream_t st, unsigned long long* maxbits = nullptr,
+                                  size_t maxbits_stride = 0);
+// The per-mode maxima are kept in NSPT_MAX_BUCKETS copies `maxbits_stride` entries apart: CTA c of a transform kernel updates
+// copy c % NSPT_MAX_BUCKETS (148+ atomicMax on ONE address per mode serialise in L2: 6 us on a 30-60 us transform), the
+// slicing pass takes the maximum over the copies.
+constexpr int NSPT_MAX_BUCKETS = 8;
 // Spectrum of the daggered series: Xd~(p) = (X~((L - p) mod L))^H.
 cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src, double* dst,
                                cudaStream_t st);
@@ -143,7 +148,8 @@ size_t ozaki_store_bytes(const FreqLayout& f, int modes, int nq, int nr);
 OzStore ozaki_store(const FreqLayout& f, int modes, int nq, int nr, void* ws);
 struct OzSliceJob {
     const double* X = nullptr;                      // FP64 spectrum, modes x N x N
-    const unsigned long long* maxbits = nullptr;    // [modes] maxima of the modes of X ...
+    const unsigned long long* maxbits = nullptr;    // [NSPT_MAX_BUCKETS][stride] maxima of the modes of X, entry of mode m at [m] ...
+    size_t maxbits_stride = 0;
     bool mirror = false;                            // ... or of the series X is the dagger spectrum of: mode p takes entry (L - p) % L
     int quad_slot = -1, rows_slot = -1;             // -1: not needed in that layout
 };
@@ -158,6 +164,6 @@ struct OzGemmGroup {
     GemmOut out;
 };
 cudaError_t launch_ozaki_gemm(const FreqLayout& f, const OzStore& S, const OzGemmGroup* groups, int ngroups, cudaStream_t st,
-                              bool pairs = false);
+                              bool pairs = false, unsigned long long* clear = nullptr, int clear_count = 0);
 
 }  // namespace nspt

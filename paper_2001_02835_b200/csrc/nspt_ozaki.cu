@@ -62,6 +62,7 @@ constexpr int OZ_MAX_JOBS = 12;
 struct SliceJobDev {
     const double2* X;
     const unsigned long long* maxbits;
+    size_t maxbits_stride;
     int8_t* quad;      // slot base or null
     int8_t* rows;      // slot base or null
     int* exps_q;
@@ -143,7 +144,13 @@ __global__ void __launch_bounds__(256) oz_slice_kernel(const __grid_constant__ S
             const int p = m % J.mirror_L;
             m = m - p + (J.mirror_L - p) % J.mirror_L;
         }
-        const int e = oz_exponent(J.maxbits[m]);
+        unsigned long long mb = J.maxbits[m];
+#pragma unroll
+        for (int b = 1; b < NSPT_MAX_BUCKETS; ++b) {   // the transforms keep NSPT_MAX_BUCKETS copies (less atomic contention)
+            const unsigned long long o = J.maxbits[m + (size_t)b * J.maxbits_stride];
+            mb = o > mb ? o : mb;
+        }
+        const int e = oz_exponent(mb);
         ssc[threadIdx.x] = oz_pow2(OZ_FRAC_BITS - e);
         if (blockIdx.x == 0) {
             if (quad) J.exps_q[m_begin + threadIdx.x] = e;
@@ -447,6 +454,8 @@ struct OzGroupDev {
 constexpr int OZ_MAX_GROUPS = 12;
 struct OzParams {
     OzGroupDev g[OZ_MAX_GROUPS];
+    unsigned long long* clear;   // per-mode maxima the slicing pass has consumed: zeroed here for the next transform (or null)
+    int clear_count;
     size_t NN;
     int N, L;
     int modes;                 // modes per group (batch * L)
@@ -497,6 +506,8 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
     const uint32_t tmem = *tmem_slot_gen;
     pdl_wait();
     pdl_trigger();
+    if (P.clear && blockIdx.x == 0)   // a memset between two kernels would cost a launch and the programmatic overlap of the next one
+        for (int i = threadIdx.x; i < P.clear_count; i += OZ_THREADS) P.clear[i] = 0ull;
     // barriers of the leader CTA, as shared::cluster addresses (identity for CG = 1)
     const uint32_t lead_full = CG == 2 ? mapa_rank(bar_full, 0) : bar_full;
     const uint32_t lead_acc_empty = CG == 2 ? mapa_rank(bar_acc_empty, 0) : bar_acc_empty;
@@ -747,7 +758,8 @@ cudaError_t oz_maps(const FreqLayout& f, const OzStore& S, int n_rows, CUtensorM
 }
 
 template <int CG>
-cudaError_t launch_oz(const FreqLayout& f, const OzStore& S, const OzGemmGroup* groups, int ngroups, cudaStream_t st) {
+cudaError_t launch_oz(const FreqLayout& f, const OzStore& S, const OzGemmGroup* groups, int ngroups, cudaStream_t st,
+                      unsigned long long* clear, int clear_count) {
     using K = OzCfg<CG>;
     const int N = f.N;
     cudaError_t e;
@@ -764,6 +776,8 @@ cudaError_t launch_oz(const FreqLayout& f, const OzStore& S, const OzGemmGroup* 
     CUtensorMap mapM, mapN;
     if ((e = oz_maps(f, S, K::N_ROWS, &mapM, &mapN)) != cudaSuccess) return e;
     OzParams P{};
+    P.clear = clear;
+    P.clear_count = clear_count;
     P.NN = f.NN;
     P.N = N;
     P.L = f.L;
@@ -841,6 +855,7 @@ cudaError_t launch_ozaki_slice(const FreqLayout& f, const OzStore& S, const OzSl
             SliceJobDev& d = P.job[j];
             d.X = reinterpret_cast<const double2*>(s.X);
             d.maxbits = s.maxbits;
+            d.maxbits_stride = s.maxbits_stride;
             d.quad = s.quad_slot >= 0 ? S.quad + (size_t)s.quad_slot * S.quad_slot_bytes : nullptr;
             d.rows = s.rows_slot >= 0 ? S.rows + (size_t)s.rows_slot * S.rows_slot_bytes : nullptr;
             d.exps_q = s.quad_slot >= 0 ? S.exps_q + (size_t)s.quad_slot * S.modes : nullptr;
@@ -874,11 +889,12 @@ cudaError_t launch_ozaki_absmax(const FreqLayout& f, int modes, const double* X,
 
 // Up to OZ_MAX_GROUPS independent products M(p) = A~(p) B~(p) of the same shape in one launch, operands from the slots of
 // the store (and, for the last N mod 32 <= 2 values of k, from the FP64 spectra they were cut from), epilogues as in
-// nspt_zgemm.cu; pairs = true runs every tile on a CTA pair (tcgen05.mma.cta_group::2)
+// nspt_zgemm.cu; pairs = true runs every tile on a CTA pair (tcgen05.mma.cta_group::2); clear (optional): clear_count per-mode
+// maxima that the slicing pass before this launch has consumed are zeroed for the next transform
 cudaError_t launch_ozaki_gemm(const FreqLayout& f, const OzStore& S, const OzGemmGroup* groups, int ngroups, cudaStream_t st,
-                              bool pairs) {
+                              bool pairs, unsigned long long* clear, int clear_count) {
     if (ngroups < 1 || ngroups > OZ_MAX_GROUPS) return cudaErrorInvalidValue;
-    return pairs ? launch_oz<2>(f, S, groups, ngroups, st) : launch_oz<1>(f, S, groups, ngroups, st);
+    return pairs ? launch_oz<2>(f, S, groups, ngroups, st, clear, clear_count) : launch_oz<1>(f, S, groups, ngroups, st, clear, clear_count);
 }
 
 }  // namespace nspt

@@ -69,6 +69,12 @@ __device__ __forceinline__ unsigned int oz_abs_hi(double2 v) {
     const unsigned int a = (unsigned int)__double2hiint(v.x) & 0x7fffffffu, b = (unsigned int)__double2hiint(v.y) & 0x7fffffffu;
     return a > b ? a : b;
 }
+// running form for the transform kernels: m = max(m, 2 |re|_hi, 2 |im|_hi) -- the sign bit is shifted out instead of masked and
+// the three-way maximum is one instruction; oz_abs_hi_shifted values are halved again when they are flushed
+__device__ __forceinline__ unsigned int oz_max_hi2(unsigned int m, double2 v) {
+    const unsigned int a = (unsigned int)__double2hiint(v.x) << 1, b = (unsigned int)__double2hiint(v.y) << 1;
+    return __vimax3_u32(m, a, b);
+}
 #endif
 
 }  // namespace nspt
