@@ -173,6 +173,45 @@ def test_int8_sliced_product_zero_and_tiny_modes(nspt):
         nspt.nspt_set_gemm_variant(1)
 
 
+def test_int8_path_with_order_scale_caller_workspace_and_second_stream(nspt):
+    # the context calls on the INT8 path: order scale s^k (applied by the transforms around the sliced product), a caller-owned
+    # workspace sized by nspt_workspace_bytes for the selected variant (too small -> NSPT_ENOMEM, no overrun), and a stream
+    # change between two calls (the new stream is ordered after the old one; the cleared-maxima bookkeeping must survive it)
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    A, B = wl.config_product(40, 31, seed=[12, 40, 31])
+    ref = oracle.series_mul(A, B)
+    bound = oracle.product_bound(A, B)
+    dA, dB = to_dev(A), to_dev(B)
+    nspt.nspt_set_gemm_variant(2)
+    side = torch.cuda.Stream()
+    try:
+        need = nspt.nspt_workspace_bytes(40, 31, 1, nspt.NSPT_OP_SERIES_MUL)
+        assert need > 3 * 64 * 40 * 40 * 16 + 256                  # the slice store comes on top of the three spectra
+        ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+        nspt.nspt_set_workspace(ws.data_ptr(), need)
+        for s in (1.0, 0.93, 1.0):
+            nspt.nspt_set_order_scale(s)
+            for _ in range(2):                                       # second call: maxima left clean by the first
+                C = nspt.nspt_series_mul(dA, dB)
+            torch.cuda.synchronize()
+            assert oracle.per_order_error(C.cpu().numpy(), ref, bound).max() <= TOL
+        nspt.nspt_set_stream(side.cuda_stream)
+        C = nspt.nspt_series_mul(dA, dB)
+        side.synchronize()
+        assert oracle.per_order_error(C.cpu().numpy(), ref, bound).max() <= TOL
+        nspt.nspt_set_workspace(ws.data_ptr(), need // 2)
+        with pytest.raises(nspt.NsptError) as ei:
+            nspt.nspt_series_mul(dA, dB)
+        assert ei.value.code == nspt.NSPT_ENOMEM
+    finally:
+        nspt.nspt_set_workspace(None, 0)
+        nspt.nspt_set_order_scale(1.0)
+        nspt.use_current_stream()
+        nspt.nspt_set_gemm_variant(1)
+
+
 @pytest.mark.parametrize("Ntrunc,seed", [(31, 2), (63, 3)])
 def test_automatic_choice_at_configs_2_and_3(nspt, Ntrunc, seed):
     # BASELINE.json configs[1] and [2] through the library's default (automatic) kernel choice -- the INT8 tensor-core path at
