@@ -50,6 +50,7 @@ WORKLOADS = {
     "cfg2": ("product", 225, 31, 1, 2),
     "batched4": ("batched", 225, 31, 4, 2),
     "staple": ("staple", 225, 31, 1, 4),
+    "mdstep": ("mdstep", 225, 31, 1, 4),          # staple + four forces + batched link update: one NSPT update of the four links
     "staple_split": ("staple", 225, 31, 1, 4),     # the paper's direction split: nspt_staple_dir per owned direction + all-gather
     "small": ("product", 9, 7, 1, 0),
     "sweep": ("sweep", 225, 31, 1, 5),
@@ -63,6 +64,7 @@ WORKLOAD_DESC = {
     "cfg2": "single star-product A*B, N=225, N_trunc=31 (L=64), complex128 (BASELINE.json configs[1])",
     "batched4": "batch of 4 star-products, N=225, N_trunc=31 (the four P_mu*U_mu of a link update)",
     "staple": "full TEK staple S_mu, mu=1..4, N=225, N_trunc=31, k=4 twist (BASELINE.json configs[3]); 36 mode-wise products per step (literal eq. 2.3: 52)",
+    "mdstep": "one update of the four TEK links at N=225, N_trunc=31 (PAPER.md:50-55): nspt_staple (36 products), four nspt_force, nspt_link_update_batched U <- exp(i eps F) * U (4 x 11 products); the integrator's momentum update is outside the library, the force series stands in for P",
     "staple_split": "full TEK staple S_mu, mu=1..4, N=225, N_trunc=31, k=4 twist (BASELINE.json configs[3]), directions split over the ranks (PAPER.md:140): 15 mode-wise products per owned direction, one all-gather of the four S_mu per step",
     "small": "single star-product A*B, N=9, N_trunc=7 (BASELINE.json configs[0])",
     "exp": "series exponential exp(X), X anti-Hermitian series, N=225, N_trunc=31 (link-update exponential; 10 mode-wise products, Paterson-Stockmeyer)",
@@ -204,7 +206,7 @@ class ClockSampler:
 
 def make_inputs(kind, N, Ntrunc, batch, seed):
     from paper_2001_02835_b200 import workloads as wl
-    if kind == "staple":
+    if kind in ("staple", "mdstep"):
         U, z = wl.config_staple(N, Ntrunc, seed=seed)
         return {"U": U, "z": z}
     if kind == "batched":
@@ -448,6 +450,25 @@ def run_cuda(args):
                     nspt.nspt_series_exp_batched(X, E)
             products_per_step = exp_products(Ntrunc)
             units_name = "exponentials"
+        elif kind == "mdstep":
+            per_set = 16 * series_bytes
+            R = max(2, int(np.ceil(2 * L2_BYTES / per_set)))
+            U0 = torch.stack([torch.from_numpy(u) for u in inp["U"]]).to(dev)          # (4, n, N, N)
+            sets = []
+            for r in range(R):
+                Ub = U0.roll(r, dims=-1).contiguous() if r else U0
+                sets.append((Ub, [torch.empty_like(Ub[0]) for _ in range(4)], torch.empty_like(Ub), torch.empty_like(Ub)))
+            z = inp["z"]
+            eps_md, c_md = 0.05, 1.0
+
+            def step(i):
+                Ub, S, F, Un = sets[i % R]
+                nspt.nspt_staple([Ub[mu] for mu in range(4)], z, S)
+                for mu in range(4):
+                    nspt.nspt_force(S[mu], c_md, F[mu])
+                nspt.nspt_link_update_batched(F, Ub, eps_md, Un)
+            products_per_step = 36 + 4 * (exp_products(Ntrunc) + 1)
+            units_name = "link_updates"
         elif kind == "staple":
             per_set = 8 * series_bytes
             R = max(2, int(np.ceil(2 * L2_BYTES / per_set)))
@@ -523,7 +544,7 @@ def run_cuda(args):
     ms_local = ev0.elapsed_time(ev1)
     launches = nspt.nspt_launch_count() - launches0
     clocks = sampler.stop()
-    units_per_step = 1 if kind == "staple" else (batch if kind == "exp" else products_per_step)
+    units_per_step = 1 if kind in ("staple", "mdstep") else (batch if kind == "exp" else products_per_step)
     if args.workload == "staple_split":
         units_per_step = 1.0 / world          # the ranks share ONE staple per step (strong scaling)
     value, ms_total = aggregate_throughput(K * units_per_step, ms_local, world, dev)
@@ -549,7 +570,7 @@ def run_cuda(args):
         flops_per_launch = 8.0 * N ** 3 * L * batch
         # a launch may carry several independent products (staple): flops of all mode-wise products of a step
         # over the summed duration of the step's GEMM launches
-        gemm_products_per_step = products_per_step if kind in ("staple", "exp") else 1
+        gemm_products_per_step = products_per_step if kind in ("staple", "exp", "mdstep") else 1
         achieved = (gemm_products_per_step * flops_per_launch * K / (gemm["ms_total"] * 1e-3) * 1e-12) if gemm else None
         traffic = read_traffic(args.workload, "zgemm_modes")
         peaks = {}
@@ -642,6 +663,13 @@ def run_cuda(args):
                 "t_roof_ms": products_per_step * t_gemm_roof * 1e3, "products_executed": products_per_step,
                 "frac": products_per_step * t_gemm_roof / step_s if step_s else None,
             }
+        elif kind == "mdstep":
+            step_s = ms_local / K * 1e-3
+            line_extra["mdstep_roofline"] = {
+                "definition": "the 36 + 4 x 11 mode-wise products of the step (staple; four Paterson-Stockmeyer exponentials and their products with U) of 8*N^3*L flops each at FP64 peak",
+                "t_roof_ms": products_per_step * t_gemm_roof * 1e3, "products_executed": products_per_step,
+                "frac": products_per_step * t_gemm_roof / step_s if step_s else None,
+            }
         elif kind != "staple":
             step_s = ms_local / K * 1e-3
             line_extra["fftconv_roofline"] = {
@@ -703,7 +731,7 @@ def run_cuda(args):
 
     # ---- CPU baseline: the oracle on this box's cores (rank 0, single-GPU runs only)
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline and kind != "exp":
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and kind not in ("exp", "mdstep"):
         import oracle
         if kind == "staple":
             # one of the 52 products of the literal staple, scaled
@@ -751,7 +779,7 @@ def run_cuda(args):
 
     desc = WORKLOAD_DESC[args.workload]
     line = {
-        "metric": {"staple": "tek_staples_per_sec", "exp": "series_exponentials_per_sec"}.get(kind, METRIC),
+        "metric": {"staple": "tek_staples_per_sec", "exp": "series_exponentials_per_sec", "mdstep": "tek_link_updates_per_sec"}.get(kind, METRIC),
         "value": value, "unit": f"{units_name}/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "strong" if args.workload == "staple_split" else "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
@@ -810,7 +838,7 @@ def main():
         args.steps = args.steps if args.steps is not None else 50
         args.warmup = args.warmup if args.warmup is not None else 3
         return run_sweep(args)
-    args.steps = args.steps if args.steps is not None else (200 if args.workload not in ("staple", "exp", "exp4") else 10)
+    args.steps = args.steps if args.steps is not None else (200 if args.workload not in ("staple", "staple_split", "mdstep", "exp", "exp4") else 10)
     args.warmup = args.warmup if args.warmup is not None else 5
     return run_cuda(args)
 

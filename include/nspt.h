@@ -132,6 +132,17 @@ int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc);
 int nspt_series_exp_batched(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int batch);
 
 /*
+ * The link update of the NSPT integrator (U-dot = i P * U, "solved with a symplectic integrator"):
+ *     Unew = exp(i eps P) * U,
+ * P a series of Hermitian coefficients whose g^0 coefficient is NOT read and taken as zero (as in nspt_series_exp), eps the
+ * real step.  One call: the exponential is formed in frequency space as above (the factor i eps only changes the coefficients
+ * (i eps)^m / m!), re-truncated, multiplied by the spectrum of U and transformed back once.  Device pointers,
+ * (Ntrunc+1)*N*N elements each; Unew may alias U or P.  The batched form updates `batch` links (the four directions).
+ */
+int nspt_link_update(const nspt_c128* P, const nspt_c128* U, double eps, nspt_c128* Unew, int N, int Ntrunc);
+int nspt_link_update_batched(const nspt_c128* P, const nspt_c128* U, double eps, nspt_c128* Unew, int N, int Ntrunc, int batch);
+
+/*
  * The force of eq. 2.3 from a staple series, order by order:
  *     F^(k) = i c [ S^(k) - S^(k)+ - Tr(S^(k) - S^(k)+)/N ],   k = 0..Ntrunc,
  * Hermitian and traceless.  c is the real coefficient the paper writes as beta; what is left of it after the

@@ -24,7 +24,7 @@ STAGES = {"fft_forward": 0, "zgemm_modes": 1, "fft_inverse": 2, "fft_retruncate"
           "int8_slicing": 6}
 
 EXPORTS = [
-    "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_staple_dir", "nspt_series_exp", "nspt_series_exp_batched", "nspt_force",
+    "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_staple_dir", "nspt_series_exp", "nspt_series_exp_batched", "nspt_link_update", "nspt_link_update_batched", "nspt_force",
     "nspt_series_mul_host", "nspt_series_mul_batched_host", "nspt_staple_host",
     "nspt_set_stream", "nspt_set_order_scale", "nspt_workspace_bytes", "nspt_set_workspace",
     "nspt_set_gemm_variant", "nspt_set_conv_algorithm", "nspt_probe_fp64_peak", "nspt_profile", "nspt_profile_read", "nspt_launch_count",
@@ -51,6 +51,8 @@ _lib.nspt_staple.argtypes = [ctypes.POINTER(_vp), _vp, ctypes.POINTER(_vp), _int
 _lib.nspt_staple_dir.argtypes = [ctypes.POINTER(_vp), _vp, _int, _vp, _int, _int]
 _lib.nspt_series_exp.argtypes = [_vp, _vp, _int, _int]
 _lib.nspt_series_exp_batched.argtypes = [_vp, _vp, _int, _int, _int]
+_lib.nspt_link_update.argtypes = [_vp, _vp, _dbl, _vp, _int, _int]
+_lib.nspt_link_update_batched.argtypes = [_vp, _vp, _dbl, _vp, _int, _int, _int]
 _lib.nspt_force.argtypes = [_vp, _vp, _dbl, _int, _int]
 _lib.nspt_series_mul_host.argtypes = [_vp, _vp, _vp, _int, _int]
 _lib.nspt_series_mul_batched_host.argtypes = [_vp, _vp, _vp, _int, _int, _int]
@@ -228,6 +230,36 @@ def nspt_series_exp_batched(X, E=None):
     _match(_dev_series(E, "E"), X, "E")
     _check(_lib.nspt_series_exp_batched(X.data_ptr(), E.data_ptr(), N, Ntrunc, batch), "nspt_series_exp_batched")
     return E
+
+
+def nspt_link_update(P, U, eps: float, Unew=None):
+    """Unew = exp(i eps P) * U; P^(0) is not read.  Device tensors, shape (Ntrunc+1, N, N); Unew may alias
+    U or P.  (A stack of links, shape (batch, Ntrunc+1, N, N), is forwarded to nspt_link_update_batched.)"""
+    torch = _torch()
+    P, U = _dev_series(P, "P"), _dev_series(U, "U")
+    if P.dim() == 4:
+        return nspt_link_update_batched(P, U, eps, Unew)
+    _match(U, P, "U")
+    _, Ntrunc, N = _shape(P, False)
+    if Unew is None:
+        Unew = torch.empty_like(U)
+    _match(_dev_series(Unew, "Unew"), P, "Unew")
+    _check(_lib.nspt_link_update(P.data_ptr(), U.data_ptr(), float(eps), Unew.data_ptr(), N, Ntrunc), "nspt_link_update")
+    return Unew
+
+
+def nspt_link_update_batched(P, U, eps: float, Unew=None):
+    """Unew_b = exp(i eps P_b) * U_b for a stack of links (the four directions), shape (batch, Ntrunc+1, N, N)."""
+    torch = _torch()
+    P, U = _dev_series(P, "P"), _dev_series(U, "U")
+    _match(U, P, "U")
+    batch, Ntrunc, N = _shape(P, True)
+    if Unew is None:
+        Unew = torch.empty_like(U)
+    _match(_dev_series(Unew, "Unew"), P, "Unew")
+    _check(_lib.nspt_link_update_batched(P.data_ptr(), U.data_ptr(), float(eps), Unew.data_ptr(), N, Ntrunc, batch),
+           "nspt_link_update_batched")
+    return Unew
 
 
 def nspt_force(S, c: float, F=None):

@@ -221,7 +221,7 @@ size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
         int s, r;
         exp_split(f.n - 1, &s, &r);
         size_t b = (size_t)(s ? s + r : 3) * spectrum_bytes(f, batch) + WS_PAD;
-        if (s && use_int8(f)) b += maxbits_bytes((s + r) * batch * f.L) + ozaki_store_bytes(f, batch * f.L, s + r, s);
+        if (s && use_int8(f)) b += maxbits_bytes((s + r + 1) * batch * f.L) + ozaki_store_bytes(f, batch * f.L, s + r, s);
         return b;
     }
     return 3 * spectrum_bytes(f, batch) + WS_PAD;
@@ -486,9 +486,13 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
 //     epilogue accumulates acc * X^s onto B_j.  s - 1 + r - 1 products instead of n - 1 (10 instead of 30 at n = 31).
 //   n < 6: plain Horner, T_n = 1 + X/n, T_m = 1 + (X * T_{m+1})/m, exp(X) = T_1; the GEMM epilogue scales by 1/m and
 //     adds the identity series (the unit matrix at every mode).
-int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int batch) {
+// With a prefactor lambda and a second series U the same machinery gives E = exp(lambda X) * U without leaving frequency
+// space (the link update U <- exp(i eps P) * U): lambda only changes the coefficients lambda^m / m! of the block
+// polynomials (or the Horner factors), and the product with U~ follows the last Horner step after one re-truncation pass.
+int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int batch, Cplx lambda = Cplx{1.0, 0.0},
+                      const nspt_c128* Umul = nullptr) {
     NSPT_TRY(check_dims(N, Ntrunc, batch));
-    if (!X || !E || !aligned16(X) || !aligned16(E)) return NSPT_EINVAL;
+    if (!X || !E || !aligned16(X) || !aligned16(E) || (Umul && !aligned16(Umul))) return NSPT_EINVAL;
     NSPT_TRY(check_arch());
     const FreqLayout f = make_layout(N, Ntrunc);
     if (!fft_length_supported(f.L)) return NSPT_EINVAL;
@@ -511,10 +515,11 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
     if (i8) {
         char* extra = ws + (size_t)(ps + pr) * sb + WS_PAD;
         mb = reinterpret_cast<unsigned long long*>(extra);
-        store = ozaki_store(f, modes, ps + pr, ps, extra + maxbits_bytes((ps + pr) * modes));
-        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * NSPT_MAX_BUCKETS * (size_t)(ps + pr) * modes, g.stream));
+        store = ozaki_store(f, modes, ps + pr, ps, extra + maxbits_bytes((ps + pr + 1) * modes));
+        NSPT_CUDA(cudaMemsetAsync(mb, 0, sizeof(unsigned long long) * NSPT_MAX_BUCKETS * (size_t)(ps + pr + 1) * modes, g.stream));
     }
-    const size_t mbs = (size_t)(ps + pr) * modes;   // distance between the copies of the maxima
+    const size_t mbs = (size_t)(ps + pr + 1) * modes;   // distance between the copies of the maxima (one extra table: U~)
+    const bool unit_lambda = lambda.re == 1.0 && lambda.im == 0.0;
     {   // X~ with the coefficient of g^0 taken as zero
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_FWD));
@@ -563,17 +568,23 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
             h += cnt;
         }
         {   // all block polynomials in one pass over X^1..X^(s-1)
-            double coef[144];
+            double coef[144], coef_im[144];
             for (int j = 0; j < pr; ++j)
                 for (int i = 0; i < ps; ++i) {
                     const int m = ps * j + i;
-                    long double fct = 1.0L;
-                    for (int q = 2; q <= m; ++q) fct *= q;
-                    coef[j * ps + i] = (m <= Ntrunc) ? (double)(1.0L / fct) : 0.0;
+                    // lambda^m / m!, in long double
+                    long double cr = 1.0L, ci = 0.0L;
+                    for (int q = 1; q <= m; ++q) {
+                        const long double nr = (cr * lambda.re - ci * lambda.im) / q, ni = (cr * lambda.im + ci * lambda.re) / q;
+                        cr = nr;
+                        ci = ni;
+                    }
+                    coef[j * ps + i] = (m <= Ntrunc) ? (double)cr : 0.0;
+                    coef_im[j * ps + i] = (m <= Ntrunc) ? (double)ci : 0.0;
                 }
             StageTimer tm;
             NSPT_TRY(tm.begin(ST_POLY));
-            NSPT_CUDA(launch_freq_block_polys(f, batch, pw(1), bj(0), ps, pr, coef, g.stream));
+            NSPT_CUDA(launch_freq_block_polys(f, batch, pw(1), bj(0), ps, pr, coef, g.stream, unit_lambda ? nullptr : coef_im));
             NSPT_TRY(tm.end());
         }
         // Horner in X^s: acc = B_{r-1}; acc = acc * X^s + B_j for j = r-2 .. 0 (the product is accumulated onto B_j)
@@ -608,13 +619,47 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
                 if (j > 0) NSPT_TRY(k_retrunc(f, t, batch, bj(j), bj(j)));
             }
         }
-        return k_inverse(f, t, batch, bj(0), E);
+        if (!Umul) return k_inverse(f, t, batch, bj(0), E);
+        // exp(lambda X) * U: re-truncate the exponential, transform U into the (free) place of X~, multiply into the place of X^2
+        double* Ut = pw(1);
+        double* Vt = pw(2);
+        if (i8) {
+            unsigned long long* mbE = mb + (size_t)ps * modes;          // B_0's table: not used so far
+            unsigned long long* mbUm = mb + (size_t)(ps + pr) * modes;  // the extra table
+            NSPT_TRY(k_retrunc(f, t, batch, bj(0), bj(0), mbE, mbs));
+            {
+                StageTimer tm;
+                NSPT_TRY(tm.begin(ST_FWD));
+                NSPT_CUDA(launch_fft_forward(f, t, batch, Umul, Ut, nullptr, nullptr, g.stream, false, mbUm, nullptr, mbs));
+                NSPT_TRY(tm.end());
+            }
+            OzSliceJob jobs[2];
+            jobs[0].X = bj(0);
+            jobs[0].maxbits = mbE;
+            jobs[0].quad_slot = ps;
+            jobs[1].X = Ut;
+            jobs[1].maxbits = mbUm;
+            jobs[1].rows_slot = 0;
+            NSPT_TRY(k_slice(f, store, jobs, 2, mbs));
+            OzGemmGroup gr;
+            gr.quad_slot = ps;
+            gr.rows_slot = 0;
+            gr.A = bj(0);
+            gr.B = Ut;
+            gr.out.C = Vt;
+            NSPT_TRY(k_gemm_i8(f, store, &gr, 1));
+        } else {
+            NSPT_TRY(k_retrunc(f, t, batch, bj(0), bj(0)));
+            NSPT_TRY(k_forward(f, t, batch, Umul, Ut, nullptr, nullptr));
+            NSPT_TRY(k_gemm(f, batch, bj(0), Ut, Vt));
+        }
+        return k_inverse(f, t, batch, Vt, E);
     }
     const int n = Ntrunc > 0 ? Ntrunc : 1;
-    {   // T_n = 1 + X/n
+    {   // T_n = 1 + lambda X / n
         StageTimer tm;
         NSPT_TRY(tm.begin(ST_OTHER));
-        NSPT_CUDA(launch_freq_scale_identity(f, batch, Xt, Tt, 1.0 / n, g.stream));
+        NSPT_CUDA(launch_freq_scale_identity(f, batch, Xt, Tt, lambda.re / n, g.stream, lambda.im / n));
         NSPT_TRY(tm.end());
     }
     double* cur = Tt;
@@ -622,15 +667,19 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
     for (int m = n - 1; m >= 1; --m) {
         GemmOut o;
         o.C = other;
-        o.alpha = Cplx{1.0 / m, 0.0};
+        o.alpha = Cplx{lambda.re / m, lambda.im / m};
         o.diag = 1.0;
         NSPT_TRY(k_gemm(f, batch, Xt, cur, o));
-        if (m > 1) NSPT_TRY(k_retrunc(f, t, batch, other, other));
+        if (m > 1 || Umul) NSPT_TRY(k_retrunc(f, t, batch, other, other));
         double* tmp = cur;
         cur = other;
         other = tmp;
     }
-    return k_inverse(f, t, batch, cur, E);
+    if (!Umul) return k_inverse(f, t, batch, cur, E);
+    if (n == 1) NSPT_TRY(k_retrunc(f, t, batch, cur, cur));   // no product has run: 1 + lambda X is already truncated, but keep one code path
+    NSPT_TRY(k_forward(f, t, batch, Umul, Xt, nullptr, nullptr));   // X~ is no longer needed
+    NSPT_TRY(k_gemm(f, batch, cur, Xt, other));
+    return k_inverse(f, t, batch, other, E);
 }
 
 int force_device(const nspt_c128* S, nspt_c128* F, double c, int N, int Ntrunc) {
@@ -1037,6 +1086,18 @@ int nspt_series_exp(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc) {
 int nspt_series_exp_batched(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int batch) {
     NSPT_LOCK();
     return series_exp_device(X, E, N, Ntrunc, batch);
+}
+
+int nspt_link_update(const nspt_c128* P, const nspt_c128* U, double eps, nspt_c128* Unew, int N, int Ntrunc) {
+    NSPT_LOCK();
+    if (!U) return NSPT_EINVAL;
+    return series_exp_device(P, Unew, N, Ntrunc, 1, Cplx{0.0, eps}, U);
+}
+
+int nspt_link_update_batched(const nspt_c128* P, const nspt_c128* U, double eps, nspt_c128* Unew, int N, int Ntrunc, int batch) {
+    NSPT_LOCK();
+    if (!U) return NSPT_EINVAL;
+    return series_exp_device(P, Unew, N, Ntrunc, batch, Cplx{0.0, eps}, U);
 }
 
 int nspt_force(const nspt_c128* S, nspt_c128* F, double c, int N, int Ntrunc) {

@@ -675,14 +675,13 @@ __global__ void __launch_bounds__(256) freq_dagger_kernel(const double2* __restr
 // dst(p) = alpha * src(p) + 1 for every mode p: alpha X + (identity series), whose spectrum is the unit matrix
 // at every mode.  First Horner step of the series exponential.
 __global__ void __launch_bounds__(256) freq_scale_identity_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
-                                                                 int N, size_t NN, double alpha, int modes) {
+                                                                 int N, size_t NN, double alpha, double alpha_im, int modes) {
     const size_t e = (size_t)blockIdx.x * 256 + threadIdx.x;
     if (e >= NN) return;
     for (int m = blockIdx.y; m < modes; m += gridDim.y) {   // the grid's y extent is capped at 65535
         const size_t o = (size_t)m * NN + e;
-        double2 v = src[o];
-        v.x *= alpha;
-        v.y *= alpha;
+        const double2 u = src[o];
+        double2 v = make_double2(alpha * u.x - alpha_im * u.y, alpha * u.y + alpha_im * u.x);
         if (e / N == e % N) v.x += 1.0;
         dst[o] = v;
     }
@@ -862,11 +861,11 @@ cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src
 }
 
 cudaError_t launch_freq_scale_identity(const FreqLayout& f, int batch, const double* src, double* dst, double alpha,
-                                       cudaStream_t st) {
+                                       cudaStream_t st, double alpha_im) {
     const int modes = batch * f.L;
     dim3 grid((unsigned)((f.NN + 255) / 256), (unsigned)(modes < 65535 ? modes : 65535));
     freq_scale_identity_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst),
-                                                     f.N, f.NN, alpha, modes);
+                                                     f.N, f.NN, alpha, alpha_im, modes);
     return cudaGetLastError();
 }
 

@@ -88,9 +88,9 @@ constexpr int NSPT_MAX_BUCKETS = 8;
 // Spectrum of the daggered series: Xd~(p) = (X~((L - p) mod L))^H.
 cudaError_t launch_freq_dagger(const FreqLayout& f, int batch, const double* src, double* dst,
                                cudaStream_t st);
-// dst(p) = alpha * src(p) + 1 (unit matrix) for every mode: spectrum of alpha X + identity series.
+// dst(p) = (alpha + i alpha_im) * src(p) + 1 (unit matrix) for every mode: spectrum of alpha X + identity series.
 cudaError_t launch_freq_scale_identity(const FreqLayout& f, int batch, const double* src, double* dst, double alpha,
-                                       cudaStream_t st);
+                                       cudaStream_t st, double alpha_im = 0.0);
 bool fft_length_supported(int L);
 
 // ---- force projection (nspt_md.cu) -------------------------------------------------------------
@@ -98,8 +98,9 @@ bool fft_length_supported(int L);
 cudaError_t launch_force(const nspt_c128* S, nspt_c128* F, double c, int N, int n, cudaStream_t st);
 // Block polynomials B_j = coef[j][0] 1 + sum_{i=1}^{s-1} coef[j][i] P_i (j < r) of spectra packed back to back:
 // powers = P_1, P_2, ... (s-1 of them), polys = B_0 .. B_{r-1}; s, r <= 12.  Used by the series exponential.
+// coef_im (optional, r x s): imaginary parts of the coefficients (exp(lambda X) with a complex lambda).
 cudaError_t launch_freq_block_polys(const FreqLayout& f, int batch, const double* powers, double* polys, int s, int r,
-                                    const double* coef, cudaStream_t st);
+                                    const double* coef, cudaStream_t st, const double* coef_im = nullptr);
 
 // ---- mode-wise matrix product (nspt_zgemm.cu) -----------------------------------------------
 // For all batch*L modes p, with M(p) = A~(p) B~(p):

@@ -59,6 +59,8 @@ __global__ void __launch_bounds__(256) force_kernel(const double2* __restrict__ 
 // every element of the s-1 powers is read once and the r results are written once.
 struct PolyCoef {
     double c[12][12];
+    double ci[12][12];   // imaginary parts (zero for the plain exponential)
+    int cplx;
 };
 
 __global__ void __launch_bounds__(256) freq_block_polys_kernel(const double2* __restrict__ pw, double2* __restrict__ out,
@@ -70,15 +72,25 @@ __global__ void __launch_bounds__(256) freq_block_polys_kernel(const double2* __
     const bool on_diag = (el / N == el % N);
     double2 acc[12];
 #pragma unroll
-    for (int j = 0; j < 12; ++j) acc[j] = make_double2((on_diag && j < r) ? K.c[j][0] : 0.0, 0.0);
+    for (int j = 0; j < 12; ++j) acc[j] = make_double2((on_diag && j < r) ? K.c[j][0] : 0.0, (on_diag && j < r) ? K.ci[j][0] : 0.0);
     for (int i = 1; i < s; ++i) {
         const double2 v = pw[(size_t)(i - 1) * stride_c + e];
 #pragma unroll
         for (int j = 0; j < 12; ++j) {
             if (j < r) {
+                // warp-uniform branches: for lambda = i eps the coefficients lambda^m / m! are real or imaginary in turn
                 const double w = K.c[j][i];
-                acc[j].x += w * v.x;
-                acc[j].y += w * v.y;
+                if (w != 0.0) {
+                    acc[j].x += w * v.x;
+                    acc[j].y += w * v.y;
+                }
+                if (K.cplx) {
+                    const double wi = K.ci[j][i];
+                    if (wi != 0.0) {
+                        acc[j].x -= wi * v.y;
+                        acc[j].y += wi * v.x;
+                    }
+                }
             }
         }
     }
@@ -90,11 +102,15 @@ __global__ void __launch_bounds__(256) freq_block_polys_kernel(const double2* __
 }  // namespace
 
 cudaError_t launch_freq_block_polys(const FreqLayout& f, int batch, const double* powers, double* polys, int s, int r,
-                                    const double* coef /* r x s, row-major */, cudaStream_t st) {
+                                    const double* coef /* r x s, row-major */, cudaStream_t st, const double* coef_im) {
     if (s < 1 || s > 12 || r < 1 || r > 12) return cudaErrorInvalidValue;
     PolyCoef K{};
+    K.cplx = coef_im ? 1 : 0;
     for (int j = 0; j < r; ++j)
-        for (int i = 0; i < s; ++i) K.c[j][i] = coef[j * s + i];
+        for (int i = 0; i < s; ++i) {
+            K.c[j][i] = coef[j * s + i];
+            K.ci[j][i] = coef_im ? coef_im[j * s + i] : 0.0;
+        }
     const size_t total = (size_t)batch * f.L * f.NN;
     const unsigned grid = (unsigned)((total + 255) / 256);
     freq_block_polys_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(powers), reinterpret_cast<double2*>(polys),

@@ -708,6 +708,52 @@ def test_series_exp_batched_int8_automatic_choice(nspt):
         assert err.max() <= TOL, (b, err.max())
 
 
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("N,Ntrunc,batch", [(5, 0, 1), (9, 3, 1), (12, 5, 2), (33, 8, 1), (50, 12, 3), (40, 31, 1)])
+def test_link_update_matches_oracle(nspt, N, Ntrunc, batch, variant):
+    # nspt_link_update: Unew = exp(i eps P) * U in one call, against the oracle's
+    # series_exp (sum of powers) followed by its star-product; Horner path (Ntrunc < 6), Paterson-Stockmeyer path on the FP64
+    # pipe (variant 1) and on the INT8 tensor cores (variant 2, where L >= 16), single and batched, in place
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([90, N, Ntrunc, batch])
+    eps = 0.37
+    P = np.zeros((batch, Ntrunc + 1, N, N), dtype=np.complex128)
+    for b in range(batch):
+        for k in range(Ntrunc + 1):          # order 0 is filled too: the call must ignore it
+            P[b, k] = wl.hermitian_traceless(N, rng)
+    U = np.stack([wl.unitary_series(N, Ntrunc, rng) for _ in range(batch)])
+    nspt.nspt_set_gemm_variant(variant)
+    try:
+        if batch == 1:
+            dU = to_dev(U[0])
+            out = nspt.nspt_link_update(to_dev(P[0]), dU, eps, dU)      # Unew aliases U
+            torch.cuda.synchronize()
+            got = out.cpu().numpy()[None]
+        else:
+            got = nspt.nspt_link_update(to_dev(P), to_dev(U), eps)
+            torch.cuda.synchronize()
+            got = got.cpu().numpy()
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+    for b in range(batch):
+        X = 1j * eps * P[b]
+        X[0] = 0
+        E = oracle.series_exp(X)
+        ref = oracle.series_mul(E, U[b])
+        # tolerance: the product bound with the exponential's own bound in place of its norms (reading c17 + north star)
+        eb = oracle.exp_bound(X)
+        un = np.sqrt((np.abs(U[b]) ** 2).sum(axis=(1, 2)))
+        bound = np.array([sum(eb[j] * un[k - j] for j in range(k + 1)) for k in range(Ntrunc + 1)])
+        err = oracle.per_order_error(got[b], ref, bound)
+        assert err.max() <= TOL, (b, err.max())
+        # and the result is unitary order by order, like U
+        W = oracle.series_mul(got[b], oracle.dagger(got[b]))
+        W[0] -= np.eye(N)
+        assert np.abs(W).max() <= 1e-10 * max(1.0, np.abs(got[b]).max()) ** 2
+
+
 def test_config4_staple_full_automatic_choice(nspt):
     # BASELINE.json configs[3] through the default kernel choice (INT8 tensor cores at N = 225), both criteria of check_staple
     from paper_2001_02835_b200 import workloads as wl
