@@ -529,15 +529,29 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
     if (ps) {
         auto pw = [&](int i) { return reinterpret_cast<double*>(ws + (size_t)(i - 1) * sb); };     // spectrum of X^i, i = 1..s
         auto bj = [&](int j) { return reinterpret_cast<double*>(ws + (size_t)(ps + j) * sb); };    // B_j, later the Horner sums
-        auto slice_powers = [&](int first, int cnt) -> int {   // X^first .. X^(first+cnt-1) into both layouts
+        // which powers serve as left factors (QUAD layout: the doubling bases X^1, X^2, X^4, ...) and as right factors (ROWS
+        // layout: X^1 .. X^cnt of the later waves, and X^s for the Horner steps); the others are only read by the block polynomials
+        bool left[13] = {}, right[13] = {};
+        for (int h = 1; h < ps;) {
+            const int cnt = (ps - h) < h ? (ps - h) : h;
+            left[h] = true;
+            for (int i = 1; i <= cnt; ++i) right[i] = true;
+            h += cnt;
+        }
+        right[ps] = true;
+        auto slice_powers = [&](int first, int cnt) -> int {   // X^first .. X^(first+cnt-1) into the layouts they are needed in
             OzSliceJob jobs[12];
+            int nj = 0;
             for (int i = 0; i < cnt; ++i) {
-                jobs[i].X = pw(first + i);
-                jobs[i].maxbits = mb + (size_t)(first + i - 1) * modes;
-                jobs[i].quad_slot = first + i - 1;
-                jobs[i].rows_slot = first + i - 1;
+                const int pwr = first + i;
+                if (!left[pwr] && !right[pwr]) continue;
+                jobs[nj].X = pw(pwr);
+                jobs[nj].maxbits = mb + (size_t)(pwr - 1) * modes;
+                jobs[nj].quad_slot = left[pwr] ? pwr - 1 : -1;
+                jobs[nj].rows_slot = right[pwr] ? pwr - 1 : -1;
+                ++nj;
             }
-            return k_slice(f, store, jobs, cnt, mbs);
+            return nj ? k_slice(f, store, jobs, nj, mbs) : NSPT_OK;
         };
         if (i8) NSPT_TRY(slice_powers(1, 1));
         // powers by doubling: with X^1..X^h known, X^(h+i) = X^h * X^i for i = 1..min(h, s-h)

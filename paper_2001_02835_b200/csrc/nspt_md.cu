@@ -59,8 +59,10 @@ __global__ void __launch_bounds__(256) force_kernel(const double2* __restrict__ 
 // every element of the s-1 powers is read once and the r results are written once.
 struct PolyCoef {
     double c[12][12];
-    double ci[12][12];   // imaginary parts (zero for the plain exponential)
-    int cplx;
+};
+struct PolyCoefC {
+    double c[12][12];
+    double ci[12][12];   // imaginary parts: exp(lambda X) with a complex lambda (the link update has lambda = i eps)
 };
 
 __global__ void __launch_bounds__(256) freq_block_polys_kernel(const double2* __restrict__ pw, double2* __restrict__ out,
@@ -72,25 +74,42 @@ __global__ void __launch_bounds__(256) freq_block_polys_kernel(const double2* __
     const bool on_diag = (el / N == el % N);
     double2 acc[12];
 #pragma unroll
+    for (int j = 0; j < 12; ++j) acc[j] = make_double2((on_diag && j < r) ? K.c[j][0] : 0.0, 0.0);
+    for (int i = 1; i < s; ++i) {
+        const double2 v = pw[(size_t)(i - 1) * stride_c + e];
+#pragma unroll
+        for (int j = 0; j < 12; ++j) {
+            if (j < r) {
+                const double w = K.c[j][i];
+                acc[j].x += w * v.x;
+                acc[j].y += w * v.y;
+            }
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 12; ++j)
+        if (j < r) out[(size_t)j * stride_c + e] = acc[j];
+}
+
+// the same with complex coefficients
+__global__ void __launch_bounds__(256) freq_block_polys_cplx_kernel(const double2* __restrict__ pw, double2* __restrict__ out,
+                                                                   size_t stride_c, size_t total, int N, size_t NN, int s, int r,
+                                                                   const __grid_constant__ PolyCoefC K) {
+    const size_t e = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (e >= total) return;
+    const size_t el = e % NN;
+    const bool on_diag = (el / N == el % N);
+    double2 acc[12];
+#pragma unroll
     for (int j = 0; j < 12; ++j) acc[j] = make_double2((on_diag && j < r) ? K.c[j][0] : 0.0, (on_diag && j < r) ? K.ci[j][0] : 0.0);
     for (int i = 1; i < s; ++i) {
         const double2 v = pw[(size_t)(i - 1) * stride_c + e];
 #pragma unroll
         for (int j = 0; j < 12; ++j) {
             if (j < r) {
-                // warp-uniform branches: for lambda = i eps the coefficients lambda^m / m! are real or imaginary in turn
-                const double w = K.c[j][i];
-                if (w != 0.0) {
-                    acc[j].x += w * v.x;
-                    acc[j].y += w * v.y;
-                }
-                if (K.cplx) {
-                    const double wi = K.ci[j][i];
-                    if (wi != 0.0) {
-                        acc[j].x -= wi * v.y;
-                        acc[j].y += wi * v.x;
-                    }
-                }
+                const double w = K.c[j][i], wi = K.ci[j][i];
+                acc[j].x += w * v.x - wi * v.y;
+                acc[j].y += w * v.y + wi * v.x;
             }
         }
     }
@@ -104,17 +123,24 @@ __global__ void __launch_bounds__(256) freq_block_polys_kernel(const double2* __
 cudaError_t launch_freq_block_polys(const FreqLayout& f, int batch, const double* powers, double* polys, int s, int r,
                                     const double* coef /* r x s, row-major */, cudaStream_t st, const double* coef_im) {
     if (s < 1 || s > 12 || r < 1 || r > 12) return cudaErrorInvalidValue;
-    PolyCoef K{};
-    K.cplx = coef_im ? 1 : 0;
-    for (int j = 0; j < r; ++j)
-        for (int i = 0; i < s; ++i) {
-            K.c[j][i] = coef[j * s + i];
-            K.ci[j][i] = coef_im ? coef_im[j * s + i] : 0.0;
-        }
     const size_t total = (size_t)batch * f.L * f.NN;
     const unsigned grid = (unsigned)((total + 255) / 256);
-    freq_block_polys_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(powers), reinterpret_cast<double2*>(polys),
-                                                  total, total, f.N, f.NN, s, r, K);
+    if (coef_im) {
+        PolyCoefC K{};
+        for (int j = 0; j < r; ++j)
+            for (int i = 0; i < s; ++i) {
+                K.c[j][i] = coef[j * s + i];
+                K.ci[j][i] = coef_im[j * s + i];
+            }
+        freq_block_polys_cplx_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(powers), reinterpret_cast<double2*>(polys),
+                                                           total, total, f.N, f.NN, s, r, K);
+    } else {
+        PolyCoef K{};
+        for (int j = 0; j < r; ++j)
+            for (int i = 0; i < s; ++i) K.c[j][i] = coef[j * s + i];
+        freq_block_polys_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(powers), reinterpret_cast<double2*>(polys),
+                                                      total, total, f.N, f.NN, s, r, K);
+    }
     return cudaGetLastError();
 }
 
