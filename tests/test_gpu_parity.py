@@ -212,6 +212,44 @@ def test_int8_path_with_order_scale_caller_workspace_and_second_stream(nspt):
         nspt.nspt_set_gemm_variant(1)
 
 
+@pytest.mark.parametrize("variant", [2, 4])
+def test_int8_path_reads_nothing_it_has_not_written(nspt, variant):
+    # a caller workspace filled with 0xFF bytes (NaN as doubles, -1 as int8 digits, garbage as maxima / exponents): product,
+    # staple, staple of one direction, exponential and link update on the INT8 path must not depend on what was there before --
+    # the k padding of the QUAD layout, the unused eighth slot, the columns beyond N of the ROWS layout, the maxima tables
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng(123)
+    nspt.nspt_set_gemm_variant(variant)
+    try:
+        for (N, Ntrunc) in [(65, 8), (70, 15), (33, 9)]:        # 65 = 2 x 32 + 1: the FP64 tail of K; 70, 33: padded K-chunks
+            A = wl.gaussian_series(N, Ntrunc, rng)
+            B = wl.gaussian_series(N, Ntrunc, rng)
+            need = max(nspt.nspt_workspace_bytes(N, Ntrunc, 1, op) for op in
+                       (nspt.NSPT_OP_SERIES_MUL, nspt.NSPT_OP_STAPLE, nspt.NSPT_OP_SERIES_EXP))
+            ws = torch.full((need,), 0xFF, dtype=torch.uint8, device="cuda")
+            nspt.nspt_set_workspace(ws.data_ptr(), need)
+            check_product(nspt, A, B)
+            ws.fill_(0xFF)
+            U = [wl.unitary_series(N, Ntrunc, rng) for _ in range(4)]
+            z = wl.twist_tensor(7, 2)
+            check_staple(nspt, U, z)
+            ws.fill_(0xFF)
+            ref = oracle.staple(U, z)
+            S2 = nspt.nspt_staple_dir([to_dev(u) for u in U], z, 2)
+            torch.cuda.synchronize()
+            assert oracle.per_order_error(S2.cpu().numpy(), ref[2], oracle.staple_bound(U)[2]).max() <= TOL
+            ws.fill_(0xFF)
+            X = anti_hermitian_series(N, Ntrunc, seed=[124, N])
+            got = gpu_exp(nspt, X)
+            assert oracle.per_order_error(got, oracle.series_exp(X), oracle.exp_bound(X)).max() <= TOL
+            nspt.nspt_set_workspace(None, 0)
+    finally:
+        nspt.nspt_set_workspace(None, 0)
+        nspt.nspt_set_gemm_variant(1)
+
+
 @pytest.mark.parametrize("Ntrunc,seed", [(31, 2), (63, 3)])
 def test_automatic_choice_at_configs_2_and_3(nspt, Ntrunc, seed):
     # BASELINE.json configs[1] and [2] through the library's default (automatic) kernel choice -- the INT8 tensor-core path at
