@@ -14,16 +14,16 @@ extern "C" {
 #endif
 
 /* Select the kernel of the mode-wise matrix product (Step 3):
- *  -1 = automatic (default): nspt_series_mul[_batched] uses the INT8 tensor-core path where it is measured faster and its error
- *       stays far below the tolerance (N >= 192, 32 <= L <= 128), the FP64 tensor-pipe kernel elsewhere,
+ *  -1 = automatic (default): the INT8 tensor-core path where it is measured faster and its error stays far below the
+ *       tolerance (32 <= L <= 128 and N >= 192 for nspt_series_mul[_batched], N >= 160 for the staple, the exponential and the
+ *       link update), the FP64 tensor-pipe kernel elsewhere,
  *   0 = reference kernel (one thread per output element, plain double FMAs; cross-check only),
  *   1 = FP64 tensor-pipe kernel (DMMA, TMA-fed, 3-multiplication complex product) everywhere,
  *   2 = INT8 tensor-core path wherever it exists (L >= 16): the forward transform records the largest element of every
  *       mode, one pass cuts both spectra into seven int8 slices per plane (fixed point relative to that maximum), a
  *       persistent tcgen05.mma.kind::i8 kernel forms the exact INT32 sums in TMEM and recombines them in FP64
- *       (SURVEY.md 8f NEXT-3).  nspt_series_mul[_batched] only; products with scaling / accumulating epilogues (staple,
- *       exponential) stay on kernel 1.  Needs extra workspace (nspt_workspace_bytes reports it for the variant that is
- *       selected when it is called),
+ *       (SURVEY.md 8f NEXT-3), with the scaling / accumulating / conjugate-transposed epilogues the staple and the exponential
+ *       need.  Needs extra workspace (nspt_workspace_bytes reports it for the variant that is selected when it is called),
  *   3 = persistent warp-specialised FP64 tensor-pipe kernel (measured slower than 1; kept as a cross-check),
  *   4 = as 2 with every tile on a CTA pair (tcgen05.mma.cta_group::2, M = 256). */
 int nspt_set_gemm_variant(int variant);

@@ -193,14 +193,17 @@ constexpr size_t WS_PAD = 256;
 
 // Mode-wise product of nspt_series_mul[_batched] on the INT8 tensor cores (nspt_ozaki.cu) or on the FP64 tensor pipe
 // (nspt_zgemm.cu).  Automatic choice, measured on one B200: the INT8 path pays a slicing pass of O(N^2 L) bytes
-// for a product kernel that is about twice as fast, so it wins from N = 192 up; it is limited to L <= 128 (N_trunc <= 63),
-// where its error stays two orders of magnitude below the 1e-11 tolerance on series shaped like the paper's (at N_trunc = 127
-// the margin shrinks to a factor of five: that range stays on the FP64 pipe unless the variant is forced).
-bool use_int8(const FreqLayout& f) {
+// for a product kernel that is about twice as fast, so it wins from N = 192 up -- from N = 160 for the staple and the
+// exponential (`chained`), whose slicing is shared between products and whose grouped launches have no partial last wave
+// (N = 169: staple 3.17 -> 2.94 ms, four exponentials 3.90 -> 3.49 ms; a single product 108 -> 125 us); between 129 and 159 the
+// second 128-column tile is nearly empty and the FP64 pipe wins everywhere.  It is limited to L <= 128 (N_trunc <= 63), where
+// its error stays two orders of magnitude below the 1e-11 tolerance on series shaped like the paper's (at N_trunc = 127 the
+// margin shrinks to a factor of five to eight: that range stays on the FP64 pipe unless the variant is forced).
+bool use_int8(const FreqLayout& f, bool chained = false) {
     if (f.L < 16) return false;   // the slicing pass takes its maxima from the TMA transform kernels
     if (g.gemm_variant == 2 || g.gemm_variant == 4) return true;
     if (g.gemm_variant != -1) return false;
-    return f.N >= 192 && f.L >= 32 && f.L <= 128;
+    return f.N >= (chained ? 160 : 192) && f.L >= 32 && f.L <= 128;
 }
 
 // INT8 staple (staple_device): slice slots per layout and per-mode maxima tables (see the slot maps there)
@@ -214,14 +217,14 @@ size_t ws_bytes_for(const FreqLayout& f, int batch, int op) {
         return 3 * spectrum_bytes(f, batch) + WS_PAD + maxbits_bytes(2 * batch * f.L) + ozaki_store_bytes(f, batch * f.L, 1, 1);
     if (op == NSPT_OP_STAPLE) {
         size_t b = 30 * spectrum_bytes(f, 1) + WS_PAD;
-        if (use_int8(f)) b += maxbits_bytes(STAPLE_MAXBITS * f.L) + ozaki_store_bytes(f, f.L, STAPLE_NQ, STAPLE_NR);
+        if (use_int8(f, true)) b += maxbits_bytes(STAPLE_MAXBITS * f.L) + ozaki_store_bytes(f, f.L, STAPLE_NQ, STAPLE_NR);
         return b;
     }
     if (op == NSPT_OP_SERIES_EXP) {
         int s, r;
         exp_split(f.n - 1, &s, &r);
         size_t b = (size_t)(s ? s + r : 3) * spectrum_bytes(f, batch) + WS_PAD;
-        if (s && use_int8(f)) b += maxbits_bytes((s + r + 1) * batch * f.L) + ozaki_store_bytes(f, batch * f.L, s + r, s);
+        if (s && use_int8(f, true)) b += maxbits_bytes((s + r + 1) * batch * f.L) + ozaki_store_bytes(f, batch * f.L, s + r, s);
         return b;
     }
     return 3 * spectrum_bytes(f, batch) + WS_PAD;
@@ -506,7 +509,7 @@ int series_exp_device(const nspt_c128* X, nspt_c128* E, int N, int Ntrunc, int b
     double* Pt = reinterpret_cast<double*>(ws + 2 * sb);
     int ps, pr;
     exp_split(Ntrunc, &ps, &pr);
-    const bool i8 = ps && use_int8(f);
+    const bool i8 = ps && use_int8(f, true);
     const int modes = batch * f.L;
     // INT8 path (use_int8): per-mode maxima of spectrum i (0-based: X^1..X^s, then B_0..B_{r-1}) and the slice store, QUAD slot
     // = spectrum index (left factors: powers and Horner sums), ROWS slot = power index (right factors: X^1..X^s)
@@ -751,7 +754,7 @@ int staple_device(const nspt_c128* const U[4], const nspt_c128 z[16], nspt_c128*
     // The same launch plan runs on the FP64 tensor pipe or, from N = 192 (use_int8), on the INT8 tensor cores: there every
     // spectrum is also cut into int8 slices -- in the QUAD layout where it is a left factor, in the ROWS layout where it is a
     // right factor (one pass per wave of spectra, both layouts from one read) -- with the per-mode maxima the transforms record.
-    const bool i8 = use_int8(f);
+    const bool i8 = use_int8(f, true);
     const int L = f.L;
     unsigned long long* mb = reinterpret_cast<unsigned long long*>(ws + 30 * sb + WS_PAD);   // [U 0..3][W 0..5][Y 0..5][T 0..5] x L
     unsigned long long *mbU = mb, *mbW = mb + 4 * L, *mbY = mb + 10 * L, *mbT = mb + 16 * L;
@@ -942,7 +945,7 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
     // FP64 tensor pipe or, from N = 192 (use_int8), INT8 tensor cores -- see staple_device.  Slots of the slice store:
     //   QUAD (left factors):  U~_d -> d, Ud_mu -> 4, W_q -> 5 + q, T_q -> 8 + q;   ROWS (right factors): Ud_d -> d, U~_d -> 4 + d,
     //   W_q -> 8 + q, Y_q -> 11 + q
-    const bool i8 = use_int8(f);
+    const bool i8 = use_int8(f, true);
     const int L = f.L;
     unsigned long long* mb = reinterpret_cast<unsigned long long*>(ws + 30 * sb + WS_PAD);   // [U 0..3][W 0..2][Y 0..2][T 0..2] x L
     unsigned long long *mbU = mb, *mbW = mb + 4 * L, *mbY = mb + 7 * L, *mbT = mb + 10 * L;

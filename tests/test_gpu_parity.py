@@ -792,6 +792,27 @@ def test_link_update_matches_oracle(nspt, N, Ntrunc, batch, variant):
         assert np.abs(W).max() <= 1e-10 * max(1.0, np.abs(got[b]).max()) ** 2
 
 
+def test_staple_automatic_choice_at_n169(nspt):
+    # a paper size (Table 3) between the two automatic thresholds: the staple (chained products, N >= 160)
+    # takes the INT8 path, a single product (N >= 192) does not
+    import torch
+    from paper_2001_02835_b200 import workloads as wl
+    U, z = wl.config_staple(169, 15, seed=44, twist_k=3)
+    nspt.nspt_set_gemm_variant(-1)
+    try:
+        nspt.nspt_profile(True)
+        nspt.nspt_profile_read("int8_slicing")
+        check_staple(nspt, U, z)
+        _, staple_launches = nspt.nspt_profile_read("int8_slicing")
+        nspt.nspt_series_mul(to_dev(U[0]), to_dev(U[1]))
+        torch.cuda.synchronize()
+        _, product_launches = nspt.nspt_profile_read("int8_slicing")
+        nspt.nspt_profile(False)
+    finally:
+        nspt.nspt_set_gemm_variant(1)
+    assert staple_launches == 3 and product_launches == 0
+
+
 def test_config4_staple_full_automatic_choice(nspt):
     # BASELINE.json configs[3] through the default kernel choice (INT8 tensor cores at N = 225), both criteria of check_staple
     from paper_2001_02835_b200 import workloads as wl
