@@ -789,6 +789,9 @@ def run_cuda(args):
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
     }
     line.update(line_extra)
+    if "i8" in line.get("roofline", {}).get("kernel", ""):
+        line["dtype_detail"] = ("transforms, slicing and recombination in f64; the mode-wise product in exact integer arithmetic "
+                                "(int8 slices, int32 tensor-core accumulators) that reproduces the f64 product to 2^-50")
     if cpu_baseline is not None:
         line["cpu_baseline"] = cpu_baseline
     print(json.dumps(line))
