@@ -305,7 +305,7 @@ def run_sweep(args):
     nspt.nspt_set_stream(stream.cuda_stream)
     nspt.nspt_set_order_scale(1.0)
     nspt.nspt_set_gemm_variant(args.gemm_variant)
-    fp64_peak = nspt.nspt_probe_fp64_peak()
+    fp64_peak = probe_fp64_peak(nspt)
     peaks = {}
     pfile = ROOT / "MEASURED_PEAKS.json"
     if pfile.exists():
@@ -398,6 +398,16 @@ def run_sweep(args):
 
 
 # ------------------------------------------------------------------------------------ CUDA arm
+
+def probe_fp64_peak(nspt) -> float:
+    """FP64 tensor-pipe peak (TFLOP/s) of this GPU: best of three probe runs a short pause apart, so that a power-capped
+    moment right after the timed loops does not lower the denominator (a lower peak would flatter every fraction)."""
+    best = 0.0
+    for _ in range(3):
+        best = max(best, nspt.nspt_probe_fp64_peak())
+        time.sleep(0.2)
+    return best
+
 
 def run_cuda(args):
     import torch
@@ -565,7 +575,7 @@ def run_cuda(args):
     # ---- roofline of the dominant kernel (mode-wise matrix product)
     line_extra = {}
     if rank == 0:
-        fp64_peak = nspt.nspt_probe_fp64_peak()
+        fp64_peak = probe_fp64_peak(nspt)
         gemm = stage_ms.get("zgemm_modes")
         flops_per_launch = 8.0 * N ** 3 * L * batch
         # a launch may carry several independent products (staple): flops of all mode-wise products of a step
@@ -603,6 +613,8 @@ def run_cuda(args):
         }
         if kind == "exp" and Ntrunc >= 6:
             fft_step_bytes["freq_block_polys"] = poly_bytes
+        if kind == "mdstep":
+            fft_step_bytes = {}       # a mix of the staple's and the exponentials' launches: per-stage bytes are in those workloads' lines
         stages_out = {}
         for name, st in stage_ms.items():
             o = {"launches_per_step": st["launches"] / K, "us_per_launch": st["ms_per_launch"] * 1e3}
@@ -636,11 +648,18 @@ def run_cuda(args):
                 # 8 + 12 + 6 spectra are cut per staple: 18 of them into both layouts (read 16, write 2 x 21 bytes per element), 8 into one
                 fft_step_bytes["int8_slicing"] = (18 * (16 + 42) + 8 * (16 + 21)) * L * N * N
             elif kind == "exp":
-                # X^1..X^s into both layouts, the r-1 Horner left factors into one, and one max pass over B_{r-1}
-                fft_step_bytes["int8_slicing"] = (s_ps * (16 + 42) + (r_ps - 1) * (16 + 21) + 16) * L * N * N * batch
-            else:
+                # the powers in the layouts the products read them in (left factors of the doubling waves X^1, X^2, X^4, ...;
+                # right factors X^1..X^cnt of each wave and X^s), the r-1 Horner left factors, one max pass over B_{r-1}
+                lf, rt, h = set(), {s_ps}, 1
+                while h < s_ps:
+                    cnt = min(s_ps - h, h)
+                    lf.add(h)
+                    rt.update(range(1, cnt + 1))
+                    h += cnt
+                fft_step_bytes["int8_slicing"] = (len(lf & rt) * (16 + 42) + len(lf ^ rt) * (16 + 21) + (r_ps - 1) * (16 + 21) + 16) * L * N * N * batch
+            elif kind != "mdstep":
                 fft_step_bytes["int8_slicing"] = 2 * (16 + 21) * L * N * N * batch   # per operand: read L*e, write 21 bytes per element
-            if "int8_slicing" in stages_out and stage_ms["int8_slicing"]["ms_total"] > 0:
+            if "int8_slicing" in fft_step_bytes and "int8_slicing" in stages_out and stage_ms["int8_slicing"]["ms_total"] > 0:
                 gbs = fft_step_bytes["int8_slicing"] * K / (stage_ms["int8_slicing"]["ms_total"] * 1e-3) * 1e-9
                 stages_out["int8_slicing"].update({"algorithmic_bytes_per_step": fft_step_bytes["int8_slicing"], "algorithmic_GB_s": gbs,
                                                    "frac_of_hbm_peak": gbs / hbm})
@@ -652,7 +671,7 @@ def run_cuda(args):
             "flops_basis": "conventional 8*N^3*L per mode-wise product (all products of a step / summed GEMM launch time); the kernel executes 6*N^3*L (3-multiplication complex product)",
             "achieved_executed": (achieved * 0.75) if achieved else None,
             "frac_executed": (achieved * 0.75 / fp64_peak) if achieved else None,
-            "peak_source": "nspt_probe_fp64_peak: DMMA m8n8k4 chain, measured in this run (MEASURED_PEAKS.json has no FP64 entry)",
+            "peak_source": "nspt_probe_fp64_peak: DMMA m8n8k4 chain, best of 3 in this run (MEASURED_PEAKS.json has no FP64 entry)",
             "hbm_peak_GB_s": hbm, "hbm_peak_source": hbm_src,
           }
         if kind == "exp":
@@ -728,12 +747,51 @@ def run_cuda(args):
         e2e = {"value": e2e_value, "unit": "staples/s", "h2d_bytes_per_step": 4 * series_bytes,
                "d2h_bytes_per_step": 4 * series_bytes, "steps": Ke,
                "how": "nspt_staple_host with pinned host buffers; wall clock around synchronous calls"}
+    elif kind in ("exp", "mdstep") and args.workload != "staple_split":
+        # no _host entry point for these: the caller's own sequence -- pinned host buffers, copies on the library stream
+        # around the device-pointer calls, one stream synchronisation per step
+        d_in, d_out = (sets[0][0], sets[0][1]) if kind == "exp" else (sets[0][0], sets[0][3])
+        h_in = d_in.cpu().pin_memory()
+        h_out = torch.empty_like(h_in).pin_memory()
+
+        def e2e_step():
+            with torch.cuda.stream(stream):
+                d_in.copy_(h_in, non_blocking=True)
+                step(0)
+                h_out.copy_(d_out, non_blocking=True)
+            stream.synchronize()
+        Ke = max(2, min(K, 5))
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(Ke):
+            e2e_step()
+        dt_ms = (time.perf_counter() - t0) * 1e3
+        e2e_value, _ = aggregate_throughput(Ke * units_per_step, dt_ms, world, dev)
+        nbytes = h_in.numel() * 16
+        e2e = {"value": e2e_value, "unit": f"{units_name}/s", "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": Ke,
+               "how": "pinned host buffers copied on the library stream around the device-pointer calls of the step "
+                      "(no _host form of these entry points); wall clock, one stream synchronisation per step"}
 
     # ---- CPU baseline: the oracle on this box's cores (rank 0, single-GPU runs only)
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline and kind not in ("exp", "mdstep"):
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
-        if kind == "staple":
+        if kind in ("exp", "mdstep"):
+            # the oracle's exponential is the Horner form of the Taylor sum: N_trunc - 1 star-products (oracle.series_exp);
+            # the step's CPU cost is estimated from ONE timed oracle product of the same shape
+            X1 = (sets[0][0][0] if (kind == "mdstep" or batch > 1) else sets[0][0]).cpu().numpy()
+            t0 = time.perf_counter()
+            oracle.series_mul(X1, X1)
+            dt = time.perf_counter() - t0
+            horner = max(Ntrunc - 1, 1)
+            nprod = horner * batch if kind == "exp" else 52 + 4 * (horner + 1)
+            cpu_baseline = {"value": (batch if kind == "exp" else 1) / (nprod * dt), "unit": f"{units_name}/s",
+                            "cores": oracle.num_threads(), "kind": "oracle",
+                            "sample": f"1 star-product N={N} N_trunc={Ntrunc} (oracle.series_mul), scaled by the {nprod} products of the "
+                                      + ("oracle's Horner exponential(s)" if kind == "exp" else
+                                         "literal staple (52) and of four Horner exponentials times U")}
+        elif kind == "staple":
             # one of the 52 products of the literal staple, scaled
             t0 = time.perf_counter()
             oracle.series_mul(inp["U"][0], inp["U"][1])
