@@ -74,7 +74,10 @@ struct SliceParams {
     int pitch_q, pitch_r;
     int N, modes;
 };
-constexpr int OZ_SLICE_MODES = 8;   // consecutive modes per thread: the loads of the next mode are in flight while one is cut
+// consecutive modes per CTA: the loads of the second are in flight while the first is cut.  Short CTAs win: 8 modes per CTA
+// (2.5 waves, all CTAs of a wave in step) measured 119 us at config 3, 4: 112, 2: 106, 1: 111; a one-wave persistent kernel
+// 123-136 us (its CTAs load, convert and store in lockstep).
+constexpr int OZ_SLICE_MODES = 2;   // consecutive modes per thread: the loads of the next mode are in flight while one is cut
 // the 21 slice words of four columns of one mode: re and im planes from the fixed-point integers V1, V2, the re + im plane from
 // floor((V1 + V2) / 2) (same accuracy as rounding (re + im) / 2, without a third conversion); w[plane][d] = digit of weight
 // 256^d of the four columns = slice 6 - d
@@ -865,8 +868,9 @@ cudaError_t launch_ozaki_slice(const FreqLayout& f, const OzStore& S, const OzSl
         }
         const int groups = N * (any_quad ? (P.pitch_q >> 5) : ((N + 3) >> 2));   // jobs without a QUAD target leave the rest of the grid at once
         const int my = (S.modes + OZ_SLICE_MODES - 1) / OZ_SLICE_MODES;
+        if (my > 65535) return cudaErrorInvalidValue;
         cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)((groups + 255) / 256), (unsigned)(my < 65535 ? my : 65535), (unsigned)nj);
+        cfg.gridDim = dim3((unsigned)((groups + 255) / 256), (unsigned)my, (unsigned)nj);
         cfg.blockDim = dim3(256, 1, 1);
         cfg.stream = st;
         cudaLaunchAttribute attr[1];
