@@ -15,8 +15,8 @@ extern "C" {
 
 /* Select the kernel of the mode-wise matrix product (Step 3):
  *  -1 = automatic (default): the INT8 tensor-core path where it is measured faster and its error stays far below the
- *       tolerance (32 <= L <= 128 and N >= 192 for nspt_series_mul[_batched], N >= 160 for the staple, the exponential and the
- *       link update), the FP64 tensor-pipe kernel elsewhere,
+ *       tolerance (16 <= L <= 128 and N >= 192; from N >= 160 for the staple, the exponential and the link update where
+ *       L >= 32), the FP64 tensor-pipe kernel elsewhere,
  *   0 = reference kernel (one thread per output element, plain double FMAs; cross-check only),
  *   1 = FP64 tensor-pipe kernel (DMMA, TMA-fed, 3-multiplication complex product) everywhere,
  *   2 = INT8 tensor-core path wherever it exists (L >= 16): the forward transform records the largest element of every

@@ -196,14 +196,16 @@ constexpr size_t WS_PAD = 256;
 // for a product kernel that is about twice as fast, so it wins from N = 192 up -- from N = 160 for the staple and the
 // exponential (`chained`), whose slicing is shared between products and whose grouped launches have no partial last wave
 // (N = 169: staple 3.17 -> 2.94 ms, four exponentials 3.90 -> 3.49 ms; a single product 108 -> 125 us); between 129 and 159 the
-// second 128-column tile is nearly empty and the FP64 pipe wins everywhere.  It is limited to L <= 128 (N_trunc <= 63), where
+// second 128-column tile is nearly empty and the FP64 pipe wins everywhere; at L = 16 (N_trunc <= 7) the threshold is 192 for all
+// operations (N = 225: product 64 -> 56 us, staple 1.66 -> 1.25 ms; N = 169: staple 0.85 -> 0.85 ms, four exponentials 0.43 -> 0.46 ms).
+// It is limited to L <= 128 (N_trunc <= 63), where
 // its error stays two orders of magnitude below the 1e-11 tolerance on series shaped like the paper's (at N_trunc = 127 the
 // margin shrinks to a factor of five to eight: that range stays on the FP64 pipe unless the variant is forced).
 bool use_int8(const FreqLayout& f, bool chained = false) {
     if (f.L < 16) return false;   // the slicing pass takes its maxima from the TMA transform kernels
     if (g.gemm_variant == 2 || g.gemm_variant == 4) return true;
     if (g.gemm_variant != -1) return false;
-    return f.N >= (chained ? 160 : 192) && f.L >= 32 && f.L <= 128;
+    return f.N >= ((chained && f.L >= 32) ? 160 : 192) && f.L <= 128;
 }
 
 // INT8 staple (staple_device): slice slots per layout and per-mode maxima tables (see the slot maps there)
