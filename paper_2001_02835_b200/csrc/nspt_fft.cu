@@ -399,12 +399,24 @@ template <int R, int S, int T>
 __device__ __forceinline__ void flush_mode_max(unsigned int (&mx)[R], int s, int c, unsigned long long* dst) {
     static_assert(T <= 32 && (32 % T) == 0, "T lanes form a part of a warp");
     const unsigned mask = (T == 32) ? 0xffffffffu : (((1u << T) - 1u) << (T * ((threadIdx.x & 31) / T)));
+    // what the table holds already (high words, read from L2; a stale value is a lower one): an atomic is issued only where this
+    // CTA raises the maximum -- the k-th CTA to arrive does so with probability ~1/k, so a mode sees a handful of atomics
+    // instead of one per CTA
+    // (measured: L = 128 forward pass 60 -> 57 us; at L <= 32 a CTA lives for two or three tiles and the extra L2 round trip
+    // costs more than it saves, 17 -> 19 us at L = 16, so short transforms issue their atomics unconditionally)
+    constexpr bool PEEK = R * S >= 128;
+    unsigned int cur[R];
+#pragma unroll
+    for (int a = 0; a < R / S; ++a)
+#pragma unroll
+        for (int p2 = 0; p2 < S; ++p2)
+            cur[a * S + p2] = (PEEK && c == 0) ? __ldcg(reinterpret_cast<const unsigned int*>(dst + ((s + S * a) + R * p2)) + 1) : 0u;
 #pragma unroll
     for (int a = 0; a < R / S; ++a)
 #pragma unroll
         for (int p2 = 0; p2 < S; ++p2) {
             const unsigned int v = __reduce_max_sync(mask, mx[a * S + p2]) >> 1;   // the running values carry 2 |x|_hi (oz_max_hi2)
-            if (c == 0 && v) atomicMax(dst + ((s + S * a) + R * p2), (unsigned long long)v << 32);
+            if (c == 0 && v > cur[a * S + p2]) atomicMax(dst + ((s + S * a) + R * p2), (unsigned long long)v << 32);
             mx[a * S + p2] = 0u;
         }
 }

@@ -351,6 +351,29 @@ __device__ __forceinline__ void tc_commit_cg(uint32_t bar) {
     }
 }
 // TMA loads whose completion is reported to a barrier that may live in the peer CTA (the leader's)
+// The slices are streamed once (each operand tile is read by the two to five CTAs that need it at about the same time) while
+// the C~ the epilogues write is read back by the next kernel: the operand loads carry an L2 evict_first policy (1-2 % measured).
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void tma_load_4d_hint(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3,
+                                                 uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5, %6}], "
+        "[%2], %7;" ::"r"(dst),
+        "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_5d_hint(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3,
+                                                 int c4, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5, %6, "
+        "%7}], [%2], %8;" ::"r"(dst),
+        "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "l"(policy)
+        : "memory");
+}
 template <int CG>
 __device__ __forceinline__ void tma_load_4d_cg(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3) {
     if constexpr (CG == 2) {
@@ -521,6 +544,7 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
             // ------------------------------------------------------------ TMA producer (one thread per CTA)
             if (lane == 0) {
                 int it = 0;
+                const uint64_t policy = l2_policy_evict_first();
                 for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
                     const int gm = tile / tiles_per_mode, rem = tile % tiles_per_mode;   // gm = group * modes + mode
                     const int grp = gm / P.modes, mode = gm % P.modes;
@@ -533,8 +557,13 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                             mbar_wait_wd(bar_empty + 8 * slot, ((it / K::STAGES) & 1) ^ 1);
                             if (rank == 0) mbar_expect_tx(bar_full + 8 * slot, K::STAGE * CG);
                             const uint32_t st = base + slot * K::STAGE;
-                            tma_load_4d_cg<CG>(st, &mapM, lead_full + 8 * slot, j0, kc * OZ_KC, 0, pb + plane);
-                            tma_load_5d_cg<CG>(st + OZ_M_STAGE, &mapN, lead_full + 8 * slot, 0, i0, 0, kc, pa + plane);
+                            if constexpr (CG == 1) {
+                                tma_load_4d_hint(st, &mapM, bar_full + 8 * slot, j0, kc * OZ_KC, 0, pb + plane, policy);
+                                tma_load_5d_hint(st + OZ_M_STAGE, &mapN, bar_full + 8 * slot, 0, i0, 0, kc, pa + plane, policy);
+                            } else {
+                                tma_load_4d_cg<CG>(st, &mapM, lead_full + 8 * slot, j0, kc * OZ_KC, 0, pb + plane);
+                                tma_load_5d_cg<CG>(st + OZ_M_STAGE, &mapN, lead_full + 8 * slot, 0, i0, 0, kc, pa + plane);
+                            }
                         }
                     }
                 }
@@ -573,6 +602,30 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
         // lane of the accumulator = output column j, column of the accumulator = output row i
         const int we = warp - 4, quarter = we & 3, half = we >> 2;
         int acc_it = 0;
+        // What a tile needs from global memory before its first drain -- the exponents of its mode and, for the tail of K
+        // (k >= 32 nkc, added in FP64), lane l's element A~[row0 + l][k] and its own column of B~[k][.] -- is fetched BEFORE the
+        // stores of the tile before it: behind 131 KB of stores per SM these loads waited 2800 cycles on the critical path.
+        int esum_next = 0;
+        double2 at_next[OZ_TAIL_MAX], bt_next[OZ_TAIL_MAX];
+        auto prefetch = [&](int tile) {
+            if (tile >= P.total_tiles) return;
+            const int gm = tile / tiles_per_mode, rem = tile % tiles_per_mode;
+            const int mode = gm % P.modes;
+            const OzGroupDev& G = P.g[gm / P.modes];
+            const int row0 = (rem / P.tiles_j) * OZ_BN + 32 * half;
+            const int col = (rem % P.tiles_j) * (OZ_BM * CG) + (int)rank * OZ_BM + 32 * quarter + lane;
+            esum_next = __ldg(G.expA + mode) + __ldg(G.expB + mode);
+#pragma unroll
+            for (int t = 0; t < OZ_TAIL_MAX; ++t) {
+                at_next[t] = bt_next[t] = make_double2(0.0, 0.0);
+                if (t < P.tail) {
+                    const int k = OZ_KC * nkc + t;
+                    if (row0 + lane < P.N) at_next[t] = __ldg(G.At + (size_t)mode * P.NN + (size_t)(row0 + lane) * P.N + k);
+                    if (col < P.N) bt_next[t] = __ldg(G.Bt + (size_t)mode * P.NN + (size_t)k * P.N + col);
+                }
+            }
+        };
+        prefetch(cluster_id);
         for (int tile = cluster_id; tile < P.total_tiles; tile += nclusters) {
             const int gm = tile / tiles_per_mode, rem = tile % tiles_per_mode;
             const int mode = gm % P.modes;
@@ -580,26 +633,24 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
             const int row0 = (rem / P.tiles_j) * OZ_BN + 32 * half;
             const int col = (rem % P.tiles_j) * (OZ_BM * CG) + (int)rank * OZ_BM + 32 * quarter + lane;
             double re[32], im[32];
-            const int esum = G.expA[mode] + G.expB[mode];
+            const int esum = esum_next;
             const double sc = esum >= (1 << 20) ? __longlong_as_double(0x7ff8000000000000ll) : oz_pow2(esum - 12);
-            // The tail of K (k >= 32 nkc) in FP64, while the MMAs of the first plane run: lane l fetches A~[row0 + l][k] and its
-            // own column of B~[k][.]; the running sums start from the tail product in units of the common scale (a power of two)
+            // the running sums start from the tail product in units of the common scale (a power of two)
 #pragma unroll
             for (int j = 0; j < 32; ++j) re[j] = im[j] = 0.0;
             if (P.tail) {
                 const double isc = oz_pow2(12 - esum);
-                for (int t = 0; t < P.tail; ++t) {
-                    const int k = OZ_KC * nkc + t;
-                    double2 at = make_double2(0.0, 0.0), bt = make_double2(0.0, 0.0);
-                    if (row0 + lane < P.N) at = __ldg(G.At + (size_t)mode * P.NN + (size_t)(row0 + lane) * P.N + k);
-                    if (col < P.N) bt = __ldg(G.Bt + (size_t)mode * P.NN + (size_t)k * P.N + col);
-                    bt.x *= isc;
-                    bt.y *= isc;
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const double ax = __shfl_sync(0xffffffffu, at.x, j), ay = __shfl_sync(0xffffffffu, at.y, j);
-                        re[j] = fma(ax, bt.x, fma(-ay, bt.y, re[j]));
-                        im[j] = fma(ax, bt.y, fma(ay, bt.x, im[j]));
+                for (int t = 0; t < OZ_TAIL_MAX; ++t) {
+                    if (t < P.tail) {
+                        const double2 at = at_next[t];
+                        const double2 bt = make_double2(bt_next[t].x * isc, bt_next[t].y * isc);
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) {
+                            const double ax = __shfl_sync(0xffffffffu, at.x, j), ay = __shfl_sync(0xffffffffu, at.y, j);
+                            re[j] = fma(ax, bt.x, fma(-ay, bt.y, re[j]));
+                            im[j] = fma(ax, bt.y, fma(ay, bt.x, im[j]));
+                        }
                     }
                 }
             }
@@ -641,6 +692,7 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                     if (CG == 2) mbar_arrive_cluster(lead_acc_empty); else mbar_arrive(bar_acc_empty);
                 }
             }
+            prefetch(tile + nclusters);
             // scaling, epilogue and stores overlap the MMAs of the next tile
             if (col < P.N) {
                 if (G.C) {
