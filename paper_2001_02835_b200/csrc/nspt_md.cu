@@ -75,14 +75,23 @@ __global__ void __launch_bounds__(256) freq_block_polys_kernel(const double2* __
     double2 acc[12];
 #pragma unroll
     for (int j = 0; j < 12; ++j) acc[j] = make_double2((on_diag && j < r) ? K.c[j][0] : 0.0, 0.0);
-    for (int i = 1; i < s; ++i) {
-        const double2 v = pw[(size_t)(i - 1) * stride_c + e];
+    // all loads of a group of four powers are issued before the first is used (with a plain loop over i every load waited for the
+    // arithmetic of the one before)
+    for (int i0 = 1; i0 < s; i0 += 4) {
+        double2 v[4];
 #pragma unroll
-        for (int j = 0; j < 12; ++j) {
-            if (j < r) {
-                const double w = K.c[j][i];
-                acc[j].x += w * v.x;
-                acc[j].y += w * v.y;
+        for (int u = 0; u < 4; ++u) v[u] = (i0 + u < s) ? __ldcs(&pw[(size_t)(i0 + u - 1) * stride_c + e]) : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (i0 + u < s) {
+#pragma unroll
+                for (int j = 0; j < 12; ++j) {
+                    if (j < r) {
+                        const double w = K.c[j][i0 + u];
+                        acc[j].x += w * v[u].x;
+                        acc[j].y += w * v[u].y;
+                    }
+                }
             }
         }
     }
@@ -102,14 +111,21 @@ __global__ void __launch_bounds__(256) freq_block_polys_cplx_kernel(const double
     double2 acc[12];
 #pragma unroll
     for (int j = 0; j < 12; ++j) acc[j] = make_double2((on_diag && j < r) ? K.c[j][0] : 0.0, (on_diag && j < r) ? K.ci[j][0] : 0.0);
-    for (int i = 1; i < s; ++i) {
-        const double2 v = pw[(size_t)(i - 1) * stride_c + e];
+    for (int i0 = 1; i0 < s; i0 += 4) {
+        double2 v[4];
 #pragma unroll
-        for (int j = 0; j < 12; ++j) {
-            if (j < r) {
-                const double w = K.c[j][i], wi = K.ci[j][i];
-                acc[j].x += w * v.x - wi * v.y;
-                acc[j].y += w * v.y + wi * v.x;
+        for (int u = 0; u < 4; ++u) v[u] = (i0 + u < s) ? __ldcs(&pw[(size_t)(i0 + u - 1) * stride_c + e]) : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (i0 + u < s) {
+#pragma unroll
+                for (int j = 0; j < 12; ++j) {
+                    if (j < r) {
+                        const double w = K.c[j][i0 + u], wi = K.ci[j][i0 + u];
+                        acc[j].x += w * v[u].x - wi * v[u].y;
+                        acc[j].y += w * v[u].y + wi * v[u].x;
+                    }
+                }
             }
         }
     }
