@@ -124,7 +124,9 @@ def test_reference_variant_agrees_with_tensor_core_variant(nspt):
 
 @pytest.mark.parametrize("variant", [2, 4])
 @pytest.mark.parametrize("N,Ntrunc", [(1, 0), (3, 2), (9, 7), (9, 8), (31, 12), (50, 12), (64, 15), (65, 8), (100, 31), (129, 9), (225, 7),
-                                      (257, 8), (33, 63)])
+                                      (257, 8), (33, 63),
+                                      # K-tail of two columns (N mod 32 = 2), K a whole number of chunks, three j-tiles
+                                      (66, 9), (130, 5), (96, 8), (224, 3), (290, 2)])
 def test_int8_sliced_product_matches_oracle(nspt, N, Ntrunc, variant):
     # the mode-wise product on tcgen05.mma.kind::i8 with exact INT32 accumulation of seven int8 slices
     # per operand plane; same tolerance as the FP64 tensor-pipe kernel.  (L < 16 has no INT8 path and runs on the FP64 pipe.)
