@@ -66,7 +66,8 @@ enum {
     NSPT_EINVAL = -1,  /* null / misaligned pointer, N < 1, Ntrunc < 0, batch < 1, Ntrunc > NSPT_MAX_NTRUNC */
     NSPT_ENOMEM = -2,  /* device or host allocation failed, or caller workspace too small */
     NSPT_ECUDA = -3,   /* CUDA runtime / launch error (text: nspt_strerror) */
-    NSPT_EARCH = -4    /* current device is not compute capability 10.x */
+    NSPT_EARCH = -4,   /* current device is not compute capability 10.x */
+    NSPT_ETOOBIG = -5  /* nspt_series_mul_noalloc: the problem does not fit the static scratch array */
 };
 
 enum { NSPT_OP_SERIES_MUL = 0, NSPT_OP_STAPLE = 1, NSPT_OP_SERIES_EXP = 2 };
@@ -94,6 +95,23 @@ int nspt_series_mul(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N,
  */
 int nspt_series_mul_batched(const nspt_c128* A, const nspt_c128* B, nspt_c128* C,
                             int N, int Ntrunc, int batch);
+
+/*
+ * nspt_series_mul for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the same FFT-CONV (Steps 1-5, eqs. 2.6-2.9) by the same kernels on the FP64 tensor
+ * pipe, with the three spectra A~, B~, C~ and the per-L tables in a static device array of NSPT_NOALLOC_SCRATCH_BYTES
+ * inside the library instead of the workspace.  The call runs no cudaMalloc, cudaFree or other allocating routine; every
+ * GPU that loads the library holds the array until the process exits.
+ * A, B, C: device pointers as for nspt_series_mul (C may be one of the inputs); asynchronous on the library stream; the
+ * order scale of nspt_set_order_scale applies; nspt_set_gemm_variant, nspt_set_conv_algorithm and nspt_set_workspace do not.
+ * Limit: 3 * 16 * L * N * N + 16640 bytes <= NSPT_NOALLOC_SCRATCH_BYTES with L the transform length (N <= 104 at
+ * N_trunc = 31, N <= 73 at N_trunc = 63, N <= 208 at N_trunc = 7); larger problems return NSPT_ETOOBIG and touch nothing.
+ * All calls on one GPU share the array, and it keeps the last call's contents: nothing in it has to start from zero (every
+ * byte a call reads it has written before), but two calls that overlap on the GPU -- issued to different streams without an
+ * ordering between them, or from two host threads with different streams -- race on it.  Calls on one stream are safe.
+ */
+#define NSPT_NOALLOC_SCRATCH_BYTES (32u << 20)
+int nspt_series_mul_noalloc(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc);
 
 /*
  * The TEK staple for all four directions (eq. 2.3; eq. 2.2):

@@ -24,7 +24,7 @@ STAGES = {"fft_forward": 0, "zgemm_modes": 1, "fft_inverse": 2, "fft_retruncate"
           "int8_slicing": 6}
 
 EXPORTS = [
-    "nspt_series_mul", "nspt_series_mul_batched", "nspt_staple", "nspt_staple_dir", "nspt_series_exp", "nspt_series_exp_batched", "nspt_link_update", "nspt_link_update_batched", "nspt_force",
+    "nspt_series_mul", "nspt_series_mul_batched", "nspt_series_mul_noalloc", "nspt_staple", "nspt_staple_dir", "nspt_series_exp", "nspt_series_exp_batched", "nspt_link_update", "nspt_link_update_batched", "nspt_force",
     "nspt_series_mul_host", "nspt_series_mul_batched_host", "nspt_staple_host",
     "nspt_set_stream", "nspt_set_order_scale", "nspt_workspace_bytes", "nspt_set_workspace",
     "nspt_set_gemm_variant", "nspt_set_conv_algorithm", "nspt_probe_fp64_peak", "nspt_profile", "nspt_profile_read", "nspt_launch_count",
@@ -47,6 +47,7 @@ _lib = ctypes.CDLL(str(_LIB_PATH))
 _vp, _int, _dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
 _lib.nspt_series_mul.argtypes = [_vp, _vp, _vp, _int, _int]
 _lib.nspt_series_mul_batched.argtypes = [_vp, _vp, _vp, _int, _int, _int]
+_lib.nspt_series_mul_noalloc.argtypes = [_vp, _vp, _vp, _int, _int]
 _lib.nspt_staple.argtypes = [ctypes.POINTER(_vp), _vp, ctypes.POINTER(_vp), _int, _int]
 _lib.nspt_staple_dir.argtypes = [ctypes.POINTER(_vp), _vp, _int, _vp, _int, _int]
 _lib.nspt_series_exp.argtypes = [_vp, _vp, _int, _int]
@@ -140,6 +141,21 @@ def nspt_series_mul(A, B, C=None):
     _match(_dev_series(B, "B"), A, "B")
     _match(_dev_series(C, "C"), A, "C")
     _check(_lib.nspt_series_mul(A.data_ptr(), B.data_ptr(), C.data_ptr(), N, Ntrunc), "nspt_series_mul")
+    return C
+
+
+NSPT_NOALLOC_SCRATCH_BYTES = 32 << 20
+NSPT_ETOOBIG = -5
+
+
+def nspt_series_mul_noalloc(A, B, C):
+    """C = A * B with the scratch in the library's static device array: no allocation anywhere, so the caller passes C.
+    Raises NsptError (code NSPT_ETOOBIG) when 3 * 16 * L * N * N + 16640 bytes exceed NSPT_NOALLOC_SCRATCH_BYTES."""
+    A, B, C = _dev_series(A, "A"), _dev_series(B, "B"), _dev_series(C, "C")
+    _, Ntrunc, N = _shape(A, False)
+    _match(B, A, "B")
+    _match(C, A, "C")
+    _check(_lib.nspt_series_mul_noalloc(A.data_ptr(), B.data_ptr(), C.data_ptr(), N, Ntrunc), "nspt_series_mul_noalloc")
     return C
 
 

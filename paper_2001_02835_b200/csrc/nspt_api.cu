@@ -1070,12 +1070,122 @@ int staple_dir_device(const nspt_c128* const U[4], const nspt_c128 z[16], int mu
     return k_inverse(f, t, 1, St, Smu);
 }
 
+// ---- nspt_series_mul_noalloc: FFT-CONV with its frequency-domain scratch in a file-scope device array ----------------------
+// For callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the three spectra and
+// the per-L tables live in ONE static array of NSPT_NOALLOC_SCRATCH_BYTES that every GPU loading the library holds until exit.
+// Layout: [0, NOALLOC_TABLE_BYTES) tables (w^m, w^-m, s^k, s^-k / L), then A~, B~, C~ back to back and the 256-byte pad.
+// In host code `noalloc_scratch` is only a handle: the device address comes from cudaGetSymbolAddress, once per device with
+// that device current (noalloc_base), and that address is what the kernels of the other files receive.
+constexpr size_t NOALLOC_TABLE_BYTES = 16384;
+constexpr int NOALLOC_MAX_L = 256;   // = transform length at NSPT_MAX_NTRUNC
+static __device__ __align__(256) unsigned char noalloc_scratch[NSPT_NOALLOC_SCRATCH_BYTES];
+
+struct NoallocState {
+    unsigned char* base = nullptr;   // device address of noalloc_scratch on this device
+    int L = 0, n = 0;                // tables currently in the array
+    double s = 0.0;
+};
+NoallocState noalloc_state[MAX_DEVICES];
+// host copies of the tables (static: nothing is allocated per call); protected by the context lock of the calling device,
+// and cudaMemcpyAsync from pageable memory has staged its source before it returns
+struct NoallocHostTables {
+    double2 f[NOALLOC_MAX_L], b[NOALLOC_MAX_L];
+    double si[NSPT_MAX_NTRUNC + 1], so[NSPT_MAX_NTRUNC + 1];
+};
+NoallocHostTables noalloc_host[MAX_DEVICES];
+
+int noalloc_base(int dev, NoallocState** out) {
+    NoallocState& st = noalloc_state[dev];
+    if (!st.base) {
+        void* ptr = nullptr;
+        NSPT_CUDA(cudaGetSymbolAddress(&ptr, noalloc_scratch));
+        if (!ptr) return NSPT_ECUDA;
+        st.base = static_cast<unsigned char*>(ptr);
+    }
+    *out = &st;
+    return NSPT_OK;
+}
+
+// the tables of get_plan (same formulas, eqs. 2.7 / 2.9), written into the static array when (L, n, s) changed
+int noalloc_tables(int dev, NoallocState& st, int L, int n, double s, PlanTables* out) {
+    double2* d_f = reinterpret_cast<double2*>(st.base);
+    double2* d_b = d_f + NOALLOC_MAX_L;
+    double* d_si = reinterpret_cast<double*>(d_b + NOALLOC_MAX_L);
+    double* d_so = d_si + (NSPT_MAX_NTRUNC + 1);
+    static_assert(2 * NOALLOC_MAX_L * sizeof(double2) + 2 * (NSPT_MAX_NTRUNC + 1) * sizeof(double) <= NOALLOC_TABLE_BYTES, "table region");
+    if (st.L != L || st.n != n || st.s != s) {
+        NoallocHostTables& h = noalloc_host[dev];
+        const long double two_pi = 6.283185307179586476925286766559005768L;
+        for (int m = 0; m < L; ++m) {
+            const long double ang = two_pi * (long double)m / (long double)L;
+            double c = (double)cosl(ang), sn = (double)sinl(ang);
+            if ((4 * m) % L == 0) {   // multiples of pi/2: exact
+                const int q = (4 * m) / L;
+                c = (q == 0) ? 1.0 : (q == 2 ? -1.0 : 0.0);
+                sn = (q == 1) ? 1.0 : (q == 3 ? -1.0 : 0.0);
+            }
+            h.f[m] = make_double2(c, sn);
+            h.b[m] = make_double2(c, -sn);
+        }
+        for (int k = 0; k < n; ++k) {
+            h.si[k] = (double)powl((long double)s, (long double)k);
+            h.so[k] = (double)(powl((long double)s, -(long double)k) / (long double)L);
+        }
+        st.L = 0;   // not valid until all four copies are enqueued
+        NSPT_CUDA(cudaMemcpyAsync(d_f, h.f, sizeof(double2) * L, cudaMemcpyHostToDevice, g.stream));
+        NSPT_CUDA(cudaMemcpyAsync(d_b, h.b, sizeof(double2) * L, cudaMemcpyHostToDevice, g.stream));
+        NSPT_CUDA(cudaMemcpyAsync(d_si, h.si, sizeof(double) * n, cudaMemcpyHostToDevice, g.stream));
+        NSPT_CUDA(cudaMemcpyAsync(d_so, h.so, sizeof(double) * n, cudaMemcpyHostToDevice, g.stream));
+        st.L = L;
+        st.n = n;
+        st.s = s;
+    }
+    *out = PlanTables{d_f, d_b, s != 1.0 ? d_si : nullptr, d_so, 1.0 / L};
+    return NSPT_OK;
+}
+
+int series_mul_noalloc_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc) {
+    NSPT_TRY(check_dims(N, Ntrunc, 1));
+    if (!A || !B || !C || !aligned16(A) || !aligned16(B) || !aligned16(C)) return NSPT_EINVAL;
+    const FreqLayout f = make_layout(N, Ntrunc);
+    if (!fft_length_supported(f.L) || f.L > NOALLOC_MAX_L) return NSPT_EINVAL;
+    const size_t sb = spectrum_bytes(f, 1);
+    if (sb > NSPT_NOALLOC_SCRATCH_BYTES || NOALLOC_TABLE_BYTES + 3 * sb + WS_PAD > NSPT_NOALLOC_SCRATCH_BYTES) return NSPT_ETOOBIG;
+    NSPT_TRY(check_arch());
+    int dev = 0;
+    NSPT_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) return NSPT_EINVAL;
+    NoallocState* st = nullptr;
+    NSPT_TRY(noalloc_base(dev, &st));
+    PlanTables t;
+    NSPT_TRY(noalloc_tables(dev, *st, f.L, f.n, g.order_scale, &t));
+    unsigned char* ws = st->base + NOALLOC_TABLE_BYTES;
+    double* At = reinterpret_cast<double*>(ws);
+    double* Bt = reinterpret_cast<double*>(ws + sb);
+    double* Ct = reinterpret_cast<double*>(ws + 2 * sb);
+    // Every scratch byte a kernel reads has been written by this call: the forward pass writes both spectra completely
+    // (Steps 1-2), the product writes the third (Step 3); nothing has to start from zero.
+    g.used = true;
+    g.launches += 3;
+    NSPT_CUDA(launch_fft_forward(f, t, 1, A, At, B, Bt, g.stream));
+    GemmOut out;
+    out.C = Ct;
+    NSPT_CUDA(launch_zgemm_modes(f, 1, At, Bt, out, 1, g.stream));   // FP64 tensor pipe (the sizes that fit are below the INT8 range)
+    NSPT_CUDA(launch_fft_inverse(f, t, 1, Ct, C, g.stream));         // Steps 4-5
+    return NSPT_OK;
+}
+
 }  // namespace
 }  // namespace nspt
 
 using namespace nspt;
 
 extern "C" {
+
+int nspt_series_mul_noalloc(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc) {
+    NSPT_LOCK();
+    return series_mul_noalloc_device(A, B, C, N, Ntrunc);
+}
 
 int nspt_series_mul(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc) {
     NSPT_LOCK();
@@ -1332,6 +1442,9 @@ const char* nspt_strerror(int code) {
         case NSPT_ENOMEM: return "out of memory, or the caller's workspace is too small";
         case NSPT_ECUDA: return g.cuda_msg;
         case NSPT_EARCH: return "the current CUDA device is not compute capability 10.x (B200, sm_100a)";
+        case NSPT_ETOOBIG:
+            return "nspt_series_mul_noalloc: the problem needs more than the static scratch (3 * 16 * L * N * N + 16640 bytes "
+                   "must not exceed NSPT_NOALLOC_SCRATCH_BYTES); use nspt_series_mul";
         default: return "unknown error code";
     }
 }
