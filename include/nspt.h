@@ -190,7 +190,9 @@ int nspt_set_stream(void* cuda_stream);
 int nspt_set_order_scale(double s);
 
 /* Bytes of device workspace a call needs (op = NSPT_OP_SERIES_MUL or
- * NSPT_OP_SERIES_EXP with theirs, or NSPT_OP_STAPLE, batch ignored).  nspt_force needs none.  batch <= 65535. */
+ * NSPT_OP_SERIES_EXP with theirs, or NSPT_OP_STAPLE, batch ignored).  nspt_force needs none.  batch <= 65535.
+ * For NSPT_OP_SERIES_MUL this is what the general FFT-CONV needs: the one-launch forms the library takes for very small
+ * matrices (nspt_debug.h, nspt_set_conv_algorithm) use no workspace at all. */
 int nspt_workspace_bytes(int N, int Ntrunc, int batch, int op, size_t* out);
 
 /* Give the library a caller-owned device workspace (256-byte aligned).  Calls that need more

@@ -30,8 +30,11 @@ int nspt_set_gemm_variant(int variant);
 
 /* Select the convolution algorithm of nspt_series_mul[_batched]: 0 = automatic (default), 1 = FFT-CONV,
  * 2 = Naive-CONV (eq. 2.5 evaluated directly, one launch of the tensor-pipe kernel with the K dimension
- * concatenated over the order index; no transforms, no workspace).  Naive-CONV reads its inputs while it writes its
- * output, so a call whose output aliases an input uses FFT-CONV whatever is selected here. */
+ * concatenated over the order index; no transforms, no workspace), 3 = FFT-CONV fused into one launch (one CTA per output
+ * series, transforms and product in shared memory; only where both operand blocks fit: 2 N (L + 1) + 256 complex128 <= 200 KB;
+ * elsewhere the general FFT-CONV runs).  The automatic choice takes 2 for very low orders of small matrices and 3 while
+ * N^3 L <= 150000 (N = 12 at N_trunc = 31, N = 16 at N_trunc = 15).  Both read their inputs while they write their output, so a call whose output aliases an input uses the general
+ * FFT-CONV whatever is selected here. */
 int nspt_set_conv_algorithm(int algorithm);
 
 /* Per-stage device timing.  After nspt_profile(1) every kernel the library launches is

@@ -33,7 +33,7 @@ struct Context {
     bool used = false;                   // a kernel has been enqueued since the library was loaded / released
     double order_scale = 1.0;
     int gemm_variant = -1;               // nspt_debug.h: -1 = automatic
-    int conv_algorithm = 0;              // 0 = automatic, 1 = FFT-CONV, 2 = Naive-CONV (nspt_debug.h)
+    int conv_algorithm = 0;              // 0 = automatic, 1 = FFT-CONV, 2 = Naive-CONV, 3 = FFT-CONV in one launch (nspt_debug.h)
     bool arch_checked = false;
     // workspace
     void* user_ws = nullptr;
@@ -389,6 +389,12 @@ int k_gemm(const FreqLayout& f, int batch, const double* A, const double* B, dou
 // N^3 L plus three transform passes, but it is a single launch without workspace traffic: it wins where the product is
 // launch- or transform-bound (see DESIGN.md 5.5 for the measured crossover).  It reads A and B while it writes C, so an
 // output that aliases an input always takes FFT-CONV.
+// Automatic choice of the one-launch FFT-CONV: its N^2 CTAs each redo the transforms of 2N series, so its time grows like
+// N^3 L, against three launches (12.5 us through the binding) of the general path.  Measured per product (one B200, us, general /
+// one-launch): N = 8, N_trunc = 63: 12.7 / 9.8; N = 12, 31: 12.7 / 9.9; N = 16, 15: 12.6 / 9.2; N = 20, 7: 12.9 / 10.7;
+// N = 16, 31: 12.5 / 12.2; N = 12, 63: 12.5 / 13.1; N = 20, 15: 12.5 / 13.5; N = 24, 31: 13.5 / 29.3.
+constexpr double FUSED_SMALL_MAX_N3L = 150000.0;
+
 bool use_naive_conv(const FreqLayout& f, const nspt_c128* A, const nspt_c128* B, const nspt_c128* C) {
     if (C == A || C == B || g.gemm_variant == 0 || g.gemm_variant == 2 || g.gemm_variant == 4) return false;
     if (g.conv_algorithm == 1) return false;
@@ -400,6 +406,16 @@ bool use_naive_conv(const FreqLayout& f, const nspt_c128* A, const nspt_c128* B,
     if (f.N <= 32) return f.n <= 4;
     if (f.N <= 64) return f.n <= 2;
     return false;
+}
+
+// FFT-CONV in one launch (nspt_small.cu) where the general path is bound by its three launches.  Like Naive-CONV it reads
+// A and B while it writes C, so an aliased output takes the general path.
+bool use_fused_small(const FreqLayout& f, int batch, const nspt_c128* A, const nspt_c128* B, const nspt_c128* C) {
+    if (C == A || C == B || (g.gemm_variant != -1 && g.gemm_variant != 1)) return false;
+    if (!fused_small_eligible(f, batch)) return false;
+    if (g.conv_algorithm == 3) return true;
+    if (g.conv_algorithm != 0) return false;
+    return (double)f.N * f.N * f.N * f.L <= FUSED_SMALL_MAX_N3L;
 }
 
 int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc, int batch) {
@@ -417,6 +433,13 @@ int series_mul_device(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int 
     }
     PlanTables t;
     NSPT_TRY(get_plan(f.L, f.n, g.order_scale, &t));
+    if (use_fused_small(f, batch, A, B, C)) {
+        // Steps 1-4 in one launch, one CTA per output series (nspt_small.cu)
+        StageTimer tm;
+        NSPT_TRY(tm.begin(ST_GEMM));
+        NSPT_CUDA(launch_fused_small(f, t, batch, A, B, C, g.stream));
+        return tm.end();
+    }
     char* ws = nullptr;
     NSPT_TRY(get_workspace(ws_bytes_for(f, batch, NSPT_OP_SERIES_MUL), &ws, use_int8(f)));
     const size_t sb = spectrum_bytes(f, batch);
@@ -1369,7 +1392,7 @@ int nspt_set_gemm_variant(int variant) {
 
 int nspt_set_conv_algorithm(int algorithm) {
     NSPT_LOCK();
-    if (algorithm < 0 || algorithm > 2) return NSPT_EINVAL;
+    if (algorithm < 0 || algorithm > 3) return NSPT_EINVAL;
     g.conv_algorithm = algorithm;
     return NSPT_OK;
 }

@@ -132,6 +132,12 @@ cudaError_t launch_zgemm_groups(const FreqLayout& f, int batch, const GemmGroup*
 cudaError_t launch_naive_conv(const FreqLayout& f, int batch, const nspt_c128* A, const nspt_c128* B, nspt_c128* C,
                               cudaStream_t st);
 
+// FFT-CONV fused into one launch for small matrices (nspt_small.cu): one CTA per output series, everything in shared memory,
+// no workspace.  C must not alias A, B.
+bool fused_small_eligible(const FreqLayout& f, int batch);
+cudaError_t launch_fused_small(const FreqLayout& f, const PlanTables& t, int batch, const nspt_c128* A, const nspt_c128* B,
+                               nspt_c128* C, cudaStream_t st);
+
 // ---- mode-wise matrix product on the INT8 tensor cores (nspt_ozaki.cu) -----------------------------------------
 // FP64 spectra, whose per-mode maxima the transforms have recorded (maxbits), are cut into int8 slices (launch_ozaki_slice),
 // multiplied exactly by tcgen05.mma.kind::i8 and recombined in FP64 (launch_ozaki_gemm, same epilogues as launch_zgemm_groups).

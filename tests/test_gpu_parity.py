@@ -353,6 +353,58 @@ def test_both_convolution_algorithms_match_oracle(nspt, N, Ntrunc, alg):
         nspt.nspt_set_conv_algorithm(0)
 
 
+@pytest.mark.parametrize("N,Ntrunc", [(1, 1), (2, 3), (3, 2), (9, 7), (16, 31), (17, 1), (24, 63), (31, 12), (47, 3), (49, 31), (12, 127),
+                                      (97, 5)])
+def test_one_launch_fftconv_matches_oracle(nspt, N, Ntrunc):
+    # FFT-CONV fused into one launch (nspt_small.cu: one CTA per output series, radix-2 transforms in shared memory), forced
+    # wherever both operand blocks fit in shared memory; the order scale on for one shape
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([9, N, Ntrunc])
+    A = wl.gaussian_series(N, Ntrunc, rng)
+    B = wl.gaussian_series(N, Ntrunc, rng)
+    nspt.nspt_set_conv_algorithm(3)
+    nspt.nspt_profile(True)
+    try:
+        for name in nspt.STAGES:
+            nspt.nspt_profile_read(name)
+        if (N, Ntrunc) == (31, 12):
+            nspt.nspt_set_order_scale(0.8)
+        check_product(nspt, A, B)
+        launched = {name: nspt.nspt_profile_read(name)[1] for name in nspt.STAGES}
+    finally:
+        nspt.nspt_profile(False)
+        nspt.nspt_set_order_scale(1.0)
+        nspt.nspt_set_conv_algorithm(0)
+    assert launched["zgemm_modes"] == 1 and launched["fft_forward"] == 0 and launched["fft_inverse"] == 0, launched
+
+
+def test_one_launch_fftconv_batched_integer_and_automatic_choice(nspt):
+    import torch
+    import oracle
+    from paper_2001_02835_b200 import workloads as wl
+    rng = np.random.default_rng([10, 12, 31])
+    A = np.stack([wl.integer_series(12, 31, rng) for _ in range(5)])
+    B = np.stack([wl.integer_series(12, 31, rng) for _ in range(5)])
+    nspt.nspt_profile(True)
+    try:
+        nspt.nspt_profile_read("fft_forward")
+        C = nspt.nspt_series_mul_batched(to_dev(A), to_dev(B))       # the automatic choice (N^3 L <= 150000)
+        torch.cuda.synchronize()
+        assert nspt.nspt_profile_read("fft_forward")[1] == 0, "N = 12, N_trunc = 31 takes the one-launch kernel"
+        C = C.cpu().numpy()
+        for b in range(5):
+            ref = oracle.series_mul(A[b], B[b])
+            assert np.array_equal(np.round(C[b].real), ref.real) and np.array_equal(np.round(C[b].imag), ref.imag)
+        # an output that aliases an input takes the general path (the fused kernel reads A and B while it writes C)
+        dA, dB = to_dev(A[0]), to_dev(B[0])
+        nspt.nspt_series_mul(dA, dB, dA)
+        torch.cuda.synchronize()
+        assert nspt.nspt_profile_read("fft_forward")[1] == 1
+        assert np.array_equal(np.round(dA.cpu().numpy().real), oracle.series_mul(A[0], B[0]).real)
+    finally:
+        nspt.nspt_profile(False)
+
+
 def test_naive_conv_integer_bit_exact_batched_and_aliased(nspt):
     import torch
     import oracle
@@ -488,6 +540,7 @@ def test_caller_workspace(nspt):
     B = wl.gaussian_series(20, 7, rng)
     need = nspt.nspt_workspace_bytes(20, 7, 1, nspt.NSPT_OP_SERIES_MUL)
     ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    nspt.nspt_set_conv_algorithm(1)      # the general FFT-CONV: the one-launch forms this size would take need no workspace
     try:
         nspt.nspt_set_workspace(ws.data_ptr(), need)
         check_product(nspt, A, B)
@@ -495,7 +548,10 @@ def test_caller_workspace(nspt):
         with pytest.raises(nspt.NsptError) as ei:
             nspt.nspt_series_mul(to_dev(A), to_dev(B))
         assert ei.value.code == nspt.NSPT_ENOMEM
+        nspt.nspt_set_conv_algorithm(0)  # the automatic choice at this size is workspace-free: the short workspace does not matter
+        check_product(nspt, A, B)
     finally:
+        nspt.nspt_set_conv_algorithm(0)
         nspt.nspt_set_workspace(None, 0)
 
 
