@@ -633,10 +633,15 @@ def run_cuda(args):
             bf16 = peaks.get("bf16_tflops", 1630.0)
             int8_peak = 2.0 * bf16
             ach_i8 = int8_ops * K / (gemm["ms_total"] * 1e-3) * 1e-12
+            k_chunks = N // 32 if (N >= 64 and 0 < N % 32 <= 2) else -(-N // 32)
+            padded_ratio = (-(-N // 128) * 128) * (-(-N // 64) * 64) * (k_chunks * 32) / float(N) ** 3
             traffic = read_traffic(args.workload, "zgemm_modes_i8")
             line_extra["roofline"] = {
                 "bound": "tensor", "kernel": "zgemm_modes_i8_kernel (tcgen05.mma.kind::i8, TMEM accumulators; FP64 product emulated with 7 int8 slices per plane)",
                 "achieved": ach_i8, "peak": int8_peak, "unit": "TOP/s", "frac": ach_i8 / int8_peak, "traffic": traffic,
+                # what the tensor cores execute: tiles of 128 (j) x 64 (i) x 32 (k), K without the columns the FP64 tail takes
+                "achieved_executed": ach_i8 * padded_ratio, "frac_executed": ach_i8 * padded_ratio / int8_peak,
+                "executed_over_algorithmic": padded_ratio,
                 "flops_basis": "84 INT8 matrix products (28 slice pairs x 3 planes of the 3M complex product) of 2*N^3 ops per mode; tiles are padded to 128 x 64 x 32, the executed count is higher",
                 "peak_source": ("MEASURED_PEAKS.json bf16_tflops (burst) x 2 (nominal INT8 : bf16 ratio, B200_PROFILING.md)" if "bf16_tflops" in peaks
                                 else "fallback 1630 TFLOP/s bf16 x 2"),
