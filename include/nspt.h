@@ -109,6 +109,9 @@ int nspt_series_mul_batched(const nspt_c128* A, const nspt_c128* B, nspt_c128* C
  * All calls on one GPU share the array, and it keeps the last call's contents: nothing in it has to start from zero (every
  * byte a call reads it has written before), but two calls that overlap on the GPU -- issued to different streams without an
  * ordering between them, or from two host threads with different streams -- race on it.  Calls on one stream are safe.
+ * The first call on a device loads the kernels (CUDA lazy loading) and takes the array's address, and a call whose
+ * (N_trunc, order scale) differ from the previous call's copies 10 KB of tables from host memory first: under stream capture,
+ * make one call with the same shape before the capture begins.
  */
 #define NSPT_NOALLOC_SCRATCH_BYTES (32u << 20)
 int nspt_series_mul_noalloc(const nspt_c128* A, const nspt_c128* B, nspt_c128* C, int N, int Ntrunc);
