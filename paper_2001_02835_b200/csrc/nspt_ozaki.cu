@@ -602,6 +602,8 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
         // lane of the accumulator = output column j, column of the accumulator = output row i
         const int we = warp - 4, quarter = we & 3, half = we >> 2;
         int acc_it = 0;
+        uint64_t keep_policy;
+        asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(keep_policy));
         // What a tile needs from global memory before its first drain -- the exponents of its mode and, for the tail of K
         // (k >= 32 nkc, added in FP64), lane l's element A~[row0 + l][k] and its own column of B~[k][.] -- is fetched BEFORE the
         // stores of the tile before it: behind 131 KB of stores per SM these loads waited 2800 cycles on the critical path.
@@ -701,7 +703,10 @@ zgemm_modes_i8_kernel(const __grid_constant__ CUtensorMap mapM, const __grid_con
                     if (plain) {
 #pragma unroll
                         for (int j = 0; j < 32; ++j)   // the 32 lanes of a warp write 512 contiguous bytes of row row0 + j
-                            if (row0 + j < P.N) c[(size_t)(row0 + j) * P.N] = make_double2(sc * re[j], sc * im[j]);
+                            if (row0 + j < P.N) {
+                                double2* dst = &c[(size_t)(row0 + j) * P.N];
+                                asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(dst), "d"(sc * re[j]), "d"(sc * im[j]), "l"(keep_policy) : "memory");
+                            }
                     } else {
                         const double ar = sc * G.alpha_re, ai = sc * G.alpha_im;
 #pragma unroll
