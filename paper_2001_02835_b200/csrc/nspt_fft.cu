@@ -35,6 +35,7 @@
 // record max(|re|, |im|) of every mode they write -- a running maximum of the high words per thread,
 // one redux.sync and one atomicMax per mode and CTA at the end -- which is the scale of the fixed-point
 // slices of that mode.
+#include <cstdlib>
 #include <map>
 #include <mutex>
 
@@ -514,7 +515,11 @@ __global__ void __launch_bounds__(T* S, 1) fft_forward_tma_kernel(const __grid_c
         fence_proxy_async_smem();
         __syncthreads();
         if (threadIdx.x == 0) {
-            tma_store_3d(z ? &out1 : &out0, out_addr + ob * C::FULL_TILE_BYTES, (int)(2 * tx * T), 0, (int)b);
+            // INT8 path: the slicing pass reads the spectrum at once -- the lines written stay in the L2 as long as they can
+            if (track)
+                tma_store_3d_hint(z ? &out1 : &out0, out_addr + ob * C::FULL_TILE_BYTES, (int)(2 * tx * T), 0, (int)b, l2_keep_policy());
+            else
+                tma_store_3d(z ? &out1 : &out0, out_addr + ob * C::FULL_TILE_BYTES, (int)(2 * tx * T), 0, (int)b);
             tma_store_commit();
         }
     }
@@ -626,7 +631,10 @@ __global__ void __launch_bounds__(T* S) fft_inverse_tma_kernel(const __grid_cons
             fence_proxy_async_smem();
             __syncthreads();
             if (threadIdx.x == 0) {
-                tma_store_3d(&out_map, exch_addr, (int)(2 * tx * T), 0, (int)b);
+                if (track)
+                    tma_store_3d_hint(&out_map, exch_addr, (int)(2 * tx * T), 0, (int)b, l2_keep_policy());
+                else
+                    tma_store_3d(&out_map, exch_addr, (int)(2 * tx * T), 0, (int)b);
                 tma_store_commit();
             }
         } else {
