@@ -75,6 +75,15 @@ __device__ __forceinline__ void red_add(double2& dst, double2 v) {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&dst.y), "d"(v.y) : "memory");
 }
 
+__device__ __forceinline__ uint64_t l2_keep_policy() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void st_keep(double2& dst, double2 v, uint64_t policy) {
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(&dst), "d"(v.x), "d"(v.y), "l"(policy) : "memory");
+}
+
 struct GemmGroupDev {
     double2* C;   // direct target:   C(p)            (+)= alpha * A(p) B(p) + diag   (may be null)
     double2* D;   // daggered target: D((L-p) mod L)  (+)= beta * (A(p) B(p))^H       (may be null)
@@ -230,6 +239,7 @@ __device__ __forceinline__ void gemm_epilogue(const GemmParams& P, const GemmGro
     const double alpha_re = G.alpha_re, alpha_im = G.alpha_im, beta_re = G.beta_re, beta_im = G.beta_im;
     const int accumulate = G.accumulate, accumulate_d = G.accumulate_d;
     const double diag = G.diag;
+    const uint64_t keep = l2_keep_policy();
 #pragma unroll
     for (int bm = 0; bm < MB; ++bm) {
         const int m = m0 + mw + 8 * bm + g;
@@ -254,9 +264,9 @@ __device__ __forceinline__ void gemm_epilogue(const GemmParams& P, const GemmGro
                             // (deterministic), and nothing waits for the old value to come back from L2 / HBM
                             red_add(d[0], o0);
                             if (second) red_add(d[1], o1);
-                        } else {
-                            d[0] = o0;
-                            if (second) d[1] = o1;
+                        } else {   // the transform that follows reads this spectrum at once: the lines stay in the L2 while they can
+                            st_keep(d[0], o0, keep);
+                            if (second) st_keep(d[1], o1, keep);
                         }
                     }
                     if (Dm) {
