@@ -8,4 +8,4 @@ load the CUDA library; ``paper_2001_02835_b200.binding`` does, and fails loudly 
 missing -- there is no CPU fallback.
 """
 __all__ = ["workloads", "binding", "build", "parallel"]
-__version__ = "0.3.0"   # nspt_version() returns 300
+__version__ = "0.4.0"   # nspt_version() returns 400

@@ -1472,6 +1472,6 @@ const char* nspt_strerror(int code) {
     }
 }
 
-int nspt_version(void) { return 300; }
+int nspt_version(void) { return 400; }
 
 }  // extern "C"
